@@ -1,0 +1,177 @@
+/* wick.h -- C-ABI of the B200-native determinant-form Wick contraction (arXiv 2411.08962).
+ *
+ * PAPER.md = /root/reference/PAPER.md (text of the paper); line numbers refer to that file.
+ *
+ * The library computes the point-sink two-point correlator of a nucleus in the paper's
+ * "optimised determinant algorithm" (Sec. III; CUDA outline App. A, :616-663):
+ *
+ *     C(t,p) = sum_x e^{i p.x} sum_k w_k det U_x(t)[a_u(k), b_u(k)] det D_x(t)[a_d(k), b_d(k)]
+ *                                                              (Eq. 15, Eq. A1/A2 :630-635)
+ *
+ * U_x(t), D_x(t): 12x12 complex128 up / down propagators from the source to sink site x
+ * (row = sink spin-colour index chi = 3*spin + colour, column = source index; Eq. 13 :178).
+ * a, b: index tuples selecting n_u (n_d) of the 12 rows / columns.  The weighted term list comes
+ * from products of nucleon interpolators eps_abc (q1_a^T C gamma5 q2_b) q3_c,gamma (Eq. 4/5 :105-107).
+ *
+ * Two groups of entry points:
+ *   host  : wick_build_terms*, wick_terms_* -- the once-per-nucleus pre-processing (Sec. III B,
+ *           PAPER.md:209-246; App. C :704-732).  Pure CPU, no CUDA call.
+ *   device: wick_contract, wick_minor_dets, wick_contract_host -- the per-configuration hot path on
+ *           one sm_100a GPU.  There is NO CPU fallback: without a CUDA device they return
+ *           WICK_ERR_CUDA.
+ *
+ * Conventions: every function returns WICK_OK (0) or a negative WICK_ERR_* code and never throws;
+ * wick_last_error() gives a thread-local message for the last failure.  Complex numbers are
+ * interleaved (re, im) doubles.  "host" / "device" on a pointer says where the memory must live.
+ */
+#ifndef WICK_B200_H
+#define WICK_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define WICK_OK              0
+#define WICK_ERR_ARG        -1   /* bad argument: NULL pointer, index >= 12, n > 12, gamma > 3, L < 1 ... */
+#define WICK_ERR_UNSUPPORTED -2  /* legal but not implemented size / combination                         */
+#define WICK_ERR_WORKSPACE  -3   /* workspace smaller than wick_contract_min_workspace_bytes()            */
+#define WICK_ERR_CUDA       -4   /* CUDA runtime error (message holds cudaGetErrorString)                 */
+#define WICK_ERR_NOMEM      -5   /* host allocation failed                                                */
+
+/* wick_build_terms* flags */
+#define WICK_BUILD_IDENTITY_TEST 1u  /* run the randomised identity test (Sec. III B PAPER.md:234-246, App. C) */
+#define WICK_BUILD_ISOSPIN       2u  /* the caller promises U == D (m_u = m_d): the identity   */
+                                     /* test then evaluates both flavours on the SAME random matrix          */
+/* wick_contract flags */
+#define WICK_CONTRACT_FORCE_FLAT 1u  /* use the flat (uid, did, w) term list even if a factorised form exists */
+
+#define WICK_NUCLEON_PROTON  0
+#define WICK_NUCLEON_NEUTRON 1
+
+/* One nucleon of a product interpolator.  kind: 0 = proton  eps_abc (u_a^T C g5 d_b) u_{c,gamma},
+ * 1 = neutron eps_abc (d_a^T C g5 u_b) d_{c,gamma} (Eq. 4/5 PAPER.md:105-107; C = gamma4 gamma2 :76,
+ * Dirac-Pauli basis).  gamma = open Dirac index 0..3 (0,1 = upper components). */
+typedef struct { int32_t kind; int32_t gamma; } wick_nucleon;
+
+/* Opaque canonical term list + unique-minor tables (the paper's zeta_u, zeta_d, Theta of Eq. A1,
+ * PAPER.md:628-633, and the "lookup table" of :719).  Owned by the library; free with
+ * wick_terms_free.  Device copies of the tables are created lazily by the first device call and
+ * are released by wick_terms_free as well. */
+typedef struct wick_terms wick_terms;
+
+typedef struct {
+    int32_t n_u, n_d;                 /* minor sizes (quarks per flavour)                                   */
+    int32_t n_rows_u, n_cols_u;       /* distinct canonical row / column tuples of the u minors (|A_u|,|B_u|) */
+    int32_t n_rows_d, n_cols_d;
+    int64_t n_minors_u, n_minors_d;   /* unique minors per site = card(zeta_u), card(zeta_d)                */
+    int64_t n_terms;                  /* terms of the flat list                                             */
+    int32_t is_outer_product;         /* 1: terms = sink list x conj(source list), factorised form present  */
+    int32_t n_sink, n_source;         /* lengths of the factor lists (0 if not an outer product)            */
+    int64_t n_raw;                    /* raw terms consumed (24^A for nucleus specs, n_raw for lists)       */
+    int64_t n_identity_merged;        /* terms removed by the identity test (0 if it did not run)           */
+} wick_terms_info;
+
+/* ---------------------------------------------------------------------------------------------
+ * Host: term builder (steps a1, a2, a2' of DESIGN.md)
+ * ------------------------------------------------------------------------------------------- */
+
+/* Expand the ordered Grassmann product of `n_nucleons` nucleons (Eq. 9) in the exterior
+ * algebra, sort every monomial into canonical order (all u indices ascending, then all d indices
+ * ascending) with its permutation sign (Eq. 19, redundancy R.1), merge equal
+ * monomials, drop Pauli zeros and exact cancellations; then form the correlator term list
+ * w_ij = c_i conj(c_j) over (sink i, source j) (Eq. 15) and the unique-minor tables (R.2 :226).
+ * nucleons: host, [n_nucleons].  *out receives a new handle.  seed is used by the identity test only.
+ * Errors: WICK_ERR_ARG (NULL, n_nucleons < 1, kind not 0/1, gamma not 0..3, more than 12 quarks
+ * of one flavour), WICK_ERR_NOMEM. */
+int wick_build_terms(const wick_nucleon* nucleons, int n_nucleons, unsigned flags, uint64_t seed,
+                     wick_terms** out);
+
+/* Same canonicalisation for a user-supplied flat list (e.g. the seed-generated random list of
+ * BASELINE.json configs[4]).  a_u, b_u: host uint8 [n_raw][n_u]; a_d, b_d: host uint8 [n_raw][n_d];
+ * entries 0..11 in ANY order; a tuple with a repeated index is legal and contributes exactly 0
+ * (dropped).  w_reim: host double [n_raw][2].  Duplicate (a_u,b_u,a_d,b_d) are merged. */
+int wick_build_terms_from_list(int n_u, int n_d, int64_t n_raw,
+                               const uint8_t* a_u, const uint8_t* b_u,
+                               const uint8_t* a_d, const uint8_t* b_d,
+                               const double* w_reim, unsigned flags, uint64_t seed, wick_terms** out);
+
+int  wick_terms_get_info(const wick_terms* terms, wick_terms_info* info);
+
+/* Copy the tables out (host, caller-allocated; any pointer may be NULL to skip it).
+ * u_rows [n_rows_u][n_u], u_cols [n_cols_u][n_u], d_rows [n_rows_d][n_d], d_cols [n_cols_d][n_d]:
+ * ascending tuples, sorted lexicographically. */
+int  wick_terms_export_tuples(const wick_terms* terms, uint8_t* u_rows, uint8_t* u_cols,
+                              uint8_t* d_rows, uint8_t* d_cols);
+/* Unique minor m of flavour u is det U[u_rows[u_minor_row[m]], u_cols[u_minor_col[m]]].
+ * u_minor_row/col: int32 [n_minors_u]; d_*: int32 [n_minors_d]. */
+int  wick_terms_export_minors(const wick_terms* terms, int32_t* u_minor_row, int32_t* u_minor_col,
+                              int32_t* d_minor_row, int32_t* d_minor_col);
+/* Flat terms first .. first+count-1: uid, did int32 [count] (unique-minor ids), w_reim double [count][2]. */
+int  wick_terms_export_terms(const wick_terms* terms, int64_t first, int64_t count,
+                             int32_t* uid, int32_t* did, double* w_reim);
+/* Factor lists of an outer-product term list: sink i = (row tuple ids, c_i), source j = (column tuple
+ * ids, conj c_j); term (i,j) has uid = sink_ru[i]*n_cols_u + src_cu[j], did likewise, w = sink_c*src_c.
+ * Returns WICK_ERR_UNSUPPORTED if !is_outer_product. */
+int  wick_terms_export_factors(const wick_terms* terms, int32_t* sink_ru, int32_t* sink_rd, double* sink_c_reim,
+                               int32_t* src_cu, int32_t* src_cd, double* src_c_reim);
+void wick_terms_free(wick_terms* terms);
+
+/* ---------------------------------------------------------------------------------------------
+ * Device: the hot path (steps a3-a6 of DESIGN.md)
+ * ------------------------------------------------------------------------------------------- */
+
+/* Workspace sizes in bytes for wick_contract on a lattice of L^3 sites and T timeslices.
+ * _min: smallest legal workspace (one 32-site batch); _workspace_bytes: the recommended size
+ * (site batches of up to ~2 GiB of minors).  Any size >= _min is accepted; more lets the library use
+ * larger site batches.  Both return 0 on a bad argument. */
+size_t wick_contract_min_workspace_bytes(const wick_terms* terms, int L, int T, int n_mom);
+size_t wick_contract_workspace_bytes(const wick_terms* terms, int L, int T, int n_mom);
+
+/* C[p][t] = sum_x e^{+2 pi i (n_p . x)/L} sum_k w_k detU detD  for t = 0..T-1 (Eq. 15 / A1 / A2 / A7).
+ * U_dev, D_dev : device, complex128 [T][L^3][12][12], site s = x + L*(y + L*z), 16-byte aligned.
+ *                U_dev == D_dev is legal.
+ * momenta      : host, int32 [n_mom][3], integer units of 2*pi/L (read before the call returns).
+ * C_out_dev    : device, complex128 [n_mom][T].
+ * sigma_out_dev: NULL or device complex128 [T][L^3]: sigma(x,t) = sum_k w_k detU detD (Eq. A5 :646).
+ * workspace_dev: device, workspace_bytes >= wick_contract_min_workspace_bytes, 256-byte aligned.
+ * cuda_stream  : a cudaStream_t (NULL = default stream).  All work is enqueued on it; the call does
+ *                not synchronise (except for a one-time upload of the tables on first use of
+ *                `terms`).  Results are bit-reproducible run to run (no floating-point atomics;
+ *                fixed-shape reductions).
+ * Ownership: the caller owns every buffer; the library only keeps the tables inside `terms`. */
+int wick_contract(const void* U_dev, const void* D_dev, const wick_terms* terms,
+                  const int32_t* momenta, int n_mom, int L, int T,
+                  void* C_out_dev, void* sigma_out_dev,
+                  void* workspace_dev, size_t workspace_bytes, unsigned flags, void* cuda_stream);
+
+/* Same computation from HOST buffers (U_host, D_host, C_out_host, sigma_out_host: host memory,
+ * pinned or pageable, same layouts).  Allocates device memory itself, streams the propagators
+ * timeslice block by timeslice block (H2D overlapped with compute), copies C back
+ * and synchronises before returning. */
+int wick_contract_host(const void* U_host, const void* D_host, const wick_terms* terms,
+                       const int32_t* momenta, int n_mom, int L, int T,
+                       void* C_out_host, void* sigma_out_host, unsigned flags);
+
+/* Step a4 alone: unique minor determinants ("analytic up to 4x4, LU above"; device_det,
+ * App. A :648-652).  out[m][s] = det P_s[rows[m], cols[m]] for n_sites matrices.
+ * P_dev  : device complex128 [n_sites][12][12].
+ * rows, cols: host uint8 [n_minors][n], entries 0..11 (any order; no canonicalisation is applied).
+ * out_dev: device complex128 [n_minors][n_sites].  n = 0..12 (n = 0 gives 1).  Synchronises. */
+int wick_minor_dets(const void* P_dev, int64_t n_sites, int n, const uint8_t* rows, const uint8_t* cols,
+                    int64_t n_minors, void* out_dev, void* cuda_stream);
+
+/* Number of kernel launches issued by this thread's device calls since the last reset (bench.py's
+ * gpu_launches); _reset returns the old value. */
+int64_t wick_launch_count(void);
+int64_t wick_launch_count_reset(void);
+
+const char* wick_last_error(void);
+const char* wick_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* WICK_B200_H */

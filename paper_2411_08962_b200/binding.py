@@ -1,0 +1,262 @@
+"""Thin Python binding of the C-ABI in include/wick.h (ctypes; argument marshalling only).
+
+Every step of the path runs inside libwick_b200.so.  PyTorch appears only as the owner of device
+memory and streams (tensors are passed as raw pointers).  There is no CPU fallback: if the shared
+library is missing or has no CUDA device, the calls raise.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Optional, Sequence, Tuple
+
+import numpy as np
+
+_LIB_PATH = os.path.join(os.path.dirname(os.path.abspath(__file__)), "libwick_b200.so")
+_lib = None
+
+BUILD_IDENTITY_TEST = 1
+BUILD_ISOSPIN = 2
+CONTRACT_FORCE_FLAT = 1
+
+EXPORTED_SYMBOLS = (
+    "wick_build_terms", "wick_build_terms_from_list", "wick_terms_get_info", "wick_terms_export_tuples",
+    "wick_terms_export_minors", "wick_terms_export_terms", "wick_terms_export_factors", "wick_terms_free",
+    "wick_contract_min_workspace_bytes", "wick_contract_workspace_bytes", "wick_contract",
+    "wick_contract_host", "wick_minor_dets", "wick_launch_count", "wick_launch_count_reset",
+    "wick_last_error", "wick_version",
+)
+
+
+class WickError(RuntimeError):
+    pass
+
+
+class _Nucleon(C.Structure):
+    _fields_ = [("kind", C.c_int32), ("gamma", C.c_int32)]
+
+
+class TermsInfo(C.Structure):
+    _fields_ = [
+        ("n_u", C.c_int32), ("n_d", C.c_int32),
+        ("n_rows_u", C.c_int32), ("n_cols_u", C.c_int32), ("n_rows_d", C.c_int32), ("n_cols_d", C.c_int32),
+        ("n_minors_u", C.c_int64), ("n_minors_d", C.c_int64), ("n_terms", C.c_int64),
+        ("is_outer_product", C.c_int32), ("n_sink", C.c_int32), ("n_source", C.c_int32),
+        ("n_raw", C.c_int64), ("n_identity_merged", C.c_int64),
+    ]
+
+
+def library_path() -> str:
+    return _LIB_PATH
+
+
+def load_library():
+    """dlopen libwick_b200.so (built in-tree by paper_2411_08962_b200.build); raises if absent."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(_LIB_PATH):
+        raise WickError(f"{_LIB_PATH} is missing: run `python -m paper_2411_08962_b200.build` "
+                        "(there is no CPU fallback for the CUDA path)")
+    lib = C.CDLL(_LIB_PATH)
+    vp, i32, i64, u64, u32, sz = C.c_void_p, C.c_int, C.c_int64, C.c_uint64, C.c_uint, C.c_size_t
+    lib.wick_build_terms.argtypes = [C.POINTER(_Nucleon), i32, u32, u64, C.POINTER(vp)]
+    lib.wick_build_terms_from_list.argtypes = [i32, i32, i64, vp, vp, vp, vp, vp, u32, u64, C.POINTER(vp)]
+    lib.wick_terms_get_info.argtypes = [vp, C.POINTER(TermsInfo)]
+    lib.wick_terms_export_tuples.argtypes = [vp, vp, vp, vp, vp]
+    lib.wick_terms_export_minors.argtypes = [vp, vp, vp, vp, vp]
+    lib.wick_terms_export_terms.argtypes = [vp, i64, i64, vp, vp, vp]
+    lib.wick_terms_export_factors.argtypes = [vp, vp, vp, vp, vp, vp, vp]
+    lib.wick_terms_free.argtypes = [vp]
+    lib.wick_terms_free.restype = None
+    for f in (lib.wick_contract_min_workspace_bytes, lib.wick_contract_workspace_bytes):
+        f.argtypes = [vp, i32, i32, i32]
+        f.restype = sz
+    lib.wick_contract.argtypes = [vp, vp, vp, vp, i32, i32, i32, vp, vp, vp, sz, u32, vp]
+    lib.wick_contract_host.argtypes = [vp, vp, vp, vp, i32, i32, i32, vp, vp, u32]
+    lib.wick_minor_dets.argtypes = [vp, i64, i32, vp, vp, i64, vp, vp]
+    lib.wick_launch_count.restype = i64
+    lib.wick_launch_count_reset.restype = i64
+    lib.wick_last_error.restype = C.c_char_p
+    lib.wick_version.restype = C.c_char_p
+    _lib = lib
+    return lib
+
+
+def _check(rc: int, what: str):
+    if rc != 0:
+        raise WickError(f"{what} failed ({rc}): {load_library().wick_last_error().decode()}")
+
+
+def _np_ptr(a: Optional[np.ndarray]):
+    return None if a is None else a.ctypes.data_as(C.c_void_p)
+
+
+class Terms:
+    """Handle of a canonical term list + unique-minor tables (wick_terms*)."""
+
+    def __init__(self, handle):
+        self._h = C.c_void_p(handle)
+        info = TermsInfo()
+        _check(load_library().wick_terms_get_info(self._h, C.byref(info)), "wick_terms_get_info")
+        self.info = info
+
+    def __del__(self):
+        h, self._h = getattr(self, "_h", None), None
+        if h and _lib is not None:
+            _lib.wick_terms_free(h)
+
+    # -- exports (host numpy arrays) --
+    def tuples(self):
+        i = self.info
+        out = [np.zeros((i.n_rows_u, i.n_u), np.uint8), np.zeros((i.n_cols_u, i.n_u), np.uint8),
+               np.zeros((i.n_rows_d, i.n_d), np.uint8), np.zeros((i.n_cols_d, i.n_d), np.uint8)]
+        _check(_lib.wick_terms_export_tuples(self._h, *[_np_ptr(a) for a in out]), "wick_terms_export_tuples")
+        return tuple(out)
+
+    def minors(self):
+        i = self.info
+        out = [np.zeros(i.n_minors_u, np.int32), np.zeros(i.n_minors_u, np.int32),
+               np.zeros(i.n_minors_d, np.int32), np.zeros(i.n_minors_d, np.int32)]
+        _check(_lib.wick_terms_export_minors(self._h, *[_np_ptr(a) for a in out]), "wick_terms_export_minors")
+        return tuple(out)
+
+    def terms(self, first: int = 0, count: Optional[int] = None):
+        count = self.info.n_terms - first if count is None else count
+        uid, did = np.zeros(count, np.int32), np.zeros(count, np.int32)
+        w = np.zeros(count, np.complex128)
+        _check(_lib.wick_terms_export_terms(self._h, first, count, _np_ptr(uid), _np_ptr(did), _np_ptr(w)),
+               "wick_terms_export_terms")
+        return uid, did, w
+
+    def factors(self):
+        i = self.info
+        sru, srd = np.zeros(i.n_sink, np.int32), np.zeros(i.n_sink, np.int32)
+        qcu, qcd = np.zeros(i.n_source, np.int32), np.zeros(i.n_source, np.int32)
+        sc, qc = np.zeros(i.n_sink, np.complex128), np.zeros(i.n_source, np.complex128)
+        _check(_lib.wick_terms_export_factors(self._h, _np_ptr(sru), _np_ptr(srd), _np_ptr(sc),
+                                              _np_ptr(qcu), _np_ptr(qcd), _np_ptr(qc)), "wick_terms_export_factors")
+        return sru, srd, sc, qcu, qcd, qc
+
+    def term_tuples(self, first: int = 0, count: Optional[int] = None):
+        """Flat terms as index tuples (a_u, b_u, a_d, b_d, w) -- what an oracle consumes."""
+        ur, uc, dr, dc = self.tuples()
+        umr, umc, dmr, dmc = self.minors()
+        uid, did, w = self.terms(first, count)
+        return ur[umr[uid]], uc[umc[uid]], dr[dmr[did]], dc[dmc[did]], w
+
+
+def build_terms(nucleus: Sequence[Tuple[str, int]], flags: int = 0, seed: int = 0) -> Terms:
+    """nucleus: sequence of ('p' | 'n', gamma) in product order -> canonical term list."""
+    lib = load_library()
+    arr = (_Nucleon * max(len(nucleus), 1))()
+    for k, (kind, gamma) in enumerate(nucleus):
+        if kind not in ("p", "n"):
+            raise WickError(f"nucleon kind must be 'p' or 'n', got {kind!r}")
+        arr[k].kind = 0 if kind == "p" else 1
+        arr[k].gamma = int(gamma)
+    h = C.c_void_p()
+    _check(lib.wick_build_terms(arr, len(nucleus), flags, seed, C.byref(h)), "wick_build_terms")
+    return Terms(h.value)
+
+
+def build_terms_from_list(a_u, b_u, a_d, b_d, w, flags: int = 0, seed: int = 0) -> Terms:
+    lib = load_library()
+    a_u, b_u, a_d, b_d = (np.ascontiguousarray(x, dtype=np.uint8) for x in (a_u, b_u, a_d, b_d))
+    w = np.ascontiguousarray(w, dtype=np.complex128)
+    n_raw = len(w)
+    n_u = a_u.shape[1] if a_u.ndim == 2 else 0
+    n_d = a_d.shape[1] if a_d.ndim == 2 else 0
+    h = C.c_void_p()
+    _check(lib.wick_build_terms_from_list(n_u, n_d, n_raw, _np_ptr(a_u), _np_ptr(b_u), _np_ptr(a_d), _np_ptr(b_d),
+                                          _np_ptr(w), flags, seed, C.byref(h)), "wick_build_terms_from_list")
+    return Terms(h.value)
+
+
+def _stream_ptr(stream):
+    import torch
+    s = torch.cuda.current_stream() if stream is None else stream
+    return C.c_void_p(s.cuda_stream)
+
+
+def _check_dev(t, name, shape=None):
+    import torch
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.complex128 and t.is_contiguous()):
+        raise WickError(f"{name} must be a contiguous CUDA complex128 tensor")
+    if shape is not None and tuple(t.shape) != tuple(shape):
+        raise WickError(f"{name} must have shape {tuple(shape)}, got {tuple(t.shape)}")
+
+
+def contract_workspace_bytes(terms: Terms, L: int, T: int, n_mom: int, minimum: bool = False) -> int:
+    lib = load_library()
+    f = lib.wick_contract_min_workspace_bytes if minimum else lib.wick_contract_workspace_bytes
+    return int(f(terms._h, L, T, n_mom))
+
+
+def contract(U, D, terms: Terms, momenta, L: int, T: int, workspace=None, want_sigma: bool = False,
+             flags: int = 0, stream=None, out=None):
+    """C[p][t] on the device (wick_contract).  U, D: CUDA complex128 [T][L^3][12][12].
+    Returns C (CUDA complex128 [n_mom][T]) or (C, sigma [T][L^3]) if want_sigma."""
+    import torch
+    lib = load_library()
+    V = L ** 3
+    _check_dev(U, "U", (T, V, 12, 12))
+    _check_dev(D, "D", (T, V, 12, 12))
+    mom = np.ascontiguousarray(momenta, dtype=np.int32).reshape(-1, 3)
+    n_mom = mom.shape[0]
+    if workspace is None:
+        workspace = torch.empty(contract_workspace_bytes(terms, L, T, n_mom), dtype=torch.uint8, device=U.device)
+    Cout = torch.empty((n_mom, T), dtype=torch.complex128, device=U.device) if out is None else out
+    sigma = torch.empty((T, V), dtype=torch.complex128, device=U.device) if want_sigma else None
+    with torch.cuda.device(U.device):
+        rc = lib.wick_contract(U.data_ptr(), D.data_ptr(), terms._h, _np_ptr(mom), n_mom, L, T, Cout.data_ptr(),
+                               None if sigma is None else sigma.data_ptr(), workspace.data_ptr(),
+                               workspace.numel() * workspace.element_size(), flags, _stream_ptr(stream))
+    _check(rc, "wick_contract")
+    return (Cout, sigma) if want_sigma else Cout
+
+
+def contract_host(U: np.ndarray, D: np.ndarray, terms: Terms, momenta, L: int, T: int, want_sigma: bool = False,
+                  flags: int = 0):
+    """Same from HOST arrays (numpy complex128 or pinned torch CPU tensors); copies are inside the call."""
+    lib = load_library()
+    V = L ** 3
+
+    def host_ptr(a, name):
+        if isinstance(a, np.ndarray):
+            if a.dtype != np.complex128 or not a.flags.c_contiguous or a.shape != (T, V, 12, 12):
+                raise WickError(f"{name} must be a C-contiguous complex128 array [T][L^3][12][12]")
+            return a.ctypes.data_as(C.c_void_p)
+        if tuple(a.shape) != (T, V, 12, 12) or not a.is_contiguous() or a.is_cuda:
+            raise WickError(f"{name} must be a contiguous CPU complex128 tensor [T][L^3][12][12]")
+        return C.c_void_p(a.data_ptr())
+
+    mom = np.ascontiguousarray(momenta, dtype=np.int32).reshape(-1, 3)
+    Cout = np.zeros((mom.shape[0], T), np.complex128)
+    sigma = np.zeros((T, V), np.complex128) if want_sigma else None
+    rc = lib.wick_contract_host(host_ptr(U, "U"), host_ptr(D, "D"), terms._h, _np_ptr(mom), mom.shape[0], L, T,
+                                _np_ptr(Cout), _np_ptr(sigma), flags)
+    _check(rc, "wick_contract_host")
+    return (Cout, sigma) if want_sigma else Cout
+
+
+def minor_dets(P, rows, cols, stream=None):
+    """Step a4 alone: out[m][s] = det P[s][rows[m], cols[m]].  P: CUDA complex128 [n_sites][12][12]."""
+    import torch
+    lib = load_library()
+    _check_dev(P, "P")
+    rows = np.ascontiguousarray(rows, dtype=np.uint8)
+    cols = np.ascontiguousarray(cols, dtype=np.uint8)
+    n_minors, n = rows.shape
+    n_sites = P.shape[0]
+    out = torch.empty((n_minors, n_sites), dtype=torch.complex128, device=P.device)
+    with torch.cuda.device(P.device):
+        rc = lib.wick_minor_dets(P.data_ptr(), n_sites, n, _np_ptr(rows), _np_ptr(cols), n_minors, out.data_ptr(),
+                                 _stream_ptr(stream))
+    _check(rc, "wick_minor_dets")
+    return out
+
+
+def launch_count(reset: bool = False) -> int:
+    lib = load_library()
+    return int(lib.wick_launch_count_reset() if reset else lib.wick_launch_count())

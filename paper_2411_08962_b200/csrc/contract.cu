@@ -1,0 +1,407 @@
+// C-ABI device entry points: wick_contract, wick_contract_host, wick_minor_dets (include/wick.h).
+// Host logic only: table upload, workspace carving, site batching and kernel launch order.
+// Every arithmetic step of the path runs in the kernels of kernels.cu.
+#include <algorithm>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "kernels.cuh"
+#include "wick_internal.h"
+
+using namespace wick;
+
+namespace {
+
+inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+#define WICK_CUDA(call)                                                                      \
+    do {                                                                                     \
+        cudaError_t e_ = (call);                                                             \
+        if (e_ != cudaSuccess) {                                                             \
+            set_error(std::string(#call) + ": " + cudaGetErrorString(e_));                   \
+            return WICK_ERR_CUDA;                                                            \
+        }                                                                                    \
+    } while (0)
+
+int ensure_configured() {
+    static thread_local int configured_device = -1;
+    int dev = -1;
+    WICK_CUDA(cudaGetDevice(&dev));
+    if (configured_device != dev) {
+        WICK_CUDA(configure_kernels());
+        configured_device = dev;
+    }
+    return WICK_OK;
+}
+
+struct BlobBuilder {
+    std::vector<unsigned char> host;
+    size_t add(const void* src, size_t bytes) {
+        const size_t off = align_up(host.size(), 256);
+        host.resize(off + bytes);
+        if (bytes) std::memcpy(host.data() + off, src, bytes);
+        return off;
+    }
+};
+
+// tuple table -> [n][16] bytes: scale * index, zero padded
+std::vector<uint8_t> elem_table(const std::vector<uint16_t>& masks, int scale) {
+    std::vector<uint8_t> out(masks.size() * 16, 0);
+    for (size_t i = 0; i < masks.size(); ++i) {
+        int k = 0;
+        for (int b = 0; b < 12; ++b)
+            if (masks[i] & (1u << b)) out[i * 16 + k++] = uint8_t(b * scale);
+    }
+    return out;
+}
+
+// Upload minor tables and factor lists once per handle and device.
+int upload_tables(const wick_terms* t, cudaStream_t stream) {
+    std::lock_guard<std::mutex> lock(t->mu);
+    int dev = -1;
+    WICK_CUDA(cudaGetDevice(&dev));
+    DeviceTables& d = t->dev;
+    if (d.blob && d.device == dev) return WICK_OK;
+    if (d.blob) { set_error("wick_terms handle was first used on another device"); return WICK_ERR_ARG; }
+    BlobBuilder bb;
+    size_t o_row[2], o_col[2], o_rc[2];
+    for (int f = 0; f < 2; ++f) {
+        const FlavourTables& ft = t->f[f];
+        if (ft.rows.size() > 65535 || ft.cols.size() > 65535) { set_error("more than 65535 distinct tuples"); return WICK_ERR_UNSUPPORTED; }
+        std::vector<uint8_t> re = elem_table(ft.rows, 12), ce = elem_table(ft.cols, 1);
+        std::vector<uint32_t> rc(ft.minor_row.size());
+        for (size_t m = 0; m < rc.size(); ++m) rc[m] = uint32_t(ft.minor_row[m]) | (uint32_t(ft.minor_col[m]) << 16);
+        o_row[f] = bb.add(re.data(), re.size());
+        o_col[f] = bb.add(ce.data(), ce.size());
+        o_rc[f] = bb.add(rc.data(), rc.size() * 4);
+    }
+    size_t o_sp = 0, o_srd = 0, o_sc = 0, o_qp = 0, o_qcu = 0, o_qc = 0;
+    if (t->outer) {
+        const int nru = int(t->f[0].rows.size()), ncd = int(t->f[1].cols.size());
+        // sink is sorted by (ru, rd): CSR over ru
+        std::vector<int32_t> sp(nru + 1, 0), srd(t->sink.size());
+        std::vector<double> sc(2 * t->sink.size());
+        for (size_t i = 0; i < t->sink.size(); ++i) {
+            sp[t->sink[i].qu + 1]++;
+            srd[i] = t->sink[i].qd;
+            sc[2 * i] = t->sink[i].c.real(); sc[2 * i + 1] = t->sink[i].c.imag();
+        }
+        int mx = 0;
+        for (int r = 0; r < nru; ++r) { mx = std::max(mx, sp[r + 1]); sp[r + 1] += sp[r]; }
+        d.max_sink_per_row = mx;
+        // source sorted by (cd, cu): CSR over cd
+        std::vector<FactorTerm> src = t->source;
+        std::stable_sort(src.begin(), src.end(), [](const FactorTerm& a, const FactorTerm& b) {
+            return a.qd != b.qd ? a.qd < b.qd : a.qu < b.qu; });
+        std::vector<int32_t> qp(ncd + 1, 0), qcu(src.size());
+        std::vector<double> qc(2 * src.size());
+        for (size_t j = 0; j < src.size(); ++j) {
+            qp[src[j].qd + 1]++;
+            qcu[j] = src[j].qu;
+            qc[2 * j] = src[j].c.real(); qc[2 * j + 1] = src[j].c.imag();
+        }
+        for (int c = 0; c < ncd; ++c) qp[c + 1] += qp[c];
+        o_sp = bb.add(sp.data(), sp.size() * 4); o_srd = bb.add(srd.data(), srd.size() * 4); o_sc = bb.add(sc.data(), sc.size() * 8);
+        o_qp = bb.add(qp.data(), qp.size() * 4); o_qcu = bb.add(qcu.data(), qcu.size() * 4); o_qc = bb.add(qc.data(), qc.size() * 8);
+    }
+    void* blob = nullptr;
+    WICK_CUDA(cudaMalloc(&blob, std::max<size_t>(bb.host.size(), 256)));
+    cudaError_t e = cudaMemcpyAsync(blob, bb.host.data(), bb.host.size(), cudaMemcpyHostToDevice, stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(stream);   // bb.host dies at scope exit
+    if (e != cudaSuccess) { cudaFree(blob); set_error(std::string("table upload: ") + cudaGetErrorString(e)); return WICK_ERR_CUDA; }
+    unsigned char* b = static_cast<unsigned char*>(blob);
+    for (int f = 0; f < 2; ++f) {
+        d.row_elem[f] = b + o_row[f];
+        d.col_elem[f] = b + o_col[f];
+        d.minor_rc[f] = reinterpret_cast<const uint32_t*>(b + o_rc[f]);
+    }
+    if (t->outer) {
+        d.sink_ptr = reinterpret_cast<const int32_t*>(b + o_sp);
+        d.sink_rd = reinterpret_cast<const int32_t*>(b + o_srd);
+        d.sink_c = reinterpret_cast<const double*>(b + o_sc);
+        d.src_ptr = reinterpret_cast<const int32_t*>(b + o_qp);
+        d.src_cu = reinterpret_cast<const int32_t*>(b + o_qcu);
+        d.src_c = reinterpret_cast<const double*>(b + o_qc);
+    }
+    d.blob = blob;
+    d.device = dev;
+    return WICK_OK;
+}
+
+int upload_flat(const wick_terms* t, cudaStream_t stream) {
+    try { t->ensure_flat(); } catch (const std::bad_alloc&) { set_error("flat term list: out of host memory"); return WICK_ERR_NOMEM; }
+    std::lock_guard<std::mutex> lock(t->mu);
+    DeviceTables& d = t->dev;
+    if (d.flat_blob) return WICK_OK;
+    const size_t n = size_t(t->n_terms);
+    const size_t o_uid = 0, o_did = align_up(n * 4, 256), o_w = o_did + align_up(n * 4, 256);
+    const size_t bytes = o_w + n * 16;
+    void* blob = nullptr;
+    WICK_CUDA(cudaMalloc(&blob, std::max<size_t>(bytes, 256)));
+    unsigned char* b = static_cast<unsigned char*>(blob);
+    cudaError_t e = cudaSuccess;
+    if (n) {
+        e = cudaMemcpyAsync(b + o_uid, t->t_uid.data(), n * 4, cudaMemcpyHostToDevice, stream);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(b + o_did, t->t_did.data(), n * 4, cudaMemcpyHostToDevice, stream);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(b + o_w, t->t_w.data(), n * 16, cudaMemcpyHostToDevice, stream);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(stream);
+    }
+    if (e != cudaSuccess) { cudaFree(blob); set_error(std::string("flat list upload: ") + cudaGetErrorString(e)); return WICK_ERR_CUDA; }
+    d.flat_blob = blob;
+    d.t_uid = reinterpret_cast<const int32_t*>(b + o_uid);
+    d.t_did = reinterpret_cast<const int32_t*>(b + o_did);
+    d.t_w = reinterpret_cast<const double*>(b + o_w);
+    return WICK_OK;
+}
+
+// ---- workspace plan --------------------------------------------------------------------------
+constexpr int MAX_CHUNKS = 256;                  // rows of the partial buffer
+constexpr size_t TARGET_MINOR_BYTES = size_t(2) << 30;
+
+struct Plan {
+    int64_t n_st = 0;                            // site-times T * L^3
+    int64_t per_st = 0;                          // bytes of minors + partials per site-time
+    size_t sigma_bytes = 0;
+    int64_t S_b = 0;                             // site-times per batch (multiple of 32)
+};
+
+bool make_plan(const wick_terms* t, int L, int T, int n_mom, size_t workspace_bytes, bool want_max, Plan* p) {
+    if (!t || L < 1 || T < 1 || n_mom < 0 || int64_t(L) * L * L > (int64_t(1) << 31) - 1) return false;
+    p->n_st = int64_t(T) * L * L * L;
+    const int64_t nm = int64_t(t->f[0].minor_row.size()) + int64_t(t->f[1].minor_row.size());
+    p->per_st = (nm + MAX_CHUNKS) * 16;
+    p->sigma_bytes = align_up(size_t(p->n_st) * 16, 256);
+    const int64_t n_st_pad = (p->n_st + GROUP - 1) / GROUP * GROUP;
+    int64_t sb;
+    if (want_max) {
+        sb = int64_t(TARGET_MINOR_BYTES / size_t(p->per_st)) / GROUP * GROUP;
+    } else {
+        if (workspace_bytes < p->sigma_bytes + 1024) { p->S_b = 0; return true; }
+        sb = int64_t((workspace_bytes - p->sigma_bytes - 1024) / size_t(p->per_st)) / GROUP * GROUP;
+    }
+    sb = std::min<int64_t>(sb, n_st_pad);
+    sb = std::min<int64_t>(sb, int64_t(1) << 22);             // keeps grid.x and 32-bit site offsets small
+    if (want_max) sb = std::max<int64_t>(sb, GROUP);
+    p->S_b = sb;
+    return true;
+}
+
+size_t plan_bytes(const Plan& p, int64_t S_b) { return p.sigma_bytes + 1024 + size_t(S_b) * size_t(p.per_st); }
+
+}  // namespace
+
+extern "C" void wick_terms_release_device(DeviceTables* d) {
+    if (d->blob) cudaFree(d->blob);
+    if (d->flat_blob) cudaFree(d->flat_blob);
+    *d = DeviceTables();
+}
+
+extern "C" int64_t wick_launch_count(void) { return launch_counter_get(); }
+extern "C" int64_t wick_launch_count_reset(void) { return launch_counter_reset(); }
+
+extern "C" size_t wick_contract_min_workspace_bytes(const wick_terms* t, int L, int T, int n_mom) {
+    Plan p;
+    if (!make_plan(t, L, T, n_mom, 0, true, &p)) return 0;
+    return plan_bytes(p, GROUP);
+}
+
+extern "C" size_t wick_contract_workspace_bytes(const wick_terms* t, int L, int T, int n_mom) {
+    Plan p;
+    if (!make_plan(t, L, T, n_mom, 0, true, &p)) return 0;
+    return plan_bytes(p, p.S_b);
+}
+
+extern "C" int wick_contract(const void* U_dev, const void* D_dev, const wick_terms* t, const int32_t* momenta,
+                             int n_mom, int L, int T, void* C_out_dev, void* sigma_out_dev, void* workspace_dev,
+                             size_t workspace_bytes, unsigned flags, void* cuda_stream) {
+    if (!U_dev || !D_dev || !t || !C_out_dev || !workspace_dev || (n_mom > 0 && !momenta)) {
+        set_error("wick_contract: NULL argument"); return WICK_ERR_ARG; }
+    if ((reinterpret_cast<uintptr_t>(U_dev) | reinterpret_cast<uintptr_t>(D_dev) | reinterpret_cast<uintptr_t>(C_out_dev) |
+         reinterpret_cast<uintptr_t>(sigma_out_dev)) & 15) { set_error("wick_contract: buffers must be 16-byte aligned"); return WICK_ERR_ARG; }
+    if (reinterpret_cast<uintptr_t>(workspace_dev) & 255) { set_error("wick_contract: workspace must be 256-byte aligned"); return WICK_ERR_ARG; }
+    Plan p;
+    if (!make_plan(t, L, T, n_mom, workspace_bytes, false, &p)) { set_error("wick_contract: need L >= 1, T >= 1, n_mom >= 0"); return WICK_ERR_ARG; }
+    if (p.S_b < GROUP) { set_error("wick_contract: workspace smaller than wick_contract_min_workspace_bytes()"); return WICK_ERR_WORKSPACE; }
+    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    int rc = ensure_configured();
+    if (rc != WICK_OK) return rc;
+    if ((rc = upload_tables(t, stream)) != WICK_OK) return rc;
+    const bool use_outer = t->outer && !(flags & WICK_CONTRACT_FORCE_FLAT);
+    if (!use_outer && (rc = upload_flat(t, stream)) != WICK_OK) return rc;
+
+    const DeviceTables& d = t->dev;
+    const int64_t nmu = int64_t(t->f[0].minor_row.size()), nmd = int64_t(t->f[1].minor_row.size());
+    const int S_b = int(p.S_b);
+    unsigned char* ws = static_cast<unsigned char*>(workspace_dev);
+    double2* sigma = reinterpret_cast<double2*>(ws);
+    double2* MU = reinterpret_cast<double2*>(ws + p.sigma_bytes);          // sigma_bytes is a multiple of 256
+    double2* MD = MU + nmu * S_b;
+    double2* partial = MD + nmd * S_b;
+    const double2* U = static_cast<const double2*>(U_dev);
+    const double2* D = static_cast<const double2*>(D_dev);
+
+    for (int64_t st0 = 0; st0 < p.n_st; st0 += S_b) {
+        const int64_t n_valid = std::min<int64_t>(S_b, p.n_st - st0);
+        const int n_groups = int((n_valid + GROUP - 1) / GROUP);
+        WICK_CUDA(launch_minors(t->n_u, U, st0, p.n_st, n_groups, S_b, d.row_elem[0], d.col_elem[0], d.minor_rc[0], nmu, MU, stream));
+        WICK_CUDA(launch_minors(t->n_d, D, st0, p.n_st, n_groups, S_b, d.row_elem[1], d.col_elem[1], d.minor_rc[1], nmd, MD, stream));
+        int n_chunks = 1;
+        if (t->n_terms == 0) {
+            WICK_CUDA(cudaMemsetAsync(sigma + st0, 0, size_t(n_valid) * 16, stream));
+        } else {
+            if (use_outer) {
+                WICK_CUDA(launch_reduce_outer(MU, MD, n_groups, S_b, int(t->f[0].rows.size()), int(t->f[0].cols.size()),
+                                              int(t->f[1].cols.size()), d.sink_ptr, d.sink_rd,
+                                              reinterpret_cast<const double2*>(d.sink_c), d.src_ptr, d.src_cu,
+                                              reinterpret_cast<const double2*>(d.src_c), partial, &n_chunks, MAX_CHUNKS, stream));
+            } else {
+                WICK_CUDA(launch_reduce_flat(MU, MD, n_groups, S_b, d.t_uid, d.t_did, reinterpret_cast<const double2*>(d.t_w),
+                                             t->n_terms, partial, &n_chunks, MAX_CHUNKS, stream));
+            }
+            WICK_CUDA(launch_finalize_sigma(partial, n_chunks, S_b, n_valid, sigma + st0, stream));
+        }
+    }
+    for (int m0 = 0; m0 < n_mom; m0 += MAX_MOMENTA) {
+        MomentumList ml;
+        ml.n = std::min(MAX_MOMENTA, n_mom - m0);
+        for (int k = 0; k < ml.n; ++k)
+            for (int c = 0; c < 3; ++c) ml.v[k][c] = momenta[3 * (m0 + k) + c];
+        WICK_CUDA(launch_project(sigma, L, T, ml, static_cast<double2*>(C_out_dev) + int64_t(m0) * T, stream));
+    }
+    if (sigma_out_dev)
+        WICK_CUDA(cudaMemcpyAsync(sigma_out_dev, sigma, size_t(p.n_st) * 16, cudaMemcpyDeviceToDevice, stream));
+    return WICK_OK;
+}
+
+extern "C" int wick_contract_host(const void* U_host, const void* D_host, const wick_terms* t, const int32_t* momenta,
+                                  int n_mom, int L, int T, void* C_out_host, void* sigma_out_host, unsigned flags) {
+    if (!U_host || !D_host || !t || !C_out_host || (n_mom > 0 && !momenta) || L < 1 || T < 1 || n_mom < 0) {
+        set_error("wick_contract_host: bad argument"); return WICK_ERR_ARG; }
+    const int64_t V = int64_t(L) * L * L;
+    // Timeslice blocks: propagators of block b+1 are copied on a second stream while block b computes.
+    // Each block is an independent wick_contract over Tb timeslices (per-timeslice results do not
+    // depend on the blocking: the reduction over sites of one timeslice always has the same shape).
+    const size_t slice_bytes = size_t(V) * 144 * 16;
+    int Tb = int(std::max<size_t>(1, (size_t(256) << 20) / slice_bytes));
+    Tb = std::min(Tb, T);
+    const size_t ws_bytes = wick_contract_workspace_bytes(t, L, Tb, n_mom);
+    if (!ws_bytes) { set_error("wick_contract_host: bad sizes"); return WICK_ERR_ARG; }
+    void *dU[2] = {nullptr, nullptr}, *dD[2] = {nullptr, nullptr}, *ws = nullptr, *dC = nullptr, *dS = nullptr;
+    cudaStream_t sc = nullptr, sx = nullptr;
+    cudaEvent_t copied[2] = {nullptr, nullptr}, consumed[2] = {nullptr, nullptr};
+    int rc = WICK_OK;
+    auto cleanup = [&]() {
+        for (int k = 0; k < 2; ++k) { cudaFree(dU[k]); cudaFree(dD[k]); if (copied[k]) cudaEventDestroy(copied[k]); if (consumed[k]) cudaEventDestroy(consumed[k]); }
+        cudaFree(ws); cudaFree(dC); cudaFree(dS);
+        if (sc) cudaStreamDestroy(sc);
+        if (sx) cudaStreamDestroy(sx);
+    };
+#define WICK_CUDA_H(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) { set_error(std::string(#call) + ": " + cudaGetErrorString(e_)); cleanup(); return WICK_ERR_CUDA; } } while (0)
+    WICK_CUDA_H(cudaStreamCreate(&sc));
+    WICK_CUDA_H(cudaStreamCreate(&sx));
+    for (int k = 0; k < 2; ++k) {
+        WICK_CUDA_H(cudaMalloc(&dU[k], slice_bytes * Tb));
+        WICK_CUDA_H(cudaMalloc(&dD[k], slice_bytes * Tb));
+        WICK_CUDA_H(cudaEventCreateWithFlags(&copied[k], cudaEventDisableTiming));
+        WICK_CUDA_H(cudaEventCreateWithFlags(&consumed[k], cudaEventDisableTiming));
+    }
+    WICK_CUDA_H(cudaMalloc(&ws, ws_bytes));
+    WICK_CUDA_H(cudaMalloc(&dC, std::max<size_t>(size_t(n_mom) * Tb * 16, 16)));
+    if (sigma_out_host) WICK_CUDA_H(cudaMalloc(&dS, size_t(V) * Tb * 16));
+    const unsigned char* Uh = static_cast<const unsigned char*>(U_host);
+    const unsigned char* Dh = static_cast<const unsigned char*>(D_host);
+    std::vector<double> Cblk(size_t(std::max(n_mom, 1)) * Tb * 2);
+    const int n_blocks = (T + Tb - 1) / Tb;
+    auto issue_copy = [&](int b) -> cudaError_t {
+        const int k = b & 1, t0 = b * Tb, nt = std::min(Tb, T - t0);
+        cudaError_t e = cudaStreamWaitEvent(sx, consumed[k], 0);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(dU[k], Uh + size_t(t0) * slice_bytes, slice_bytes * nt, cudaMemcpyHostToDevice, sx);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(dD[k], Dh + size_t(t0) * slice_bytes, slice_bytes * nt, cudaMemcpyHostToDevice, sx);
+        if (e == cudaSuccess) e = cudaEventRecord(copied[k], sx);
+        return e;
+    };
+    WICK_CUDA_H(issue_copy(0));
+    for (int b = 0; b < n_blocks && rc == WICK_OK; ++b) {
+        const int k = b & 1, t0 = b * Tb, nt = std::min(Tb, T - t0);
+        if (b + 1 < n_blocks) WICK_CUDA_H(issue_copy(b + 1));
+        WICK_CUDA_H(cudaStreamWaitEvent(sc, copied[k], 0));
+        rc = wick_contract(dU[k], dD[k], t, momenta, n_mom, L, nt, dC, dS, ws, ws_bytes, flags, sc);
+        if (rc != WICK_OK) break;
+        WICK_CUDA_H(cudaEventRecord(consumed[k], sc));
+        WICK_CUDA_H(cudaMemcpyAsync(Cblk.data(), dC, size_t(n_mom) * nt * 16, cudaMemcpyDeviceToHost, sc));
+        if (sigma_out_host)
+            WICK_CUDA_H(cudaMemcpyAsync(static_cast<unsigned char*>(sigma_out_host) + size_t(t0) * V * 16, dS, size_t(V) * nt * 16, cudaMemcpyDeviceToHost, sc));
+        WICK_CUDA_H(cudaStreamSynchronize(sc));
+        double* Co = static_cast<double*>(C_out_host);
+        for (int m = 0; m < n_mom; ++m)
+            std::memcpy(Co + (size_t(m) * T + t0) * 2, Cblk.data() + size_t(m) * nt * 2, size_t(nt) * 16);
+    }
+    WICK_CUDA_H(cudaStreamSynchronize(sx));
+    cleanup();
+#undef WICK_CUDA_H
+    return rc;
+}
+
+extern "C" int wick_minor_dets(const void* P_dev, int64_t n_sites, int n, const uint8_t* rows, const uint8_t* cols,
+                               int64_t n_minors, void* out_dev, void* cuda_stream) {
+    if (!P_dev || !out_dev || n < 0 || n > 12 || n_sites < 0 || n_minors < 0 || (n > 0 && n_minors > 0 && (!rows || !cols))) {
+        set_error("wick_minor_dets: bad argument"); return WICK_ERR_ARG; }
+    for (int64_t k = 0; k < n_minors * n; ++k)
+        if (rows[k] > 11 || cols[k] > 11) { set_error("wick_minor_dets: index >= 12"); return WICK_ERR_ARG; }
+    if (n_sites == 0 || n_minors == 0) return WICK_OK;
+    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    int rc = ensure_configured();
+    if (rc != WICK_OK) return rc;
+    const int64_t n_pad = (n_sites + GROUP - 1) / GROUP * GROUP;
+    const bool direct = (n_pad == n_sites);                   // out[m][s] has row length n_sites: usable as S_b only if padded
+    // tables: one row tuple and one column tuple per minor, processed in slabs of 32768 minors
+    const int64_t slab = 32768;
+    std::vector<uint8_t> re(size_t(std::min(slab, n_minors)) * 16), ce(re.size());
+    std::vector<uint32_t> rcv(size_t(std::min(slab, n_minors)));
+    void *d_re = nullptr, *d_ce = nullptr, *d_rc = nullptr, *d_tmp = nullptr;
+    auto cleanup = [&]() { cudaFree(d_re); cudaFree(d_ce); cudaFree(d_rc); cudaFree(d_tmp); };
+#define WICK_CUDA_M(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) { set_error(std::string(#call) + ": " + cudaGetErrorString(e_)); cleanup(); return WICK_ERR_CUDA; } } while (0)
+    WICK_CUDA_M(cudaMalloc(&d_re, re.size()));
+    WICK_CUDA_M(cudaMalloc(&d_ce, ce.size()));
+    WICK_CUDA_M(cudaMalloc(&d_rc, rcv.size() * 4));
+    // site batches so that the padded staging buffer stays small when n_sites is not a multiple of 32
+    const int64_t S_b = direct ? n_sites : std::min<int64_t>(n_pad, 4096);
+    if (!direct) WICK_CUDA_M(cudaMalloc(&d_tmp, size_t(std::min(slab, n_minors)) * size_t(S_b) * 16));
+    if (S_b > (int64_t(1) << 22) && direct) {                 // keep 32-bit S_b
+        cleanup(); set_error("wick_minor_dets: n_sites too large for one call (max 2^22)"); return WICK_ERR_UNSUPPORTED; }
+    for (int64_t m0 = 0; m0 < n_minors; m0 += slab) {
+        const int64_t nm = std::min(slab, n_minors - m0);
+        std::fill(re.begin(), re.end(), 0); std::fill(ce.begin(), ce.end(), 0);
+        for (int64_t m = 0; m < nm; ++m) {
+            for (int i = 0; i < n; ++i) {
+                re[size_t(m) * 16 + i] = uint8_t(rows[(m0 + m) * n + i] * 12);
+                ce[size_t(m) * 16 + i] = cols[(m0 + m) * n + i];
+            }
+            rcv[size_t(m)] = uint32_t(m) | (uint32_t(m) << 16);
+        }
+        WICK_CUDA_M(cudaMemcpyAsync(d_re, re.data(), size_t(nm) * 16, cudaMemcpyHostToDevice, stream));
+        WICK_CUDA_M(cudaMemcpyAsync(d_ce, ce.data(), size_t(nm) * 16, cudaMemcpyHostToDevice, stream));
+        WICK_CUDA_M(cudaMemcpyAsync(d_rc, rcv.data(), size_t(nm) * 4, cudaMemcpyHostToDevice, stream));
+        double2* out = static_cast<double2*>(out_dev) + m0 * n_sites;
+        if (direct) {
+            WICK_CUDA_M(launch_minors(n, static_cast<const double2*>(P_dev), 0, n_sites, int(n_sites / GROUP), int(S_b),
+                                      static_cast<const uint8_t*>(d_re), static_cast<const uint8_t*>(d_ce),
+                                      static_cast<const uint32_t*>(d_rc), nm, out, stream));
+        } else {
+            for (int64_t s0 = 0; s0 < n_sites; s0 += S_b) {
+                const int64_t nv = std::min(S_b, n_sites - s0);
+                WICK_CUDA_M(launch_minors(n, static_cast<const double2*>(P_dev), s0, n_sites, int((nv + GROUP - 1) / GROUP), int(S_b),
+                                          static_cast<const uint8_t*>(d_re), static_cast<const uint8_t*>(d_ce),
+                                          static_cast<const uint32_t*>(d_rc), nm, static_cast<double2*>(d_tmp), stream));
+                WICK_CUDA_M(cudaMemcpy2DAsync(out + s0, size_t(n_sites) * 16, d_tmp, size_t(S_b) * 16, size_t(nv) * 16, size_t(nm),
+                                              cudaMemcpyDeviceToDevice, stream));
+            }
+        }
+        WICK_CUDA_M(cudaStreamSynchronize(stream));           // host tables are reused by the next slab
+    }
+    cleanup();
+#undef WICK_CUDA_M
+    return WICK_OK;
+}

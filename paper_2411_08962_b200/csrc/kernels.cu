@@ -1,0 +1,526 @@
+// Device kernels of the hot path, sm_100a.  See kernels.cuh for the on-chip layout.
+//
+//  a3  stage_tile          : propagators of 32 site-times -> shared memory, element-major / lane-minor
+//  a4  minors_kernel<N>    : one unique minor per (warp iteration, lane = site).  N <= 4: analytic
+//                            expression; N >= 5: LU with partial pivoting.  The LU is
+//                            LEFT-LOOKING: column j of the minor is gathered from shared memory only
+//                            after the pivots of columns < j are known, in the lane's current row
+//                            order, so the only data that ever has to be exchanged in registers is
+//                            the active column and the multipliers (O(N^2) selects, not O(N^3)).
+//  a5  reduce_flat / reduce_outer : sigma(x,t) = sum_k w_k MU[uid_k] MD[did_k]  (Eq. A1-A5)
+//  a6  finalize_sigma, project    : fixed-order sum of the partials, momentum phases, fixed tree over sites
+#include "kernels.cuh"
+
+namespace wick {
+
+typedef double2 c128;
+
+static thread_local int64_t g_launches = 0;
+int64_t launch_counter_get() { return g_launches; }
+int64_t launch_counter_reset() { const int64_t v = g_launches; g_launches = 0; return v; }
+
+__device__ __forceinline__ c128 cmul(c128 a, c128 b) {
+    return make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x);
+}
+__device__ __forceinline__ c128 cfma(c128 a, c128 b, c128 c) {       // a*b + c
+    return make_double2(fma(a.x, b.x, fma(-a.y, b.y, c.x)), fma(a.x, b.y, fma(a.y, b.x, c.y)));
+}
+__device__ __forceinline__ c128 cfnma(c128 a, c128 b, c128 c) {      // c - a*b
+    return make_double2(fma(-a.x, b.x, fma(a.y, b.y, c.x)), fma(-a.x, b.y, fma(-a.y, b.x, c.y)));
+}
+__device__ __forceinline__ c128 csub(c128 a, c128 b) { return make_double2(a.x - b.x, a.y - b.y); }
+__device__ __forceinline__ c128 cadd(c128 a, c128 b) { return make_double2(a.x + b.x, a.y + b.y); }
+
+// ---------------------------------------------------------------------------------------------
+// a3: stage the 12x12 propagators of one 32-site group: tile[e][lane], e = 12*row + col
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ void stage_tile(c128* tile, const c128* __restrict__ P, int64_t st_first,
+                                           int64_t n_st_total, int nthreads) {
+    // consecutive threads read consecutive 16-byte elements of one site (coalesced); sites beyond the
+    // end of the lattice are filled with zeros (their lanes never store a result)
+    for (int idx = threadIdx.x; idx < TILE_ELEMS; idx += nthreads) {
+        const int site = idx / 144, e = idx - site * 144;
+        const int64_t st = st_first + site;
+        c128 v = make_double2(0.0, 0.0);
+        if (st < n_st_total) v = __ldg(P + st * 144 + e);
+        tile[e * GROUP + site] = v;
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// a4: determinants.  `tl` points at tile[0][lane]; re[i] = 12*a_i, ce[j] = b_j (warp-uniform).
+// ---------------------------------------------------------------------------------------------
+template <int N> struct Idx { int re[N > 0 ? N : 1]; int ce[N > 0 ? N : 1]; };
+
+__device__ __forceinline__ c128 ld(const c128* tl, int re, int ce) { return tl[(re + ce) * GROUP]; }
+
+__device__ __forceinline__ c128 det2(c128 a, c128 b, c128 c, c128 d) {   // a d - b c
+    return cfnma(b, c, cmul(a, d));
+}
+
+template <int N>
+__device__ __forceinline__ c128 det_small(const c128* tl, const Idx<N>& ix) {
+    if (N == 0) return make_double2(1.0, 0.0);
+    if (N == 1) return ld(tl, ix.re[0], ix.ce[0]);
+    if (N == 2)
+        return det2(ld(tl, ix.re[0], ix.ce[0]), ld(tl, ix.re[0], ix.ce[1]),
+                    ld(tl, ix.re[1], ix.ce[0]), ld(tl, ix.re[1], ix.ce[1]));
+    if (N == 3) {
+        c128 m[3][3];
+#pragma unroll
+        for (int i = 0; i < 3; ++i)
+#pragma unroll
+            for (int j = 0; j < 3; ++j) m[i][j] = ld(tl, ix.re[i], ix.ce[j]);
+        // expansion along the first row
+        c128 d = cmul(m[0][0], det2(m[1][1], m[1][2], m[2][1], m[2][2]));
+        d = cfnma(m[0][1], det2(m[1][0], m[1][2], m[2][0], m[2][2]), d);
+        d = cfma(m[0][2], det2(m[1][0], m[1][1], m[2][0], m[2][1]), d);
+        return d;
+    }
+    // N == 4: Laplace expansion along the first two rows: sum over column pairs of
+    // (2x2 minor of rows 0,1) * (complementary 2x2 minor of rows 2,3) * sign
+    c128 m[4][4];
+#pragma unroll
+    for (int i = 0; i < 4; ++i)
+#pragma unroll
+        for (int j = 0; j < 4; ++j) m[i][j] = ld(tl, ix.re[i], ix.ce[j]);
+    const c128 s01 = det2(m[0][0], m[0][1], m[1][0], m[1][1]);
+    const c128 s02 = det2(m[0][0], m[0][2], m[1][0], m[1][2]);
+    const c128 s03 = det2(m[0][0], m[0][3], m[1][0], m[1][3]);
+    const c128 s12 = det2(m[0][1], m[0][2], m[1][1], m[1][2]);
+    const c128 s13 = det2(m[0][1], m[0][3], m[1][1], m[1][3]);
+    const c128 s23 = det2(m[0][2], m[0][3], m[1][2], m[1][3]);
+    const c128 b01 = det2(m[2][0], m[2][1], m[3][0], m[3][1]);
+    const c128 b02 = det2(m[2][0], m[2][2], m[3][0], m[3][2]);
+    const c128 b03 = det2(m[2][0], m[2][3], m[3][0], m[3][3]);
+    const c128 b12 = det2(m[2][1], m[2][2], m[3][1], m[3][2]);
+    const c128 b13 = det2(m[2][1], m[2][3], m[3][1], m[3][3]);
+    const c128 b23 = det2(m[2][2], m[2][3], m[3][2], m[3][3]);
+    c128 d = cmul(s01, b23);
+    d = cfnma(s02, b13, d);
+    d = cfma(s03, b12, d);
+    d = cfma(s12, b03, d);
+    d = cfnma(s13, b02, d);
+    d = cfma(s23, b01, d);
+    return d;
+}
+
+// reciprocal of a pivot: 1/(x + i y) = (x - i y) / (x^2 + y^2); an exactly zero pivot (singular
+// column: every candidate was 0) gives multipliers 0 so that det stays exactly 0 instead of NaN
+__device__ __forceinline__ c128 crecip(c128 p) {
+    const double d = fma(p.x, p.x, p.y * p.y);
+    const double r = d > 0.0 ? 1.0 / d : 0.0;
+    return make_double2(p.x * r, -p.y * r);
+}
+
+// Left-looking LU with partial pivoting, multipliers L in registers (N = 5..8).
+// Pivot = candidate with the largest |re| + |im| (the LAPACK izamax / cabs1 rule), first maximum wins.
+template <int N>
+__device__ __forceinline__ c128 det_lu_reg(const c128* tl, const Idx<N>& ix) {
+    int roff[N];                       // per-lane row order: element offset of the row at position r
+#pragma unroll
+    for (int r = 0; r < N; ++r) roff[r] = ix.re[r];
+    double Lr[N][N], Li[N][N];         // multipliers; only [r][i] with r > i is used
+    c128 det = make_double2(1.0, 0.0);
+#pragma unroll
+    for (int j = 0; j < N; ++j) {
+        double cr[N], ci[N];
+#pragma unroll
+        for (int r = 0; r < N; ++r) {
+            const c128 v = ld(tl, roff[r], ix.ce[j]);
+            cr[r] = v.x; ci[r] = v.y;
+        }
+        // apply the eliminations of columns i < j to the new column
+#pragma unroll
+        for (int i = 0; i < j; ++i) {
+#pragma unroll
+            for (int r = i + 1; r < N; ++r) {
+                cr[r] = fma(-Lr[r][i], cr[i], fma(Li[r][i], ci[i], cr[r]));
+                ci[r] = fma(-Lr[r][i], ci[i], fma(-Li[r][i], cr[i], ci[r]));
+            }
+        }
+        if (j < N - 1) {
+            int p = j;
+            double best = fabs(cr[j]) + fabs(ci[j]);
+#pragma unroll
+            for (int r = j + 1; r < N; ++r) {
+                const double m = fabs(cr[r]) + fabs(ci[r]);
+                if (m > best) { best = m; p = r; }
+            }
+            // exchange positions j and p: active column, row order, multipliers of columns < j
+            double pr = cr[j], pi = ci[j];
+            int po = roff[j];
+#pragma unroll
+            for (int r = j + 1; r < N; ++r) {
+                const bool hit = (p == r);
+                const double tr = cr[r], ti = ci[r];
+                const int to = roff[r];
+                cr[r] = hit ? cr[j] : tr; ci[r] = hit ? ci[j] : ti; roff[r] = hit ? roff[j] : to;
+                pr = hit ? tr : pr; pi = hit ? ti : pi; po = hit ? to : po;
+            }
+            cr[j] = pr; ci[j] = pi; roff[j] = po;
+#pragma unroll
+            for (int i = 0; i < j; ++i) {
+                double gr = Lr[j][i], gi = Li[j][i];
+#pragma unroll
+                for (int r = j + 1; r < N; ++r) {
+                    const bool hit = (p == r);
+                    const double tr = Lr[r][i], ti = Li[r][i];
+                    Lr[r][i] = hit ? Lr[j][i] : tr; Li[r][i] = hit ? Li[j][i] : ti;
+                    gr = hit ? tr : gr; gi = hit ? ti : gi;
+                }
+                Lr[j][i] = gr; Li[j][i] = gi;
+            }
+            const c128 piv = make_double2(pr, pi);
+            det = cmul(det, piv);
+            if (p != j) { det.x = -det.x; det.y = -det.y; }
+            const c128 inv = crecip(piv);
+#pragma unroll
+            for (int r = j + 1; r < N; ++r) {
+                Lr[r][j] = cr[r] * inv.x - ci[r] * inv.y;
+                Li[r][j] = cr[r] * inv.y + ci[r] * inv.x;
+            }
+        } else {
+            det = cmul(det, make_double2(cr[N - 1], ci[N - 1]));
+        }
+    }
+    return det;
+}
+
+// Same algorithm with the multipliers in shared memory (N = 9..12: N(N-1)/2 complex numbers do not
+// fit one thread's registers).  Ls points at this thread's slot; entry (r, i), r > i, lives at
+// Ls[(r(r-1)/2 + i) * NT] so that consecutive lanes hit consecutive 16-byte words (conflict free,
+// also for the per-lane dynamic row p of the exchange).
+template <int N, int NT>
+__device__ __forceinline__ c128 det_lu_smem(const c128* tl, c128* Ls, const Idx<N>& ix) {
+    int roff[N];
+#pragma unroll
+    for (int r = 0; r < N; ++r) roff[r] = ix.re[r];
+    c128 det = make_double2(1.0, 0.0);
+#pragma unroll
+    for (int j = 0; j < N; ++j) {
+        double cr[N], ci[N];
+#pragma unroll
+        for (int r = 0; r < N; ++r) {
+            const c128 v = ld(tl, roff[r], ix.ce[j]);
+            cr[r] = v.x; ci[r] = v.y;
+        }
+#pragma unroll
+        for (int i = 0; i < j; ++i) {
+#pragma unroll
+            for (int r = i + 1; r < N; ++r) {
+                const c128 l = Ls[(r * (r - 1) / 2 + i) * NT];
+                cr[r] = fma(-l.x, cr[i], fma(l.y, ci[i], cr[r]));
+                ci[r] = fma(-l.x, ci[i], fma(-l.y, cr[i], ci[r]));
+            }
+        }
+        if (j < N - 1) {
+            int p = j;
+            double best = fabs(cr[j]) + fabs(ci[j]);
+#pragma unroll
+            for (int r = j + 1; r < N; ++r) {
+                const double m = fabs(cr[r]) + fabs(ci[r]);
+                if (m > best) { best = m; p = r; }
+            }
+            double pr = cr[j], pi = ci[j];
+            int po = roff[j];
+#pragma unroll
+            for (int r = j + 1; r < N; ++r) {
+                const bool hit = (p == r);
+                const double tr = cr[r], ti = ci[r];
+                const int to = roff[r];
+                cr[r] = hit ? cr[j] : tr; ci[r] = hit ? ci[j] : ti; roff[r] = hit ? roff[j] : to;
+                pr = hit ? tr : pr; pi = hit ? ti : pi; po = hit ? to : po;
+            }
+            cr[j] = pr; ci[j] = pi; roff[j] = po;
+            if (p != j) {                                   // exchange multiplier rows j and p (columns < j)
+                const int pb = p * (p - 1) / 2;
+#pragma unroll
+                for (int i = 0; i < j; ++i) {
+                    const c128 a = Ls[(j * (j - 1) / 2 + i) * NT];
+                    const c128 b = Ls[(pb + i) * NT];
+                    Ls[(j * (j - 1) / 2 + i) * NT] = b;
+                    Ls[(pb + i) * NT] = a;
+                }
+            }
+            const c128 piv = make_double2(pr, pi);
+            det = cmul(det, piv);
+            if (p != j) { det.x = -det.x; det.y = -det.y; }
+            const c128 inv = crecip(piv);
+#pragma unroll
+            for (int r = j + 1; r < N; ++r)
+                Ls[(r * (r - 1) / 2 + j) * NT] = make_double2(cr[r] * inv.x - ci[r] * inv.y, cr[r] * inv.y + ci[r] * inv.x);
+        } else {
+            det = cmul(det, make_double2(cr[N - 1], ci[N - 1]));
+        }
+    }
+    return det;
+}
+
+template <int N> struct MinorCfg {
+    static constexpr bool kSmemL = (N >= 9);
+    static constexpr int kThreads = kSmemL ? 128 : 256;
+    static constexpr int kMinBlocks = (N <= 4) ? 2 : 1;
+    static constexpr size_t kSmem = size_t(TILE_BYTES) + (kSmemL ? size_t(N * (N - 1) / 2) * 16 * kThreads : 0);
+};
+
+template <int N>
+__global__ void __launch_bounds__(MinorCfg<N>::kThreads, MinorCfg<N>::kMinBlocks)
+minors_kernel(const c128* __restrict__ P, int64_t st0, int64_t n_st_total, int S_b,
+              const uint8_t* __restrict__ row_elem, const uint8_t* __restrict__ col_elem,
+              const uint32_t* __restrict__ minor_rc, int n_minors, int chunk, c128* __restrict__ out) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    c128* tile = reinterpret_cast<c128*>(smem_raw);
+    constexpr int NT = MinorCfg<N>::kThreads;
+    const int g = blockIdx.x;
+    const int64_t st_first = st0 + int64_t(g) * GROUP;
+    stage_tile(tile, P, st_first, n_st_total, NT);
+    __syncthreads();
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const c128* tl = tile + lane;
+    const bool valid = st_first + lane < n_st_total;
+    const int m_begin = blockIdx.y * chunk;
+    const int m_end = min(n_minors, m_begin + chunk);
+    for (int m = m_begin + warp; m < m_end; m += NT / 32) {
+        const uint32_t rc = __ldg(minor_rc + m);
+        const uint4 rw = __ldg(reinterpret_cast<const uint4*>(row_elem) + (rc & 0xffffu));
+        const uint4 cw = __ldg(reinterpret_cast<const uint4*>(col_elem) + (rc >> 16));
+        const uint32_t rws[4] = {rw.x, rw.y, rw.z, rw.w}, cws[4] = {cw.x, cw.y, cw.z, cw.w};
+        Idx<N> ix;
+#pragma unroll
+        for (int i = 0; i < N; ++i) {
+            ix.re[i] = (rws[i >> 2] >> (8 * (i & 3))) & 0xff;
+            ix.ce[i] = (cws[i >> 2] >> (8 * (i & 3))) & 0xff;
+        }
+        c128 det;
+        if constexpr (N <= 4) det = det_small<N>(tl, ix);
+        else if constexpr (!MinorCfg<N>::kSmemL) det = det_lu_reg<N>(tl, ix);
+        else det = det_lu_smem<N, NT>(tl, tile + TILE_ELEMS + threadIdx.x, ix);
+        if (valid) out[int64_t(m) * S_b + int64_t(g) * GROUP + lane] = det;
+    }
+}
+
+template <int N>
+static cudaError_t launch_minors_n(const c128* P, int64_t st0, int64_t n_st_total, int n_groups, int S_b,
+                                   const uint8_t* row_elem, const uint8_t* col_elem, const uint32_t* minor_rc,
+                                   int64_t n_minors, c128* out, cudaStream_t stream) {
+    constexpr int NT = MinorCfg<N>::kThreads;
+    constexpr int warps = NT / 32;
+    // enough CTAs for ~4 waves on 148 SMs, but at least 2 minors per warp per CTA
+    int chunks = (148 * 4 + n_groups - 1) / n_groups;
+    const int64_t max_chunks = (n_minors + 2 * warps - 1) / (2 * warps);
+    if (chunks > max_chunks) chunks = int(max_chunks);
+    if (chunks < 1) chunks = 1;
+    if (chunks > 65535) chunks = 65535;
+    int chunk = int((n_minors + chunks - 1) / chunks);
+    chunk = ((chunk + warps - 1) / warps) * warps;            // every warp of a CTA gets the same count
+    chunks = int((n_minors + chunk - 1) / chunk);
+    dim3 grid(n_groups, chunks);
+    minors_kernel<N><<<grid, NT, MinorCfg<N>::kSmem, stream>>>(P, st0, n_st_total, S_b, row_elem, col_elem,
+                                                             minor_rc, int(n_minors), chunk, out);
+    ++g_launches;
+    return cudaGetLastError();
+}
+
+cudaError_t launch_minors(int n, const double2* P, int64_t st0, int64_t n_st_total, int n_groups, int S_b,
+                          const uint8_t* row_elem, const uint8_t* col_elem, const uint32_t* minor_rc,
+                          int64_t n_minors, double2* out, cudaStream_t stream) {
+    if (n_minors == 0 || n_groups == 0) return cudaSuccess;
+#define WICK_CASE(N) case N: return launch_minors_n<N>(P, st0, n_st_total, n_groups, S_b, row_elem, col_elem, minor_rc, n_minors, out, stream);
+    switch (n) {
+        WICK_CASE(0) WICK_CASE(1) WICK_CASE(2) WICK_CASE(3) WICK_CASE(4) WICK_CASE(5) WICK_CASE(6)
+        WICK_CASE(7) WICK_CASE(8) WICK_CASE(9) WICK_CASE(10) WICK_CASE(11) WICK_CASE(12)
+        default: return cudaErrorInvalidValue;
+    }
+#undef WICK_CASE
+}
+
+template <int N> static cudaError_t set_smem_attr() {
+    return cudaFuncSetAttribute(minors_kernel<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(MinorCfg<N>::kSmem));
+}
+
+cudaError_t configure_kernels() {
+    cudaError_t e;
+#define WICK_ATTR(N) if ((e = set_smem_attr<N>()) != cudaSuccess) return e;
+    WICK_ATTR(0) WICK_ATTR(1) WICK_ATTR(2) WICK_ATTR(3) WICK_ATTR(4) WICK_ATTR(5) WICK_ATTR(6)
+    WICK_ATTR(7) WICK_ATTR(8) WICK_ATTR(9) WICK_ATTR(10) WICK_ATTR(11) WICK_ATTR(12)
+#undef WICK_ATTR
+    return cudaSuccess;
+}
+
+// ---------------------------------------------------------------------------------------------
+// a5: weighted bilinear products.  Lane = site; term indices and weights are warp-uniform.
+// Each CTA handles one 32-site group and one chunk of the work; its warps' partial sums are
+// combined in a fixed order and written to partial[chunk][site] (no atomics).
+// ---------------------------------------------------------------------------------------------
+constexpr int RED_THREADS = 256;
+
+__device__ __forceinline__ void cta_combine_store(c128 acc, c128* partial_out /* &partial[chunk*S_b + g*32] */) {
+    __shared__ c128 sm[RED_THREADS];
+    sm[threadIdx.x] = acc;
+    __syncthreads();
+    if (threadIdx.x < GROUP) {
+        c128 s = sm[threadIdx.x];
+#pragma unroll
+        for (int w = 1; w < RED_THREADS / 32; ++w) s = cadd(s, sm[w * 32 + threadIdx.x]);
+        partial_out[threadIdx.x] = s;
+    }
+}
+
+__global__ void __launch_bounds__(RED_THREADS)
+reduce_flat_kernel(const c128* __restrict__ MU, const c128* __restrict__ MD, int S_b,
+                   const int32_t* __restrict__ uid, const int32_t* __restrict__ did, const c128* __restrict__ w,
+                   int64_t n_terms, int64_t chunk, c128* __restrict__ partial) {
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int64_t s = int64_t(blockIdx.x) * GROUP + lane;
+    const int64_t k0 = int64_t(blockIdx.y) * chunk;
+    const int64_t k1 = min(n_terms, k0 + chunk);
+    c128 acc = make_double2(0.0, 0.0);
+    for (int64_t k = k0 + warp; k < k1; k += RED_THREADS / 32) {
+        const c128 u = MU[int64_t(__ldg(uid + k)) * S_b + s];
+        const c128 d = MD[int64_t(__ldg(did + k)) * S_b + s];
+        acc = cfma(cmul(__ldg(w + k), u), d, acc);
+    }
+    cta_combine_store(acc, partial + int64_t(blockIdx.y) * S_b + int64_t(blockIdx.x) * GROUP);
+}
+
+// Outer-product lists: terms (i, j) = sink i x source j with uid = ru_i * NBu + cu_j,
+// did = rd_i * NBd + cd_j, w = c_i * cbar_j.  For a fixed u row tuple ru and d column tuple cd
+//     sum_{i in sink[ru]} sum_{j in src[cd]} c_i cbar_j MU[ru, cu_j] MD[rd_i, cd]
+//   = ( sum_j cbar_j MU[ru, cu_j] ) * ( sum_i c_i MD[rd_i, cd] ),
+// i.e. |sink[ru]| + |src[cd]| loads for |sink[ru]| * |src[cd]| terms.
+__global__ void __launch_bounds__(RED_THREADS)
+reduce_outer_kernel(const c128* __restrict__ MU, const c128* __restrict__ MD, int S_b,
+                    int n_rows_u, int n_cols_u, int n_cols_d,
+                    const int32_t* __restrict__ sink_ptr, const int32_t* __restrict__ sink_rd, const c128* __restrict__ sink_c,
+                    const int32_t* __restrict__ src_ptr, const int32_t* __restrict__ src_cu, const c128* __restrict__ src_c,
+                    int rows_per_cta, c128* __restrict__ partial) {
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int64_t s = int64_t(blockIdx.x) * GROUP + lane;
+    const int r0 = blockIdx.y * rows_per_cta;
+    const int r1 = min(n_rows_u, r0 + rows_per_cta);
+    c128 acc = make_double2(0.0, 0.0);
+    for (int ru = r0 + warp; ru < r1; ru += RED_THREADS / 32) {
+        const int i0 = __ldg(sink_ptr + ru), i1 = __ldg(sink_ptr + ru + 1);
+        if (i0 == i1) continue;
+        const c128* MUrow = MU + int64_t(ru) * n_cols_u * S_b + s;
+        for (int cd = 0; cd < n_cols_d; ++cd) {
+            const int j0 = __ldg(src_ptr + cd), j1 = __ldg(src_ptr + cd + 1);
+            if (j0 == j1) continue;
+            c128 wsum = make_double2(0.0, 0.0);
+            for (int j = j0; j < j1; ++j)
+                wsum = cfma(__ldg(src_c + j), MUrow[int64_t(__ldg(src_cu + j)) * S_b], wsum);
+            c128 tsum = make_double2(0.0, 0.0);
+            const c128* MDcol = MD + int64_t(cd) * S_b + s;
+            for (int i = i0; i < i1; ++i)
+                tsum = cfma(__ldg(sink_c + i), MDcol[int64_t(__ldg(sink_rd + i)) * n_cols_d * S_b], tsum);
+            acc = cfma(wsum, tsum, acc);
+        }
+    }
+    cta_combine_store(acc, partial + int64_t(blockIdx.y) * S_b + int64_t(blockIdx.x) * GROUP);
+}
+
+cudaError_t launch_reduce_flat(const double2* MU, const double2* MD, int n_groups, int S_b,
+                               const int32_t* uid, const int32_t* did, const double2* w, int64_t n_terms,
+                               double2* partial, int* n_chunks_out, int max_chunks, cudaStream_t stream) {
+    int chunks = (148 * 8 + n_groups - 1) / n_groups;
+    const int64_t cap = (n_terms + 63) / 64;                  // at least 8 terms per warp
+    if (chunks > cap) chunks = int(cap);
+    if (chunks > max_chunks) chunks = max_chunks;
+    if (chunks < 1) chunks = 1;
+    const int64_t chunk = (n_terms + chunks - 1) / chunks;
+    chunks = chunk > 0 ? int((n_terms + chunk - 1) / chunk) : 1;
+    if (chunks < 1) chunks = 1;
+    dim3 grid(n_groups, chunks);
+    reduce_flat_kernel<<<grid, RED_THREADS, 0, stream>>>(MU, MD, S_b, uid, did, w, n_terms, chunk > 0 ? chunk : 1, partial);
+    ++g_launches;
+    *n_chunks_out = chunks;
+    return cudaGetLastError();
+}
+
+cudaError_t launch_reduce_outer(const double2* MU, const double2* MD, int n_groups, int S_b,
+                                int n_rows_u, int n_cols_u, int n_cols_d,
+                                const int32_t* sink_ptr, const int32_t* sink_rd, const double2* sink_c,
+                                const int32_t* src_ptr, const int32_t* src_cu, const double2* src_c,
+                                double2* partial, int* n_chunks_out, int max_chunks, cudaStream_t stream) {
+    int chunks = (148 * 8 + n_groups - 1) / n_groups;
+    const int cap = (n_rows_u + 7) / 8;                       // at least one row tuple per warp
+    if (chunks > cap) chunks = cap;
+    if (chunks > max_chunks) chunks = max_chunks;
+    if (chunks < 1) chunks = 1;
+    const int rows_per_cta = (n_rows_u + chunks - 1) / chunks;
+    chunks = (n_rows_u + rows_per_cta - 1) / rows_per_cta;
+    dim3 grid(n_groups, chunks);
+    reduce_outer_kernel<<<grid, RED_THREADS, 0, stream>>>(MU, MD, S_b, n_rows_u, n_cols_u, n_cols_d, sink_ptr, sink_rd,
+                                                          sink_c, src_ptr, src_cu, src_c, rows_per_cta, partial);
+    ++g_launches;
+    *n_chunks_out = chunks;
+    return cudaGetLastError();
+}
+
+// ---------------------------------------------------------------------------------------------
+// a6: sigma = fixed-order sum of the chunk partials; C(t,p) = sum_x e^{ip.x} sigma(x,t), fixed tree
+// ---------------------------------------------------------------------------------------------
+__global__ void finalize_sigma_kernel(const c128* __restrict__ partial, int n_chunks, int S_b, int64_t n_valid,
+                                      c128* __restrict__ sigma_batch) {
+    const int64_t s = int64_t(blockIdx.x) * blockDim.x + threadIdx.x;
+    if (s >= n_valid) return;
+    c128 acc = partial[s];
+    for (int c = 1; c < n_chunks; ++c) acc = cadd(acc, partial[int64_t(c) * S_b + s]);
+    sigma_batch[s] = acc;
+}
+
+cudaError_t launch_finalize_sigma(const double2* partial, int n_chunks, int S_b, int64_t n_valid,
+                                  double2* sigma_batch, cudaStream_t stream) {
+    if (n_valid <= 0) return cudaSuccess;
+    const int threads = 128;
+    finalize_sigma_kernel<<<unsigned((n_valid + threads - 1) / threads), threads, 0, stream>>>(partial, n_chunks, S_b, n_valid, sigma_batch);
+    ++g_launches;
+    return cudaGetLastError();
+}
+
+constexpr int PROJ_THREADS = 256;
+
+// one CTA per (momentum, timeslice): each thread sums its sites in index order, then a fixed tree
+__global__ void __launch_bounds__(PROJ_THREADS)
+project_kernel(const c128* __restrict__ sigma, int L, int T, MomentumList mom, c128* __restrict__ C_out) {
+    __shared__ c128 sm[PROJ_THREADS];
+    const int t = blockIdx.x, p = blockIdx.y;
+    const int V = L * L * L;
+    const int nx = mom.v[p][0], ny = mom.v[p][1], nz = mom.v[p][2];
+    const bool zero = (nx == 0 && ny == 0 && nz == 0);
+    const c128* sg = sigma + int64_t(t) * V;
+    c128 acc = make_double2(0.0, 0.0);
+    for (int s = threadIdx.x; s < V; s += PROJ_THREADS) {
+        const c128 v = sg[s];
+        if (zero) {
+            acc = cadd(acc, v);
+        } else {
+            const int x = s % L, y = (s / L) % L, z = s / (L * L);
+            long long m = (long long)nx * x + (long long)ny * y + (long long)nz * z;
+            m %= L;
+            if (m < 0) m += L;
+            double sn, cs;
+            sincospi(2.0 * double(m) / double(L), &sn, &cs);   // exact at multiples of L/4
+            acc = cfma(make_double2(cs, sn), v, acc);
+        }
+    }
+    sm[threadIdx.x] = acc;
+    __syncthreads();
+    for (int h = PROJ_THREADS / 2; h > 0; h >>= 1) {
+        if (threadIdx.x < h) sm[threadIdx.x] = cadd(sm[threadIdx.x], sm[threadIdx.x + h]);
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) C_out[int64_t(p) * T + t] = sm[0];
+}
+
+cudaError_t launch_project(const double2* sigma, int L, int T, const MomentumList& mom, double2* C_out,
+                           cudaStream_t stream) {
+    if (T <= 0 || mom.n <= 0) return cudaSuccess;
+    dim3 grid(T, mom.n);
+    project_kernel<<<grid, PROJ_THREADS, 0, stream>>>(sigma, L, T, mom, C_out);
+    ++g_launches;
+    return cudaGetLastError();
+}
+
+}  // namespace wick

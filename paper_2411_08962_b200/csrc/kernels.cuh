@@ -1,0 +1,43 @@
+// Device kernels of the hot path (steps a3-a6 of DESIGN.md), sm_100a.
+//
+// Data layout on chip ("site per lane"): a warp works on GROUP = 32 consecutive site-times; lane l
+// owns site-time st0 + 32 g + l.  The propagators of the 32 sites are staged once per CTA in shared
+// memory as tile[element e = 12*row + col][lane] (complex128, 16 B): the bank of an access depends on
+// the lane only, so gathers with PER-LANE row order (needed by partial pivoting) are conflict free,
+// and the row / column tuples of a minor are warp-uniform.  Minors are written as M[minor][site]
+// (site fastest), so every global access of the minor and reduction kernels is a coalesced 512-byte row.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace wick {
+
+constexpr int GROUP = 32;                 // site-times per warp
+constexpr int TILE_ELEMS = 144 * GROUP;   // complex128 elements of one flavour tile
+constexpr int TILE_BYTES = TILE_ELEMS * 16;
+constexpr int MAX_MOMENTA = 64;
+
+struct MomentumList { int n; int v[MAX_MOMENTA][3]; };
+
+// launchers (kernels.cu); all enqueue on `stream` and return the cudaGetLastError() code
+cudaError_t launch_minors(int n, const double2* P, int64_t st0, int64_t n_st_total, int n_groups, int S_b,
+                          const uint8_t* row_elem, const uint8_t* col_elem, const uint32_t* minor_rc,
+                          int64_t n_minors, double2* out, cudaStream_t stream);
+cudaError_t launch_reduce_flat(const double2* MU, const double2* MD, int n_groups, int S_b,
+                               const int32_t* uid, const int32_t* did, const double2* w, int64_t n_terms,
+                               double2* partial, int* n_chunks_out, int max_chunks, cudaStream_t stream);
+cudaError_t launch_reduce_outer(const double2* MU, const double2* MD, int n_groups, int S_b,
+                                int n_rows_u, int n_cols_u, int n_cols_d,
+                                const int32_t* sink_ptr, const int32_t* sink_rd, const double2* sink_c,
+                                const int32_t* src_ptr, const int32_t* src_cu, const double2* src_c,
+                                double2* partial, int* n_chunks_out, int max_chunks, cudaStream_t stream);
+cudaError_t launch_finalize_sigma(const double2* partial, int n_chunks, int S_b, int64_t n_valid,
+                                  double2* sigma_batch, cudaStream_t stream);
+cudaError_t launch_project(const double2* sigma, int L, int T, const MomentumList& mom, double2* C_out,
+                           cudaStream_t stream);
+cudaError_t configure_kernels();          // cudaFuncSetAttribute for the large-shared-memory kernels (once per device)
+
+int64_t launch_counter_get();
+int64_t launch_counter_reset();
+
+}  // namespace wick

@@ -1,0 +1,68 @@
+// Internal structures shared by the host term builder (term_builder.cpp) and the device path
+// (contract.cu).  Not part of the C-ABI (include/wick.h).  No CUDA types here so that the host
+// builder compiles as plain C++.
+#pragma once
+#include <complex>
+#include <cstdint>
+#include <mutex>
+#include <string>
+#include <vector>
+
+#include "../../include/wick.h"
+
+namespace wick {
+
+typedef std::complex<double> cplx;
+
+// One flavour's unique-minor tables (the paper's zeta_q, Eq. A1).
+struct FlavourTables {
+    int n = 0;                                  // minor size
+    std::vector<uint16_t> rows, cols;           // distinct index sets as 12-bit masks, in lexicographic tuple order
+    std::vector<int32_t> minor_row, minor_col;  // unique minor m = (rows[minor_row[m]], cols[minor_col[m]])
+};
+
+// Factor of an outer-product list.  Sink: (row-tuple ids, c_i).  Source: (column-tuple ids, conj c_j).
+struct FactorTerm { int32_t qu, qd; cplx c; };
+
+// Device-resident copies, created by the first device call that needs them (contract.cu).
+struct DeviceTables {
+    int device = -1;
+    void* blob = nullptr;                       // one allocation holding the minor tables + factor lists
+    const uint8_t* row_elem[2] = {nullptr, nullptr};   // [n_rows][16]: a_i * 12 (element offset of row a_i), zero padded
+    const uint8_t* col_elem[2] = {nullptr, nullptr};   // [n_cols][16]: b_j
+    const uint32_t* minor_rc[2] = {nullptr, nullptr};  // [n_minors]: row id | col id << 16
+    // factorised reduction: sink CSR over u row-tuple id, source CSR over d column-tuple id
+    const int32_t* sink_ptr = nullptr;          // [n_rows_u + 1]
+    const int32_t* sink_rd = nullptr;           // [n_sink]   d row-tuple id
+    const double* sink_c = nullptr;             // [n_sink][2]
+    const int32_t* src_ptr = nullptr;           // [n_cols_d + 1]
+    const int32_t* src_cu = nullptr;            // [n_source] u column-tuple id
+    const double* src_c = nullptr;              // [n_source][2]
+    int max_sink_per_row = 0;
+    // flat list (uploaded only when the flat path runs)
+    void* flat_blob = nullptr;
+    const int32_t* t_uid = nullptr;
+    const int32_t* t_did = nullptr;
+    const double* t_w = nullptr;                // [n_terms][2]
+};
+
+void set_error(const std::string& msg);         // thread-local message behind wick_last_error()
+
+}  // namespace wick
+
+struct wick_terms {
+    int n_u = 0, n_d = 0;
+    wick::FlavourTables f[2];                   // 0 = u, 1 = d
+    bool outer = false;
+    std::vector<wick::FactorTerm> sink, source; // outer-product factor lists (source holds conj c_j)
+    int64_t n_terms = 0, n_raw = 0, n_identity_merged = 0;
+    // flat list: always present for generic lists, materialised on demand for outer-product lists
+    mutable std::mutex mu;
+    mutable bool flat_ready = false;
+    mutable std::vector<int32_t> t_uid, t_did;
+    mutable std::vector<wick::cplx> t_w;
+    mutable wick::DeviceTables dev;
+    void ensure_flat() const;                   // term_builder.cpp
+};
+
+extern "C" void wick_terms_release_device(wick::DeviceTables* d);   // contract.cu (cudaFree)

@@ -27,3 +27,18 @@ def load_golden():
 @pytest.fixture(scope="session")
 def golden():
     return load_golden()
+
+
+def pytest_sessionstart(session):
+    """Build libwick_b200.so in-tree if it is missing or older than its sources (nvcc cross-compiles
+    sm_100a without a GPU).  The product path itself never builds or falls back: it raises."""
+    from paper_2411_08962_b200.build import build_library
+    build_library()
+
+
+@pytest.fixture(scope="session")
+def cuda_device():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("this test is marked gpu and needs a CUDA device (no CPU fallback exists)")
+    return torch.device("cuda:0")

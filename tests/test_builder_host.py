@@ -1,0 +1,206 @@
+"""Host-side tests of the C-ABI library (no GPU): the term builder (steps a1, a2, a2') against the
+oracle's own, independently written expansion; error codes; exported symbols; workspace planning."""
+import ctypes
+import re
+
+import numpy as np
+import pytest
+
+import paper_2411_08962_b200 as wk
+from oracle import wick_oracle as wo
+from wick_inputs import CONFIGS, make_random_term_list
+
+NUCLEI = {k: CONFIGS[k].nucleus for k in ("cfg0", "cfg1", "cfg2", "cfg3", "cfg4")}
+# SURVEY.md section 8 structure table (re-derived by the oracle in tests/test_oracle_pins.py)
+EXPECT = {
+    "cfg0": dict(n_u=2, n_d=1, n_sink=21, rows_u=21, rows_d=12, minors_u=441, minors_d=144),
+    "cfg1": dict(n_u=3, n_d=3, n_sink=231, rows_u=121, rows_d=121, minors_u=14641, minors_d=14641),
+    "cfg2": dict(n_u=5, n_d=4, n_sink=1311, rows_u=483, rows_d=342, minors_u=233289, minors_d=116964),
+    "cfg3": dict(n_u=6, n_d=6, n_sink=2716, rows_u=655, rows_d=655, minors_u=429025, minors_d=429025),
+    "cfg4": dict(n_u=10, n_d=11, n_sink=21, rows_u=21, rows_d=12, minors_u=441, minors_d=144),
+}
+
+
+def _rand(rng, *shape):
+    return rng.standard_normal(shape) + 1j * rng.standard_normal(shape)
+
+
+def test_library_exports_every_declared_symbol():
+    lib = wk.load_library()
+    with open("include/wick.h") as f:
+        header = f.read()
+    declared = set(re.findall(r"\b(wick_[a-z_]+)\s*\(", header))
+    assert declared == set(wk.EXPORTED_SYMBOLS)
+    for name in declared:
+        assert getattr(lib, name) is not None
+    assert b"sm_100a" in lib.wick_version()
+
+
+@pytest.mark.parametrize("cfg", ["cfg0", "cfg1", "cfg2", "cfg3", "cfg4"])
+def test_sink_list_matches_oracle_expansion(cfg, golden):
+    t = wk.build_terms(NUCLEI[cfg])
+    i, e = t.info, EXPECT[cfg]
+    assert (i.n_u, i.n_d, i.n_sink, i.n_source) == (e["n_u"], e["n_d"], e["n_sink"], e["n_sink"])
+    assert (i.n_rows_u, i.n_cols_u, i.n_rows_d, i.n_cols_d) == (e["rows_u"], e["rows_u"], e["rows_d"], e["rows_d"])
+    assert (i.n_minors_u, i.n_minors_d) == (e["minors_u"], e["minors_d"])
+    assert i.n_terms == e["n_sink"] ** 2 and i.is_outer_product == 1
+    assert i.n_raw == 24 ** len(NUCLEI[cfg])
+    if cfg == "cfg3":
+        assert i.n_sink == int(golden["he4_terms"])
+    ur, uc, dr, dc = t.tuples()
+    assert np.array_equal(ur, uc) and np.array_equal(dr, dc)
+    for tab in (ur, dr):                                        # ascending tuples in lexicographic order
+        assert np.all(np.diff(tab.astype(int), axis=1) > 0)
+        as_list = [tuple(r) for r in tab]
+        assert as_list == sorted(set(as_list))
+    sru, srd, sc, qcu, qcd, qc = t.factors()
+    mine = {(tuple(ur[a]), tuple(dr[b])): c for a, b, c in zip(sru, srd, sc)}
+    ref = {(u, d): c for u, d, c in wo.merged_terms(NUCLEI[cfg])}
+    assert set(mine) == set(ref)
+    # the overall sign of C gamma5 is a convention that cancels in c_i conj(c_j): compare up to one global sign
+    k0 = next(iter(ref))
+    g = mine[k0] / ref[k0]
+    assert g in (1, -1)
+    assert all(mine[k] == g * ref[k] for k in ref)
+    assert np.array_equal(qcu, sru) and np.array_equal(qcd, srd) and np.array_equal(qc, np.conj(sc))
+
+
+@pytest.mark.parametrize("cfg", ["cfg0", "cfg1"])
+def test_flat_terms_consistent_and_site_value_matches_oracle(cfg):
+    t = wk.build_terms(NUCLEI[cfg])
+    i = t.info
+    uid, did, w = t.terms()
+    sru, srd, sc, qcu, qcd, qc = t.factors()
+    assert np.array_equal(uid, (sru[:, None] * i.n_cols_u + qcu[None, :]).ravel())
+    assert np.array_equal(did, (srd[:, None] * i.n_cols_d + qcd[None, :]).ravel())
+    assert np.array_equal(w, (sc[:, None] * qc[None, :]).ravel())
+    umr, umc, dmr, dmc = t.minors()
+    assert np.array_equal(umr, np.repeat(np.arange(i.n_rows_u), i.n_cols_u))
+    assert np.array_equal(umc, np.tile(np.arange(i.n_cols_u), i.n_rows_u))
+    # evaluate the builder's flat list with the oracle's determinant and compare with the oracle's RAW sum
+    rng = np.random.default_rng(21)
+    U, D = _rand(rng, 12, 12), _rand(rng, 12, 12)
+    a_u, b_u, a_d, b_d, ww = t.term_tuples()
+    got, sabs = wo.site_terms_value(U, D, a_u, b_u, a_d, b_d, ww)
+    if cfg == "cfg0":
+        raw = wo.nucleus_raw_terms(NUCLEI[cfg])
+        ref = wo.raw_site_value(U, D, raw, raw)
+    else:
+        ref, _ = wo.site_value_outer(U, D, wo.merged_terms(NUCLEI[cfg]))
+    assert abs(got - ref) < 1e-12 * sabs
+
+
+def test_from_list_canonicalisation_signs_and_merging():
+    """Raw tuples in any order, with repeats and duplicates: sum_k w_k detU detD over the RAW list
+    (oracle, no sorting) must equal the sum over the canonical list the builder returns."""
+    rng = np.random.default_rng(22)
+    n_u, n_d, n_raw = 4, 3, 300
+    a_u = np.array([rng.permutation(12)[:n_u] for _ in range(n_raw)], np.uint8)
+    b_u = np.array([rng.permutation(12)[:n_u] for _ in range(n_raw)], np.uint8)
+    a_d = np.array([rng.permutation(12)[:n_d] for _ in range(n_raw)], np.uint8)
+    b_d = np.array([rng.permutation(12)[:n_d] for _ in range(n_raw)], np.uint8)
+    w = _rand(rng, n_raw)
+    a_u[5, 1] = a_u[5, 0]                                        # Pauli zeros
+    b_d[9, 2] = b_d[9, 0]
+    for src, dst in ((20, 21), (30, 31), (30, 32)):              # duplicates, one with permuted rows (sign flips)
+        a_u[dst], b_u[dst], a_d[dst], b_d[dst] = a_u[src], b_u[src], a_d[src], b_d[src]
+    a_u[31] = a_u[31][[1, 0, 2, 3]]
+    w[40] = 0.0
+    t = wk.build_terms_from_list(a_u, b_u, a_d, b_d, w)
+    i = t.info
+    assert i.is_outer_product == 0 and i.n_raw == n_raw
+    assert i.n_terms == n_raw - 2 - 3 - 1                        # 2 Pauli zeros, 3 merged duplicates, 1 zero weight
+    U, D = _rand(rng, 12, 12), _rand(rng, 12, 12)
+    ref, sabs = wo.site_terms_value(U, D, a_u, b_u, a_d, b_d, w)
+    ca_u, cb_u, ca_d, cb_d, cw = t.term_tuples()
+    assert np.all(np.diff(ca_u.astype(int), axis=1) > 0) and np.all(np.diff(cb_d.astype(int), axis=1) > 0)
+    got, _ = wo.site_terms_value(U, D, ca_u, cb_u, ca_d, cb_d, cw)
+    assert abs(got - ref) < 1e-12 * sabs
+    # unique minors: every (row tuple, col tuple) pair appears once
+    ur, uc, dr, dc = t.tuples()
+    umr, umc, dmr, dmc = t.minors()
+    assert len({(a, b) for a, b in zip(umr, umc)}) == i.n_minors_u == len(umr)
+    assert len({(a, b) for a, b in zip(dmr, dmc)}) == i.n_minors_d == len(dmr)
+
+
+def test_cfg4b_random_list_roundtrip():
+    c = CONFIGS["cfg4b"]
+    a_u, b_u, a_d, b_d, w = make_random_term_list(c.seed, c.n_u, c.n_d, c.n_random_terms)
+    t = wk.build_terms_from_list(a_u, b_u, a_d, b_d, w)
+    i = t.info
+    assert (i.n_u, i.n_d) == (10, 11) and i.n_terms <= 441 and i.n_terms >= 430
+    assert i.n_minors_u <= 441 and i.n_minors_d <= 144
+    rng = np.random.default_rng(23)
+    U, D = _rand(rng, 12, 12), _rand(rng, 12, 12)
+    ref, sabs = wo.site_terms_value(U, D, a_u, b_u, a_d, b_d, w)
+    got, _ = wo.site_terms_value(U, D, *t.term_tuples())
+    assert abs(got - ref) < 1e-11 * sabs
+
+
+def test_identity_test_merges_nothing_for_distinct_flavours():
+    for cfg in ("cfg0", "cfg1"):
+        t = wk.build_terms(NUCLEI[cfg], flags=wk.BUILD_IDENTITY_TEST, seed=7)
+        assert t.info.n_identity_merged == 0 and t.info.is_outer_product == 1
+        assert t.info.n_terms == EXPECT[cfg]["n_sink"] ** 2
+
+
+def test_identity_test_isospin_finds_flavour_swap_classes():
+    """With U == D (m_u = m_d) products related by exchanging the u and d minors coincide.
+    The expected class count is obtained independently: numerical values of all products at a random
+    complex point, clustered up to sign."""
+    nuc = NUCLEI["cfg1"]
+    plain = wk.build_terms(nuc)
+    t = wk.build_terms(nuc, flags=wk.BUILD_IDENTITY_TEST | wk.BUILD_ISOSPIN, seed=11)
+    rng = np.random.default_rng(24)
+    U = _rand(rng, 12, 12)
+    a_u, b_u, a_d, b_d, w = plain.term_tuples()
+    v = wo.det_elim(U[a_u[:, :, None], b_u[:, None, :]]) * wo.det_elim(U[a_d[:, :, None], b_d[:, None, :]])
+    # canonical representative of {v, -v}: the one whose real part is positive; round relative to |v|
+    s = np.where(v.real < 0, -1.0, 1.0)
+    key = np.round((v * s) / np.abs(v).max() * 1e9).astype(np.complex128)
+    n_classes = len(np.unique(key))
+    # merged weights that cancel exactly drop out; count the classes whose summed weight is non-zero
+    order = np.unique(key, return_inverse=True)[1]
+    wsum = np.zeros(n_classes, complex)
+    np.add.at(wsum, order, w * s)
+    expected = int(np.count_nonzero(np.abs(wsum) > 1e-9))
+    assert t.info.n_terms == expected
+    assert t.info.n_identity_merged == plain.info.n_terms - expected
+    assert expected < plain.info.n_terms and t.info.is_outer_product == 0
+    # merged list evaluates to the same number at another U == D point
+    U2 = _rand(rng, 12, 12)
+    ref, sabs = wo.site_terms_value(U2, U2, a_u, b_u, a_d, b_d, w)
+    got, _ = wo.site_terms_value(U2, U2, *t.term_tuples())
+    assert abs(got - ref) < 1e-11 * sabs
+
+
+def test_error_codes():
+    with pytest.raises(wk.WickError, match="kind"):
+        wk.build_terms([("x", 0)])
+    with pytest.raises(wk.WickError, match="gamma"):
+        wk.build_terms([("p", 4)])
+    with pytest.raises(wk.WickError, match="12 quarks"):
+        wk.build_terms([("p", g % 4) for g in range(7)])        # 14 u quarks
+    with pytest.raises(wk.WickError, match="n_nucleons"):
+        wk.build_terms([])
+    bad = np.array([[0, 12]], np.uint8)
+    ok = np.array([[0, 1]], np.uint8)
+    with pytest.raises(wk.WickError, match=">= 12"):
+        wk.build_terms_from_list(bad, ok, ok, ok, np.ones(1, complex))
+    lib = wk.load_library()
+    assert lib.wick_terms_get_info(None, None) == -1
+    assert lib.wick_contract_workspace_bytes(None, 4, 4, 1) == 0
+    # p0 p0 vanishes by Pauli: a legal, empty list
+    t = wk.build_terms([("p", 0), ("p", 0)])
+    assert t.info.n_terms == 0 and t.info.n_sink == 0
+
+
+def test_workspace_planning():
+    t = wk.build_terms(NUCLEI["cfg3"])
+    lo = wk.contract_workspace_bytes(t, 32, 64, 1, minimum=True)
+    hi = wk.contract_workspace_bytes(t, 32, 64, 1)
+    per_site = (429025 * 2) * 16
+    assert lo >= 32 * per_site + 64 * 32768 * 16
+    assert lo < hi <= (2 << 30) + 64 * 32768 * 16 + 4096
+    t0 = wk.build_terms(NUCLEI["cfg0"])
+    assert wk.contract_workspace_bytes(t0, 4, 8, 1) >= 512 * 585 * 16
