@@ -163,6 +163,17 @@ int wick_contract_host(const void* U_host, const void* D_host, const wick_terms*
 int wick_minor_dets(const void* P_dev, int64_t n_sites, int n, const uint8_t* rows, const uint8_t* cols,
                     int64_t n_minors, void* out_dev, void* cuda_stream);
 
+/* Measurement helpers (bench.py).  wick_profile_enable(1) makes every kernel launch of this thread's
+ * device calls record CUDA events on its stream; wick_profile_read synchronises them, returns the
+ * summed device time and launch count per class and clears the record.  Classes: 0 = u minors,
+ * 1 = d minors, 2 = weighted-product reduction, 3 = sigma finalisation + momentum projection.
+ * wick_measure_fp64_peak times a register-only DFMA stream on all SMs (the FP64 roofline
+ * denominator) and returns TFLOP/s; it synchronises. */
+typedef struct { double ms[4]; int64_t launches[4]; } wick_profile;
+int wick_profile_enable(int on);
+int wick_profile_read(wick_profile* out);
+int wick_measure_fp64_peak(double* tflops_out, void* cuda_stream);
+
 /* Number of kernel launches issued by this thread's device calls since the last reset (bench.py's
  * gpu_launches); _reset returns the old value. */
 int64_t wick_launch_count(void);

@@ -24,7 +24,7 @@ EXPORTED_SYMBOLS = (
     "wick_terms_export_minors", "wick_terms_export_terms", "wick_terms_export_factors", "wick_terms_free",
     "wick_contract_min_workspace_bytes", "wick_contract_workspace_bytes", "wick_contract",
     "wick_contract_host", "wick_minor_dets", "wick_launch_count", "wick_launch_count_reset",
-    "wick_last_error", "wick_version",
+    "wick_last_error", "wick_version", "wick_profile_enable", "wick_profile_read", "wick_measure_fp64_peak",
 )
 
 
@@ -44,6 +44,10 @@ class TermsInfo(C.Structure):
         ("is_outer_product", C.c_int32), ("n_sink", C.c_int32), ("n_source", C.c_int32),
         ("n_raw", C.c_int64), ("n_identity_merged", C.c_int64),
     ]
+
+
+class Profile(C.Structure):
+    _fields_ = [("ms", C.c_double * 4), ("launches", C.c_int64 * 4)]
 
 
 def library_path() -> str:
@@ -75,6 +79,9 @@ def load_library():
     lib.wick_contract.argtypes = [vp, vp, vp, vp, i32, i32, i32, vp, vp, vp, sz, u32, vp]
     lib.wick_contract_host.argtypes = [vp, vp, vp, vp, i32, i32, i32, vp, vp, u32]
     lib.wick_minor_dets.argtypes = [vp, i64, i32, vp, vp, i64, vp, vp]
+    lib.wick_profile_enable.argtypes = [i32]
+    lib.wick_profile_read.argtypes = [C.POINTER(Profile)]
+    lib.wick_measure_fp64_peak.argtypes = [C.POINTER(C.c_double), vp]
     lib.wick_launch_count.restype = i64
     lib.wick_launch_count_reset.restype = i64
     lib.wick_last_error.restype = C.c_char_p
@@ -260,3 +267,23 @@ def minor_dets(P, rows, cols, stream=None):
 def launch_count(reset: bool = False) -> int:
     lib = load_library()
     return int(lib.wick_launch_count_reset() if reset else lib.wick_launch_count())
+
+
+def profile_enable(on: bool = True) -> None:
+    _check(load_library().wick_profile_enable(1 if on else 0), "wick_profile_enable")
+
+
+def profile_read():
+    """Per-class device time (ms) and launch counts recorded since the last read:
+    {'minors_u': (ms, n), 'minors_d': ..., 'reduce': ..., 'project': ...}."""
+    p = Profile()
+    _check(load_library().wick_profile_read(C.byref(p)), "wick_profile_read")
+    names = ("minors_u", "minors_d", "reduce", "project")
+    return {k: (float(p.ms[i]), int(p.launches[i])) for i, k in enumerate(names)}
+
+
+def measure_fp64_peak(stream=None) -> float:
+    """TFLOP/s of a register-only DFMA stream on all SMs."""
+    out = C.c_double(0.0)
+    _check(load_library().wick_measure_fp64_peak(C.byref(out), _stream_ptr(stream)), "wick_measure_fp64_peak")
+    return float(out.value)

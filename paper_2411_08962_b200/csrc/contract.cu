@@ -201,6 +201,20 @@ extern "C" void wick_terms_release_device(DeviceTables* d) {
 extern "C" int64_t wick_launch_count(void) { return launch_counter_get(); }
 extern "C" int64_t wick_launch_count_reset(void) { return launch_counter_reset(); }
 
+extern "C" int wick_profile_enable(int on) { profile_enable(on != 0); return WICK_OK; }
+
+extern "C" int wick_profile_read(wick_profile* out) {
+    if (!out) { set_error("wick_profile_read: NULL argument"); return WICK_ERR_ARG; }
+    WICK_CUDA(profile_read(out->ms, out->launches));
+    return WICK_OK;
+}
+
+extern "C" int wick_measure_fp64_peak(double* tflops_out, void* cuda_stream) {
+    if (!tflops_out) { set_error("wick_measure_fp64_peak: NULL argument"); return WICK_ERR_ARG; }
+    WICK_CUDA(measure_fp64_peak(tflops_out, static_cast<cudaStream_t>(cuda_stream)));
+    return WICK_OK;
+}
+
 extern "C" size_t wick_contract_min_workspace_bytes(const wick_terms* t, int L, int T, int n_mom) {
     Plan p;
     if (!make_plan(t, L, T, n_mom, 0, true, &p)) return 0;
@@ -245,8 +259,8 @@ extern "C" int wick_contract(const void* U_dev, const void* D_dev, const wick_te
     for (int64_t st0 = 0; st0 < p.n_st; st0 += S_b) {
         const int64_t n_valid = std::min<int64_t>(S_b, p.n_st - st0);
         const int n_groups = int((n_valid + GROUP - 1) / GROUP);
-        WICK_CUDA(launch_minors(t->n_u, U, st0, p.n_st, n_groups, S_b, d.row_elem[0], d.col_elem[0], d.minor_rc[0], nmu, MU, stream));
-        WICK_CUDA(launch_minors(t->n_d, D, st0, p.n_st, n_groups, S_b, d.row_elem[1], d.col_elem[1], d.minor_rc[1], nmd, MD, stream));
+        WICK_CUDA(launch_minors(t->n_u, U, st0, p.n_st, n_groups, S_b, d.row_elem[0], d.col_elem[0], d.minor_rc[0], nmu, MU, PROF_MINORS_U, stream));
+        WICK_CUDA(launch_minors(t->n_d, D, st0, p.n_st, n_groups, S_b, d.row_elem[1], d.col_elem[1], d.minor_rc[1], nmd, MD, PROF_MINORS_D, stream));
         int n_chunks = 1;
         if (t->n_terms == 0) {
             WICK_CUDA(cudaMemsetAsync(sigma + st0, 0, size_t(n_valid) * 16, stream));
@@ -388,13 +402,13 @@ extern "C" int wick_minor_dets(const void* P_dev, int64_t n_sites, int n, const 
         if (direct) {
             WICK_CUDA_M(launch_minors(n, static_cast<const double2*>(P_dev), 0, n_sites, int(n_sites / GROUP), int(S_b),
                                       static_cast<const uint8_t*>(d_re), static_cast<const uint8_t*>(d_ce),
-                                      static_cast<const uint32_t*>(d_rc), nm, out, stream));
+                                      static_cast<const uint32_t*>(d_rc), nm, out, PROF_MINORS_U, stream));
         } else {
             for (int64_t s0 = 0; s0 < n_sites; s0 += S_b) {
                 const int64_t nv = std::min(S_b, n_sites - s0);
                 WICK_CUDA_M(launch_minors(n, static_cast<const double2*>(P_dev), s0, n_sites, int((nv + GROUP - 1) / GROUP), int(S_b),
                                           static_cast<const uint8_t*>(d_re), static_cast<const uint8_t*>(d_ce),
-                                          static_cast<const uint32_t*>(d_rc), nm, static_cast<double2*>(d_tmp), stream));
+                                          static_cast<const uint32_t*>(d_rc), nm, static_cast<double2*>(d_tmp), PROF_MINORS_U, stream));
                 WICK_CUDA_M(cudaMemcpy2DAsync(out + s0, size_t(n_sites) * 16, d_tmp, size_t(S_b) * 16, size_t(nv) * 16, size_t(nm),
                                               cudaMemcpyDeviceToDevice, stream));
             }

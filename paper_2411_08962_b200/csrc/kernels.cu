@@ -9,6 +9,8 @@
 //                            the active column and the multipliers (O(N^2) selects, not O(N^3)).
 //  a5  reduce_flat / reduce_outer : sigma(x,t) = sum_k w_k MU[uid_k] MD[did_k]  (Eq. A1-A5)
 //  a6  finalize_sigma, project    : fixed-order sum of the partials, momentum phases, fixed tree over sites
+#include <vector>
+
 #include "kernels.cuh"
 
 namespace wick {
@@ -18,6 +20,37 @@ typedef double2 c128;
 static thread_local int64_t g_launches = 0;
 int64_t launch_counter_get() { return g_launches; }
 int64_t launch_counter_reset() { const int64_t v = g_launches; g_launches = 0; return v; }
+
+// Optional per-launch timing (bench.py's roofline): CUDA events on the launching stream around every
+// kernel of a class, read back with profile_read().  Off by default; thread-local.
+struct ProfRec { cudaEvent_t a, b; int cls; };
+static thread_local bool g_prof_on = false;
+static thread_local std::vector<ProfRec> g_prof;
+void profile_enable(bool on) { g_prof_on = on; }
+struct ProfScope {
+    ProfRec r; cudaStream_t s; bool on;
+    ProfScope(int cls, cudaStream_t stream) : s(stream), on(g_prof_on) {
+        if (!on) return;
+        r.cls = cls;
+        cudaEventCreate(&r.a); cudaEventCreate(&r.b);
+        cudaEventRecord(r.a, s);
+    }
+    ~ProfScope() { if (on) { cudaEventRecord(r.b, s); g_prof.push_back(r); } }
+};
+cudaError_t profile_read(double ms[PROF_CLASSES], int64_t count[PROF_CLASSES]) {
+    for (int c = 0; c < PROF_CLASSES; ++c) { ms[c] = 0.0; count[c] = 0; }
+    cudaError_t err = cudaSuccess;
+    for (ProfRec& r : g_prof) {
+        float t = 0.f;
+        cudaError_t e = cudaEventSynchronize(r.b);
+        if (e == cudaSuccess) e = cudaEventElapsedTime(&t, r.a, r.b);
+        if (e != cudaSuccess) err = e;
+        ms[r.cls] += t; count[r.cls] += 1;
+        cudaEventDestroy(r.a); cudaEventDestroy(r.b);
+    }
+    g_prof.clear();
+    return err;
+}
 
 __device__ __forceinline__ c128 cmul(c128 a, c128 b) {
     return make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x);
@@ -303,7 +336,7 @@ minors_kernel(const c128* __restrict__ P, int64_t st0, int64_t n_st_total, int S
 template <int N>
 static cudaError_t launch_minors_n(const c128* P, int64_t st0, int64_t n_st_total, int n_groups, int S_b,
                                    const uint8_t* row_elem, const uint8_t* col_elem, const uint32_t* minor_rc,
-                                   int64_t n_minors, c128* out, cudaStream_t stream) {
+                                   int64_t n_minors, c128* out, int prof_cls, cudaStream_t stream) {
     constexpr int NT = MinorCfg<N>::kThreads;
     constexpr int warps = NT / 32;
     // enough CTAs for ~4 waves on 148 SMs, but at least 2 minors per warp per CTA
@@ -316,6 +349,7 @@ static cudaError_t launch_minors_n(const c128* P, int64_t st0, int64_t n_st_tota
     chunk = ((chunk + warps - 1) / warps) * warps;            // every warp of a CTA gets the same count
     chunks = int((n_minors + chunk - 1) / chunk);
     dim3 grid(n_groups, chunks);
+    ProfScope prof(prof_cls, stream);
     minors_kernel<N><<<grid, NT, MinorCfg<N>::kSmem, stream>>>(P, st0, n_st_total, S_b, row_elem, col_elem,
                                                              minor_rc, int(n_minors), chunk, out);
     ++g_launches;
@@ -324,9 +358,9 @@ static cudaError_t launch_minors_n(const c128* P, int64_t st0, int64_t n_st_tota
 
 cudaError_t launch_minors(int n, const double2* P, int64_t st0, int64_t n_st_total, int n_groups, int S_b,
                           const uint8_t* row_elem, const uint8_t* col_elem, const uint32_t* minor_rc,
-                          int64_t n_minors, double2* out, cudaStream_t stream) {
+                          int64_t n_minors, double2* out, int prof_cls, cudaStream_t stream) {
     if (n_minors == 0 || n_groups == 0) return cudaSuccess;
-#define WICK_CASE(N) case N: return launch_minors_n<N>(P, st0, n_st_total, n_groups, S_b, row_elem, col_elem, minor_rc, n_minors, out, stream);
+#define WICK_CASE(N) case N: return launch_minors_n<N>(P, st0, n_st_total, n_groups, S_b, row_elem, col_elem, minor_rc, n_minors, out, prof_cls, stream);
     switch (n) {
         WICK_CASE(0) WICK_CASE(1) WICK_CASE(2) WICK_CASE(3) WICK_CASE(4) WICK_CASE(5) WICK_CASE(6)
         WICK_CASE(7) WICK_CASE(8) WICK_CASE(9) WICK_CASE(10) WICK_CASE(11) WICK_CASE(12)
@@ -432,6 +466,7 @@ cudaError_t launch_reduce_flat(const double2* MU, const double2* MD, int n_group
     chunks = chunk > 0 ? int((n_terms + chunk - 1) / chunk) : 1;
     if (chunks < 1) chunks = 1;
     dim3 grid(n_groups, chunks);
+    ProfScope prof(PROF_REDUCE, stream);
     reduce_flat_kernel<<<grid, RED_THREADS, 0, stream>>>(MU, MD, S_b, uid, did, w, n_terms, chunk > 0 ? chunk : 1, partial);
     ++g_launches;
     *n_chunks_out = chunks;
@@ -451,6 +486,7 @@ cudaError_t launch_reduce_outer(const double2* MU, const double2* MD, int n_grou
     const int rows_per_cta = (n_rows_u + chunks - 1) / chunks;
     chunks = (n_rows_u + rows_per_cta - 1) / rows_per_cta;
     dim3 grid(n_groups, chunks);
+    ProfScope prof(PROF_REDUCE, stream);
     reduce_outer_kernel<<<grid, RED_THREADS, 0, stream>>>(MU, MD, S_b, n_rows_u, n_cols_u, n_cols_d, sink_ptr, sink_rd,
                                                           sink_c, src_ptr, src_cu, src_c, rows_per_cta, partial);
     ++g_launches;
@@ -474,6 +510,7 @@ cudaError_t launch_finalize_sigma(const double2* partial, int n_chunks, int S_b,
                                   double2* sigma_batch, cudaStream_t stream) {
     if (n_valid <= 0) return cudaSuccess;
     const int threads = 128;
+    ProfScope prof(PROF_PROJECT, stream);
     finalize_sigma_kernel<<<unsigned((n_valid + threads - 1) / threads), threads, 0, stream>>>(partial, n_chunks, S_b, n_valid, sigma_batch);
     ++g_launches;
     return cudaGetLastError();
@@ -518,9 +555,53 @@ cudaError_t launch_project(const double2* sigma, int L, int T, const MomentumLis
                            cudaStream_t stream) {
     if (T <= 0 || mom.n <= 0) return cudaSuccess;
     dim3 grid(T, mom.n);
+    ProfScope prof(PROF_PROJECT, stream);
     project_kernel<<<grid, PROJ_THREADS, 0, stream>>>(sigma, L, T, mom, C_out);
     ++g_launches;
     return cudaGetLastError();
+}
+
+
+// ---------------------------------------------------------------------------------------------
+// Measurement helper: register-only DFMA stream (the FP64 roofline denominator)
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) dfma_probe_kernel(double* out, int iters, double a, double b) {
+    double x[8];
+#pragma unroll
+    for (int k = 0; k < 8; ++k) x[k] = double(threadIdx.x + k);
+    for (int i = 0; i < iters; ++i) {
+#pragma unroll
+        for (int k = 0; k < 8; ++k) x[k] = fma(x[k], a, b);
+    }
+    double s = 0.0;
+#pragma unroll
+    for (int k = 0; k < 8; ++k) s += x[k];
+    if (s == 12345.678) out[0] = s;                              // never true: keeps the chain alive
+}
+
+cudaError_t measure_fp64_peak(double* tflops, cudaStream_t stream) {
+    double* d = nullptr;
+    cudaError_t e = cudaMalloc(&d, 8);
+    if (e != cudaSuccess) return e;
+    cudaEvent_t a, b;
+    cudaEventCreate(&a); cudaEventCreate(&b);
+    const int blocks = 148 * 8, iters = 1 << 15;
+    double best = 0.0;
+    for (int rep = 0; rep < 5; ++rep) {
+        cudaEventRecord(a, stream);
+        dfma_probe_kernel<<<blocks, 256, 0, stream>>>(d, iters, 0.999999, 1e-9);
+        cudaEventRecord(b, stream);
+        e = cudaEventSynchronize(b);
+        if (e != cudaSuccess) break;
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, a, b);
+        const double tf = 2.0 * 8.0 * double(iters) * 256.0 * blocks / (double(ms) * 1e-3) / 1e12;
+        if (rep > 0 && tf > best) best = tf;                     // rep 0 is the warm-up
+    }
+    cudaEventDestroy(a); cudaEventDestroy(b);
+    cudaFree(d);
+    *tflops = best;
+    return e;
 }
 
 }  // namespace wick

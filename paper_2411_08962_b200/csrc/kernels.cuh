@@ -19,10 +19,16 @@ constexpr int MAX_MOMENTA = 64;
 
 struct MomentumList { int n; int v[MAX_MOMENTA][3]; };
 
+// profiling classes (wick_profile in include/wick.h)
+constexpr int PROF_MINORS_U = 0, PROF_MINORS_D = 1, PROF_REDUCE = 2, PROF_PROJECT = 3, PROF_CLASSES = 4;
+void profile_enable(bool on);
+cudaError_t profile_read(double ms[PROF_CLASSES], int64_t count[PROF_CLASSES]);
+cudaError_t measure_fp64_peak(double* tflops, cudaStream_t stream);
+
 // launchers (kernels.cu); all enqueue on `stream` and return the cudaGetLastError() code
 cudaError_t launch_minors(int n, const double2* P, int64_t st0, int64_t n_st_total, int n_groups, int S_b,
                           const uint8_t* row_elem, const uint8_t* col_elem, const uint32_t* minor_rc,
-                          int64_t n_minors, double2* out, cudaStream_t stream);
+                          int64_t n_minors, double2* out, int prof_cls, cudaStream_t stream);
 cudaError_t launch_reduce_flat(const double2* MU, const double2* MD, int n_groups, int S_b,
                                const int32_t* uid, const int32_t* did, const double2* w, int64_t n_terms,
                                double2* partial, int* n_chunks_out, int max_chunks, cudaStream_t stream);

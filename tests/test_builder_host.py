@@ -29,7 +29,7 @@ def test_library_exports_every_declared_symbol():
     lib = wk.load_library()
     with open("include/wick.h") as f:
         header = f.read()
-    declared = set(re.findall(r"\b(wick_[a-z_]+)\s*\(", header))
+    declared = set(re.findall(r"\b(wick_[a-z_0-9]+)\s*\(", header))
     assert declared == set(wk.EXPORTED_SYMBOLS)
     for name in declared:
         assert getattr(lib, name) is not None

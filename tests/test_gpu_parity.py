@@ -1,0 +1,251 @@
+"""GPU parity tests (-m gpu): the CUDA path, called through the C-ABI binding, against the CPU oracle on
+the same seeded inputs.  Tolerance (BASELINE.json north_star): |C_gpu - C_oracle| <= 1e-10 * S_abs(t),
+S_abs(t) = sum_x sum_terms |w detU detD| (oracle).  Per-site sigma uses the per-site S_abs.
+
+What runs where: full-lattice C(t) for cfg 0 at full size and for every
+other config on a shrunken lattice with the FULL term list; at BASELINE's full sizes per-site sigma on
+a seeded sample of sites (cfg 1-4), the device reduction against a CPU sum of the device sigma, and
+closed-form structural checks (site-scaled propagators) with a one-site oracle."""
+import numpy as np
+import pytest
+import torch
+
+import paper_2411_08962_b200 as wk
+from oracle import wick_oracle as wo
+from wick_inputs import CONFIGS, make_propagators_numpy, make_random_term_list, sample_site_times
+
+pytestmark = pytest.mark.gpu
+REL_TOL = 1e-10
+
+
+def _dev(a, device):
+    return torch.from_numpy(np.ascontiguousarray(a)).to(device)
+
+
+def _terms_for(cfg):
+    c = CONFIGS[cfg]
+    if c.random_list:
+        return wk.build_terms_from_list(*make_random_term_list(c.seed, c.n_u, c.n_d, c.n_random_terms))
+    return wk.build_terms(c.nucleus)
+
+
+_SINK_CACHE = {}
+
+
+def _oracle_site(cfg, U, D):
+    """sigma and S_abs of one site from the oracle's OWN expansion (never from the builder's tables)."""
+    c = CONFIGS[cfg]
+    if c.random_list:
+        a_u, b_u, a_d, b_d, w = make_random_term_list(c.seed, c.n_u, c.n_d, c.n_random_terms)
+        return wo.site_terms_value(U, D, a_u, b_u, a_d, b_d, w)
+    if cfg not in _SINK_CACHE:
+        _SINK_CACHE[cfg] = wo.merged_terms(c.nucleus)
+    return wo.site_value_outer(U, D, _SINK_CACHE[cfg])
+
+
+def _oracle_lattice(cfg, U, D, momenta, L):
+    T, V = U.shape[:2]
+    sigma = np.zeros((T, V), complex)
+    sabs = np.zeros((T, V))
+    for t in range(T):
+        for s in range(V):
+            sigma[t, s], sabs[t, s] = _oracle_site(cfg, U[t, s], D[t, s])
+    return wo.reduce_sites(sigma, momenta, L), sigma, sabs
+
+
+# ---------------------------------------------------------------------------------------------
+# a4 alone: every minor size, ragged site counts, unsorted index tuples
+# ---------------------------------------------------------------------------------------------
+
+@pytest.mark.parametrize("n", list(range(0, 13)))
+@pytest.mark.parametrize("n_sites", [70, 64])
+def test_minor_dets_vs_oracle(n, n_sites, cuda_device):
+    rng = np.random.default_rng(100 + n)
+    P = rng.standard_normal((n_sites, 12, 12)) + 1j * rng.standard_normal((n_sites, 12, 12))
+    P[3] *= 1e-3                                                # scale spread across sites
+    P[5, 2, :] = 0.0                                            # an exactly zero row: singular minors
+    n_minors = 37 if n_sites == 70 else 300                      # spans several warps and a ragged tail
+    rows = np.array([rng.permutation(12)[:n] for _ in range(n_minors)], np.uint8).reshape(n_minors, n)
+    cols = np.array([rng.permutation(12)[:n] for _ in range(n_minors)], np.uint8).reshape(n_minors, n)
+    got = wk.minor_dets(_dev(P, cuda_device), rows, cols).cpu().numpy()
+    assert got.shape == (n_minors, n_sites)
+    if n == 0:
+        assert np.all(got == 1.0)
+        return
+    sub = P[:, rows[:, :, None], cols[:, None, :]]              # [site][minor][n][n]
+    ref = wo.det_elim(sub).T
+    # Hadamard bound prod_i ||row_i|| is the natural scale of the rounding error of a determinant
+    scale = np.prod(np.linalg.norm(sub, axis=3), axis=2).T
+    assert np.all(np.abs(got - ref) <= 1e-13 * n * scale + 1e-300)
+    zero_row = np.any(rows == 2, axis=1)
+    assert np.all(got[zero_row, 5] == 0.0)                      # exact zeros, no NaN from a zero pivot
+    assert np.all(np.isfinite(got.view(np.float64)))
+
+
+def test_minor_dets_repeated_index_is_zero(cuda_device):
+    rng = np.random.default_rng(7)
+    P = rng.standard_normal((32, 12, 12)) + 1j * rng.standard_normal((32, 12, 12))
+    for n in (2, 3, 4, 6, 10):
+        rows = np.array([list(range(n))], np.uint8)
+        rows[0, n - 1] = rows[0, 0]                             # Pauli: repeated row index
+        cols = np.array([list(range(1, n + 1))], np.uint8)
+        got = wk.minor_dets(_dev(P, cuda_device), rows, cols).cpu().numpy()
+        scale = np.prod(np.linalg.norm(P[:, rows[0]][:, :, cols[0]], axis=2), axis=1)
+        assert np.all(np.abs(got[0]) <= 1e-13 * n * scale)
+
+
+# ---------------------------------------------------------------------------------------------
+# full path, full lattice
+# ---------------------------------------------------------------------------------------------
+
+def _check_C(C_gpu, C_ref, sabs_t):
+    err = np.abs(C_gpu - C_ref)
+    assert np.all(err <= REL_TOL * sabs_t[None, :]), (err / sabs_t[None, :]).max()
+
+
+@pytest.mark.parametrize("flags", [0, wk.CONTRACT_FORCE_FLAT])
+def test_cfg0_proton_full_lattice(flags, cuda_device):
+    c = CONFIGS["cfg0"]
+    U, D = make_propagators_numpy(c.seed, c.L, c.T)
+    mom = [(0, 0, 0), (1, 0, 0), (0, 1, 2), (-1, 3, 0)]
+    t = wk.build_terms(c.nucleus)
+    Cg, sg = wk.contract(_dev(U, cuda_device), _dev(D, cuda_device), t, mom, c.L, c.T, want_sigma=True, flags=flags)
+    Cg, sg = Cg.cpu().numpy(), sg.cpu().numpy()
+    Cr, sr, sabs = _oracle_lattice("cfg0", U, D, mom, c.L)
+    assert np.all(np.abs(sg - sr) <= REL_TOL * sabs)
+    _check_C(Cg, Cr, sabs.sum(axis=1))
+    # RAW-mode oracle (no sorting, no merging) on one timeslice
+    raw = wo.nucleus_raw_terms(c.nucleus)
+    for s in (0, 17, 63):
+        v = wo.raw_site_value(U[3, s], D[3, s], raw, raw)
+        assert abs(sg[3, s] - v) <= REL_TOL * sabs[3, s]
+
+
+SHRUNK = {  # cfg -> (L, T, momenta): full term list, lattice the oracle finishes in about a minute
+    "cfg1": (3, 2, [(0, 0, 0), (1, 0, 0)]),
+    "cfg2": (2, 2, [(0, 0, 0), (1, 0, 0)]),
+    "cfg3": (2, 1, [(0, 0, 0)]),
+    "cfg4": (4, 3, [(0, 0, 0), (0, 0, 1)]),
+    "cfg4b": (4, 3, [(0, 0, 0), (1, 1, 1)]),
+}
+
+
+@pytest.mark.parametrize("cfg", ["cfg1", "cfg2", "cfg3", "cfg4", "cfg4b"])
+def test_shrunken_lattice_full_term_list(cfg, cuda_device):
+    c = CONFIGS[cfg]
+    L, T, mom = SHRUNK[cfg]
+    U, D = make_propagators_numpy(c.seed, L, T)
+    t = _terms_for(cfg)
+    Cg, sg = wk.contract(_dev(U, cuda_device), _dev(D, cuda_device), t, mom, L, T, want_sigma=True)
+    Cg, sg = Cg.cpu().numpy(), sg.cpu().numpy()
+    Cr, sr, sabs = _oracle_lattice(cfg, U, D, mom, L)
+    assert np.all(np.abs(sg - sr) <= REL_TOL * sabs), (np.abs(sg - sr) / sabs).max()
+    _check_C(Cg, Cr, sabs.sum(axis=1))
+    if cfg in ("cfg1", "cfg4"):                                 # the flat path on the same list
+        Cf = wk.contract(_dev(U, cuda_device), _dev(D, cuda_device), t, mom, L, T, flags=wk.CONTRACT_FORCE_FLAT)
+        _check_C(Cf.cpu().numpy(), Cr, sabs.sum(axis=1))
+
+
+# ---------------------------------------------------------------------------------------------
+# BASELINE's full sizes: sampled sites + device reduction + structure
+# ---------------------------------------------------------------------------------------------
+
+FULL = {  # cfg -> (timeslices to run, sites sampled per timeslice)
+    "cfg1": ([0, 16, 31], 6),
+    "cfg2": ([47], 4),
+    "cfg3": ([63], 3),
+    "cfg4": ([0, 47], 8),
+    "cfg4b": ([24], 8),
+}
+
+
+@pytest.mark.parametrize("cfg", ["cfg1", "cfg2", "cfg3", "cfg4", "cfg4b"])
+def test_full_size_sampled_sites_and_reduction(cfg, cuda_device):
+    c = CONFIGS[cfg]
+    times, n_sites = FULL[cfg]
+    t = _terms_for(cfg)
+    for tt in times:
+        U, D = make_propagators_numpy(c.seed, c.L, c.T, t0=tt, nt=1)
+        Cg, sg = wk.contract(_dev(U, cuda_device), _dev(D, cuda_device), t, c.momenta, c.L, 1, want_sigma=True)
+        Cg, sg = Cg.cpu().numpy(), sg.cpu().numpy()
+        assert np.all(np.isfinite(sg.view(np.float64)))
+        for (_, s) in sample_site_times(c.seed, c.L, c.T, n_sites, times=[tt]):
+            ref, sabs = _oracle_site(cfg, U[0, s], D[0, s])
+            assert abs(sg[0, s] - ref) <= REL_TOL * sabs, (cfg, tt, s, abs(sg[0, s] - ref) / sabs)
+        # device reduction (momentum phases + fixed tree) against the oracle's sum of the device sigma
+        Cr = wo.reduce_sites(sg, c.momenta, c.L)
+        assert np.all(np.abs(Cg - Cr) <= 1e-13 * np.sum(np.abs(sg)))
+
+
+@pytest.mark.parametrize("cfg", ["cfg2", "cfg3"])
+def test_full_size_site_scaled_propagators(cfg, cuda_device):
+    """U_x = s_x U0 with s_x = exp(-i p.x / n_u), D_x = D0: the projection at momentum p returns
+    L^3 sigma0, at another momentum 0; sigma0 from a one-site oracle call."""
+    c = CONFIGS[cfg]
+    L = c.L
+    rng = np.random.default_rng(c.seed)
+    U0 = rng.standard_normal((12, 12)) + 1j * rng.standard_normal((12, 12))
+    D0 = rng.standard_normal((12, 12)) + 1j * rng.standard_normal((12, 12))
+    p = np.array([1, 0, 0])
+    s = np.arange(L ** 3)
+    xyz = np.stack([s % L, (s // L) % L, s // (L * L)], axis=1)
+    sx = np.exp(-2j * np.pi * (xyz @ p) / L / c.n_u)
+    U = (U0[None] * sx[:, None, None])[None]
+    D = np.broadcast_to(D0, (1, L ** 3, 12, 12)).copy()
+    t = _terms_for(cfg)
+    mom = [(1, 0, 0), (0, 0, 0), (0, 1, 0)]
+    Cg = wk.contract(_dev(U, cuda_device), _dev(D, cuda_device), t, mom, L, 1).cpu().numpy()
+    sigma0, sabs0 = _oracle_site(cfg, U0, D0)
+    tol = REL_TOL * sabs0 * L ** 3
+    assert abs(Cg[0, 0] - L ** 3 * sigma0) <= tol
+    assert abs(Cg[1, 0]) <= tol and abs(Cg[2, 0]) <= tol
+
+
+# ---------------------------------------------------------------------------------------------
+# edge cases, determinism, host entry point
+# ---------------------------------------------------------------------------------------------
+
+def test_ragged_lattices_small_workspace_and_determinism(cuda_device):
+    c = CONFIGS["cfg1"]
+    t = wk.build_terms(c.nucleus)
+    for L, T in ((1, 1), (3, 3), (5, 1)):                       # V = 1, 27, 125: not multiples of 32
+        U, D = make_propagators_numpy(77, L, T)
+        mom = [(0, 0, 0), (1, 2, 0)]
+        Ud, Dd = _dev(U, cuda_device), _dev(D, cuda_device)
+        C1, s1 = wk.contract(Ud, Dd, t, mom, L, T, want_sigma=True)
+        C2 = wk.contract(Ud, Dd, t, mom, L, T)
+        assert torch.equal(C1, C2)                              # bit-reproducible run to run
+        ws = torch.empty(wk.contract_workspace_bytes(t, L, T, 2, minimum=True), dtype=torch.uint8, device=cuda_device)
+        C3, s3 = wk.contract(Ud, Dd, t, mom, L, T, workspace=ws, want_sigma=True)   # 32-site batches
+        Cr, sr, sabs = _oracle_lattice("cfg1", U, D, mom, L)
+        assert np.all(np.abs(s1.cpu().numpy() - sr) <= REL_TOL * sabs)
+        assert np.all(np.abs(s3.cpu().numpy() - sr) <= REL_TOL * sabs)
+        _check_C(C1.cpu().numpy(), Cr, sabs.sum(axis=1))
+        _check_C(C3.cpu().numpy(), Cr, sabs.sum(axis=1))
+    with pytest.raises(wk.WickError, match="workspace"):
+        wk.contract(Ud, Dd, t, mom, L, T, workspace=torch.empty(1024, dtype=torch.uint8, device=cuda_device))
+
+
+def test_empty_term_list_and_isospin_alias(cuda_device):
+    U, D = make_propagators_numpy(5, 2, 2)
+    Ud, Dd = _dev(U, cuda_device), _dev(D, cuda_device)
+    empty = wk.build_terms([("p", 0), ("p", 0)])                # Pauli-blocked: no terms
+    C = wk.contract(Ud, Dd, empty, [(0, 0, 0)], 2, 2)
+    assert torch.all(C == 0)
+    t = wk.build_terms(CONFIGS["cfg0"].nucleus)
+    C = wk.contract(Ud, Ud, t, [(0, 0, 0)], 2, 2).cpu().numpy()  # U_dev == D_dev is legal
+    Cr, _, sabs = _oracle_lattice("cfg0", U, U, [(0, 0, 0)], 2)
+    _check_C(C, Cr, sabs.sum(axis=1))
+
+
+def test_contract_host_matches_device_call(cuda_device):
+    c = CONFIGS["cfg0"]
+    U, D = make_propagators_numpy(c.seed, c.L, c.T)
+    t = wk.build_terms(c.nucleus)
+    mom = [(0, 0, 0), (1, 1, 0)]
+    Ch, sh = wk.contract_host(U, D, t, mom, c.L, c.T, want_sigma=True)
+    Cd, sd = wk.contract(_dev(U, cuda_device), _dev(D, cuda_device), t, mom, c.L, c.T, want_sigma=True)
+    assert np.array_equal(sh, sd.cpu().numpy())
+    assert np.array_equal(Ch, Cd.cpu().numpy())
+    n0 = wk.launch_count(reset=True)
+    assert n0 > 0
