@@ -57,6 +57,108 @@ std::vector<uint8_t> elem_table(const std::vector<uint16_t>& masks, int scale) {
     return out;
 }
 
+
+// Connected components of the bipartite graph (qu -- qd) of a factor list.  Physical sink lists are
+// block diagonal (He-4: 199 blocks of at most 15 x 15 tuples), so the factorised reduction
+//   sigma = sum_{ru,cd} (sum_i c_i MD[rd_i,cd]) (sum_j cbar_j MU[ru,cu_j])
+// splits into (sink block, source block) items that each touch a small, disjoint set of minors:
+// every MU / MD element belongs to exactly one item, so the minor buffers are read from DRAM once.
+struct Components { std::vector<int> of_u, of_d; int n = 0; };
+
+Components factor_components(int n_u, int n_d, const std::vector<FactorTerm>& list) {
+    std::vector<int> parent(size_t(n_u) + size_t(n_d));
+    for (size_t i = 0; i < parent.size(); ++i) parent[i] = int(i);
+    auto find = [&](int x) { while (parent[x] != x) { parent[x] = parent[parent[x]]; x = parent[x]; } return x; };
+    for (const FactorTerm& f : list) {
+        const int a = find(f.qu), b = find(n_u + f.qd);
+        if (a != b) parent[std::max(a, b)] = std::min(a, b);
+    }
+    Components c;
+    c.of_u.assign(n_u, -1); c.of_d.assign(n_d, -1);
+    std::vector<int> label(parent.size(), -1);
+    for (const FactorTerm& f : list) {                        // label in order of first appearance
+        const int r = find(f.qu);
+        if (label[r] < 0) label[r] = c.n++;
+        c.of_u[f.qu] = label[r]; c.of_d[f.qd] = label[r];
+    }
+    return c;
+}
+
+constexpr int MAX_RED_BINS = 2048;               // warps of work per site group (8 per CTA -> 256 partial rows)
+
+struct ReduceSchedule {
+    std::vector<int32_t> ru_ptr, ru_list, cd_ptr, cd_list, bin_ptr, items;
+    int n_bins = 0;
+};
+
+// items = (sink block k, source block k'); cost = complex FMAs of its (ru, cd) double loop.
+// Longest-processing-time assignment to n_bins warps; every bin's item order is fixed, so the
+// reduction stays bit-reproducible.
+ReduceSchedule build_reduce_schedule(const wick_terms* t, const std::vector<int32_t>& sink_ptr,
+                                     const std::vector<int32_t>& src_ptr) {
+    const int nru = int(t->f[0].rows.size()), nrd = int(t->f[1].rows.size());
+    const int ncu = int(t->f[0].cols.size()), ncd = int(t->f[1].cols.size());
+    const Components cs = factor_components(nru, nrd, t->sink);
+    const Components cq = factor_components(ncu, ncd, t->source);
+    ReduceSchedule r;
+    auto group = [](const std::vector<int>& comp_of, int n_comp, std::vector<int32_t>& ptr, std::vector<int32_t>& list) {
+        ptr.assign(size_t(n_comp) + 1, 0);
+        for (int c : comp_of) if (c >= 0) ptr[size_t(c) + 1]++;
+        for (int c = 0; c < n_comp; ++c) ptr[size_t(c) + 1] += ptr[size_t(c)];
+        list.resize(size_t(ptr[size_t(n_comp)]));
+        std::vector<int32_t> fill(ptr.begin(), ptr.end() - 1);
+        for (size_t x = 0; x < comp_of.size(); ++x) if (comp_of[x] >= 0) list[size_t(fill[size_t(comp_of[x])]++)] = int32_t(x);
+    };
+    group(cs.of_u, cs.n, r.ru_ptr, r.ru_list);
+    group(cq.of_d, cq.n, r.cd_ptr, r.cd_list);
+    std::vector<int64_t> nnz_s(size_t(cs.n), 0), nnz_q(size_t(cq.n), 0);
+    for (int k = 0; k < cs.n; ++k)
+        for (int a = r.ru_ptr[size_t(k)]; a < r.ru_ptr[size_t(k) + 1]; ++a) {
+            const int ru = r.ru_list[size_t(a)];
+            nnz_s[size_t(k)] += sink_ptr[size_t(ru) + 1] - sink_ptr[size_t(ru)];
+        }
+    for (int k = 0; k < cq.n; ++k)
+        for (int b = r.cd_ptr[size_t(k)]; b < r.cd_ptr[size_t(k) + 1]; ++b) {
+            const int cd = r.cd_list[size_t(b)];
+            nnz_q[size_t(k)] += src_ptr[size_t(cd) + 1] - src_ptr[size_t(cd)];
+        }
+    struct Item { int64_t cost; int32_t k, kp; };
+    std::vector<Item> items;
+    items.reserve(size_t(cs.n) * size_t(cq.n));
+    for (int k = 0; k < cs.n; ++k) {
+        const int64_t na = r.ru_ptr[size_t(k) + 1] - r.ru_ptr[size_t(k)];
+        for (int kp = 0; kp < cq.n; ++kp) {
+            const int64_t nb = r.cd_ptr[size_t(kp) + 1] - r.cd_ptr[size_t(kp)];
+            items.push_back({nb * nnz_s[size_t(k)] + na * nnz_q[size_t(kp)] + na * nb + 4, k, kp});
+        }
+    }
+    std::stable_sort(items.begin(), items.end(), [](const Item& a, const Item& b) { return a.cost > b.cost; });
+    int n_bins = int(std::min<size_t>(items.size(), size_t(MAX_RED_BINS)));
+    n_bins = std::max(8, (n_bins + 7) / 8 * 8);
+    std::vector<int64_t> load(size_t(n_bins), 0);
+    std::vector<std::vector<int32_t>> bins(static_cast<size_t>(n_bins));
+    // min-heap over (load, bin)
+    std::vector<std::pair<int64_t, int>> heap;
+    for (int b = 0; b < n_bins; ++b) heap.push_back({0, b});
+    auto cmp = [](const std::pair<int64_t, int>& a, const std::pair<int64_t, int>& b) { return a > b; };
+    std::make_heap(heap.begin(), heap.end(), cmp);
+    for (const Item& it : items) {
+        std::pop_heap(heap.begin(), heap.end(), cmp);
+        std::pair<int64_t, int>& top = heap.back();
+        bins[size_t(top.second)].push_back(it.k);
+        bins[size_t(top.second)].push_back(it.kp);
+        top.first += it.cost;
+        std::push_heap(heap.begin(), heap.end(), cmp);
+    }
+    r.n_bins = n_bins;
+    r.bin_ptr.assign(size_t(n_bins) + 1, 0);
+    for (int b = 0; b < n_bins; ++b) {
+        r.bin_ptr[size_t(b) + 1] = r.bin_ptr[size_t(b)] + int32_t(bins[size_t(b)].size() / 2);
+        r.items.insert(r.items.end(), bins[size_t(b)].begin(), bins[size_t(b)].end());
+    }
+    return r;
+}
+
 // Upload minor tables and factor lists once per handle and device.
 int upload_tables(const wick_terms* t, cudaStream_t stream) {
     std::lock_guard<std::mutex> lock(t->mu);
@@ -78,6 +180,8 @@ int upload_tables(const wick_terms* t, cudaStream_t stream) {
         o_rc[f] = bb.add(rc.data(), rc.size() * 4);
     }
     size_t o_sp = 0, o_srd = 0, o_sc = 0, o_qp = 0, o_qcu = 0, o_qc = 0;
+    size_t o_srdoff = 0, o_rup = 0, o_rul = 0, o_cdp = 0, o_cdl = 0, o_binp = 0, o_items = 0;
+    int n_red_bins = 0;
     if (t->outer) {
         const int nru = int(t->f[0].rows.size()), ncd = int(t->f[1].cols.size());
         // sink is sorted by (ru, rd): CSR over ru
@@ -105,6 +209,14 @@ int upload_tables(const wick_terms* t, cudaStream_t stream) {
         for (int c = 0; c < ncd; ++c) qp[c + 1] += qp[c];
         o_sp = bb.add(sp.data(), sp.size() * 4); o_srd = bb.add(srd.data(), srd.size() * 4); o_sc = bb.add(sc.data(), sc.size() * 8);
         o_qp = bb.add(qp.data(), qp.size() * 4); o_qcu = bb.add(qcu.data(), qcu.size() * 4); o_qc = bb.add(qc.data(), qc.size() * 8);
+        std::vector<int32_t> srdoff(srd.size());
+        for (size_t i = 0; i < srd.size(); ++i) srdoff[i] = srd[i] * ncd;
+        const ReduceSchedule rs = build_reduce_schedule(t, sp, qp);
+        n_red_bins = rs.n_bins;
+        o_srdoff = bb.add(srdoff.data(), srdoff.size() * 4);
+        o_rup = bb.add(rs.ru_ptr.data(), rs.ru_ptr.size() * 4); o_rul = bb.add(rs.ru_list.data(), rs.ru_list.size() * 4);
+        o_cdp = bb.add(rs.cd_ptr.data(), rs.cd_ptr.size() * 4); o_cdl = bb.add(rs.cd_list.data(), rs.cd_list.size() * 4);
+        o_binp = bb.add(rs.bin_ptr.data(), rs.bin_ptr.size() * 4); o_items = bb.add(rs.items.data(), rs.items.size() * 4);
     }
     void* blob = nullptr;
     WICK_CUDA(cudaMalloc(&blob, std::max<size_t>(bb.host.size(), 256)));
@@ -124,6 +236,12 @@ int upload_tables(const wick_terms* t, cudaStream_t stream) {
         d.src_ptr = reinterpret_cast<const int32_t*>(b + o_qp);
         d.src_cu = reinterpret_cast<const int32_t*>(b + o_qcu);
         d.src_c = reinterpret_cast<const double*>(b + o_qc);
+        d.sink_rdoff = reinterpret_cast<const int32_t*>(b + o_srdoff);
+        d.ru_ptr = reinterpret_cast<const int32_t*>(b + o_rup); d.ru_list = reinterpret_cast<const int32_t*>(b + o_rul);
+        d.cd_ptr = reinterpret_cast<const int32_t*>(b + o_cdp); d.cd_list = reinterpret_cast<const int32_t*>(b + o_cdl);
+        d.red_bin_ptr = reinterpret_cast<const int32_t*>(b + o_binp);
+        d.red_items = reinterpret_cast<const int32_t*>(b + o_items);
+        d.n_red_bins = n_red_bins;
     }
     d.blob = blob;
     d.device = dev;
@@ -266,10 +384,13 @@ extern "C" int wick_contract(const void* U_dev, const void* D_dev, const wick_te
             WICK_CUDA(cudaMemsetAsync(sigma + st0, 0, size_t(n_valid) * 16, stream));
         } else {
             if (use_outer) {
-                WICK_CUDA(launch_reduce_outer(MU, MD, n_groups, S_b, int(t->f[0].rows.size()), int(t->f[0].cols.size()),
-                                              int(t->f[1].cols.size()), d.sink_ptr, d.sink_rd,
-                                              reinterpret_cast<const double2*>(d.sink_c), d.src_ptr, d.src_cu,
-                                              reinterpret_cast<const double2*>(d.src_c), partial, &n_chunks, MAX_CHUNKS, stream));
+                OuterTables ot;
+                ot.n_cols_u = int(t->f[0].cols.size()); ot.n_cols_d = int(t->f[1].cols.size());
+                ot.sink_ptr = d.sink_ptr; ot.sink_rdoff = d.sink_rdoff; ot.sink_c = reinterpret_cast<const double2*>(d.sink_c);
+                ot.src_ptr = d.src_ptr; ot.src_cu = d.src_cu; ot.src_c = reinterpret_cast<const double2*>(d.src_c);
+                ot.ru_ptr = d.ru_ptr; ot.ru_list = d.ru_list; ot.cd_ptr = d.cd_ptr; ot.cd_list = d.cd_list;
+                ot.bin_ptr = d.red_bin_ptr; ot.items = reinterpret_cast<const int2*>(d.red_items); ot.n_bins = d.n_red_bins;
+                WICK_CUDA(launch_reduce_outer(MU, MD, n_groups, S_b, ot, partial, &n_chunks, stream));
             } else {
                 WICK_CUDA(launch_reduce_flat(MU, MD, n_groups, S_b, d.t_uid, d.t_did, reinterpret_cast<const double2*>(d.t_w),
                                              t->n_terms, partial, &n_chunks, MAX_CHUNKS, stream));

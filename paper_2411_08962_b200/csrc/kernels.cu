@@ -422,33 +422,40 @@ reduce_flat_kernel(const c128* __restrict__ MU, const c128* __restrict__ MD, int
 // did = rd_i * NBd + cd_j, w = c_i * cbar_j.  For a fixed u row tuple ru and d column tuple cd
 //     sum_{i in sink[ru]} sum_{j in src[cd]} c_i cbar_j MU[ru, cu_j] MD[rd_i, cd]
 //   = ( sum_j cbar_j MU[ru, cu_j] ) * ( sum_i c_i MD[rd_i, cd] ),
-// i.e. |sink[ru]| + |src[cd]| loads for |sink[ru]| * |src[cd]| terms.
-__global__ void __launch_bounds__(RED_THREADS)
-reduce_outer_kernel(const c128* __restrict__ MU, const c128* __restrict__ MD, int S_b,
-                    int n_rows_u, int n_cols_u, int n_cols_d,
-                    const int32_t* __restrict__ sink_ptr, const int32_t* __restrict__ sink_rd, const c128* __restrict__ sink_c,
-                    const int32_t* __restrict__ src_ptr, const int32_t* __restrict__ src_cu, const c128* __restrict__ src_c,
-                    int rows_per_cta, c128* __restrict__ partial) {
+// i.e. |sink[ru]| + |src[cd]| loads for |sink[ru]| * |src[cd]| terms.  The (ru, cd) plane is walked
+// block by block: an item is (sink block k, source block k') of the block-diagonal factor lists
+// (contract.cu: build_reduce_schedule), whose minors are a few KB per warp and are re-read from L1;
+// every minor is fetched from DRAM / L2 once.  One warp = one bin of items, fixed order.
+__global__ void __launch_bounds__(RED_THREADS, 2)
+reduce_outer_kernel(const c128* __restrict__ MU, const c128* __restrict__ MD, int S_b, OuterTables ot,
+                    c128* __restrict__ partial) {
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int64_t s = int64_t(blockIdx.x) * GROUP + lane;
-    const int r0 = blockIdx.y * rows_per_cta;
-    const int r1 = min(n_rows_u, r0 + rows_per_cta);
+    const int bin = blockIdx.y * (RED_THREADS / 32) + warp;
     c128 acc = make_double2(0.0, 0.0);
-    for (int ru = r0 + warp; ru < r1; ru += RED_THREADS / 32) {
-        const int i0 = __ldg(sink_ptr + ru), i1 = __ldg(sink_ptr + ru + 1);
-        if (i0 == i1) continue;
-        const c128* MUrow = MU + int64_t(ru) * n_cols_u * S_b + s;
-        for (int cd = 0; cd < n_cols_d; ++cd) {
-            const int j0 = __ldg(src_ptr + cd), j1 = __ldg(src_ptr + cd + 1);
-            if (j0 == j1) continue;
-            c128 wsum = make_double2(0.0, 0.0);
-            for (int j = j0; j < j1; ++j)
-                wsum = cfma(__ldg(src_c + j), MUrow[int64_t(__ldg(src_cu + j)) * S_b], wsum);
-            c128 tsum = make_double2(0.0, 0.0);
-            const c128* MDcol = MD + int64_t(cd) * S_b + s;
-            for (int i = i0; i < i1; ++i)
-                tsum = cfma(__ldg(sink_c + i), MDcol[int64_t(__ldg(sink_rd + i)) * n_cols_d * S_b], tsum);
-            acc = cfma(wsum, tsum, acc);
+    const int it0 = __ldg(ot.bin_ptr + bin), it1 = __ldg(ot.bin_ptr + bin + 1);
+    for (int it = it0; it < it1; ++it) {
+        const int2 kk = __ldg(ot.items + it);
+        const int a0 = __ldg(ot.ru_ptr + kk.x), a1 = __ldg(ot.ru_ptr + kk.x + 1);
+        const int b0 = __ldg(ot.cd_ptr + kk.y), b1 = __ldg(ot.cd_ptr + kk.y + 1);
+        for (int a = a0; a < a1; ++a) {
+            const int ru = __ldg(ot.ru_list + a);
+            const int i0 = __ldg(ot.sink_ptr + ru), i1 = __ldg(ot.sink_ptr + ru + 1);
+            const c128* MUrow = MU + int64_t(ru) * ot.n_cols_u * S_b + s;
+            for (int b = b0; b < b1; ++b) {
+                const int cd = __ldg(ot.cd_list + b);
+                const int j0 = __ldg(ot.src_ptr + cd), j1 = __ldg(ot.src_ptr + cd + 1);
+                c128 q = make_double2(0.0, 0.0);
+#pragma unroll 4
+                for (int j = j0; j < j1; ++j)
+                    q = cfma(__ldg(ot.src_c + j), MUrow[int64_t(__ldg(ot.src_cu + j)) * S_b], q);
+                c128 p = make_double2(0.0, 0.0);
+                const c128* MDcol = MD + int64_t(cd) * S_b + s;
+#pragma unroll 4
+                for (int i = i0; i < i1; ++i)
+                    p = cfma(__ldg(ot.sink_c + i), MDcol[int64_t(__ldg(ot.sink_rdoff + i)) * S_b], p);
+                acc = cfma(q, p, acc);
+            }
         }
     }
     cta_combine_store(acc, partial + int64_t(blockIdx.y) * S_b + int64_t(blockIdx.x) * GROUP);
@@ -473,22 +480,12 @@ cudaError_t launch_reduce_flat(const double2* MU, const double2* MD, int n_group
     return cudaGetLastError();
 }
 
-cudaError_t launch_reduce_outer(const double2* MU, const double2* MD, int n_groups, int S_b,
-                                int n_rows_u, int n_cols_u, int n_cols_d,
-                                const int32_t* sink_ptr, const int32_t* sink_rd, const double2* sink_c,
-                                const int32_t* src_ptr, const int32_t* src_cu, const double2* src_c,
-                                double2* partial, int* n_chunks_out, int max_chunks, cudaStream_t stream) {
-    int chunks = (148 * 8 + n_groups - 1) / n_groups;
-    const int cap = (n_rows_u + 7) / 8;                       // at least one row tuple per warp
-    if (chunks > cap) chunks = cap;
-    if (chunks > max_chunks) chunks = max_chunks;
-    if (chunks < 1) chunks = 1;
-    const int rows_per_cta = (n_rows_u + chunks - 1) / chunks;
-    chunks = (n_rows_u + rows_per_cta - 1) / rows_per_cta;
+cudaError_t launch_reduce_outer(const double2* MU, const double2* MD, int n_groups, int S_b, const OuterTables& ot,
+                                double2* partial, int* n_chunks_out, cudaStream_t stream) {
+    const int chunks = ot.n_bins / (RED_THREADS / 32);         // n_bins is a multiple of 8 (contract.cu)
     dim3 grid(n_groups, chunks);
     ProfScope prof(PROF_REDUCE, stream);
-    reduce_outer_kernel<<<grid, RED_THREADS, 0, stream>>>(MU, MD, S_b, n_rows_u, n_cols_u, n_cols_d, sink_ptr, sink_rd,
-                                                          sink_c, src_ptr, src_cu, src_c, rows_per_cta, partial);
+    reduce_outer_kernel<<<grid, RED_THREADS, 0, stream>>>(MU, MD, S_b, ot, partial);
     ++g_launches;
     *n_chunks_out = chunks;
     return cudaGetLastError();

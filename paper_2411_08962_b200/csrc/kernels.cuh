@@ -32,11 +32,16 @@ cudaError_t launch_minors(int n, const double2* P, int64_t st0, int64_t n_st_tot
 cudaError_t launch_reduce_flat(const double2* MU, const double2* MD, int n_groups, int S_b,
                                const int32_t* uid, const int32_t* did, const double2* w, int64_t n_terms,
                                double2* partial, int* n_chunks_out, int max_chunks, cudaStream_t stream);
-cudaError_t launch_reduce_outer(const double2* MU, const double2* MD, int n_groups, int S_b,
-                                int n_rows_u, int n_cols_u, int n_cols_d,
-                                const int32_t* sink_ptr, const int32_t* sink_rd, const double2* sink_c,
-                                const int32_t* src_ptr, const int32_t* src_cu, const double2* src_c,
-                                double2* partial, int* n_chunks_out, int max_chunks, cudaStream_t stream);
+// factor lists + block schedule of the factorised reduction (device pointers; contract.cu builds them)
+struct OuterTables {
+    int n_cols_u, n_cols_d, n_bins;
+    const int32_t *sink_ptr, *sink_rdoff; const double2* sink_c;   // CSR over u row tuple: (rd * n_cols_d, c_i)
+    const int32_t *src_ptr, *src_cu; const double2* src_c;         // CSR over d column tuple: (cu, conj c_j)
+    const int32_t *ru_ptr, *ru_list, *cd_ptr, *cd_list;            // tuples grouped by sink / source block
+    const int32_t* bin_ptr; const int2* items;                     // per warp: list of (sink block, source block)
+};
+cudaError_t launch_reduce_outer(const double2* MU, const double2* MD, int n_groups, int S_b, const OuterTables& ot,
+                                double2* partial, int* n_chunks_out, cudaStream_t stream);
 cudaError_t launch_finalize_sigma(const double2* partial, int n_chunks, int S_b, int64_t n_valid,
                                   double2* sigma_batch, cudaStream_t stream);
 cudaError_t launch_project(const double2* sigma, int L, int T, const MomentumList& mom, double2* C_out,

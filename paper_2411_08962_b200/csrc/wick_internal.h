@@ -39,6 +39,15 @@ struct DeviceTables {
     const int32_t* src_cu = nullptr;            // [n_source] u column-tuple id
     const double* src_c = nullptr;              // [n_source][2]
     int max_sink_per_row = 0;
+    // block schedule of the factorised reduction (contract.cu: build_reduce_schedule)
+    const int32_t* sink_rdoff = nullptr;        // [n_sink]   rd * n_cols_d (element offset of the MD row)
+    const int32_t* ru_ptr = nullptr;            // [n_sink_comp + 1]  u row tuples grouped by sink component
+    const int32_t* ru_list = nullptr;
+    const int32_t* cd_ptr = nullptr;            // [n_src_comp + 1]   d column tuples grouped by source component
+    const int32_t* cd_list = nullptr;
+    const int32_t* red_bin_ptr = nullptr;       // [n_red_bins + 1]
+    const int32_t* red_items = nullptr;         // [n_items][2]  (sink component, source component)
+    int n_red_bins = 0;
     // flat list (uploaded only when the flat path runs)
     void* flat_blob = nullptr;
     const int32_t* t_uid = nullptr;
