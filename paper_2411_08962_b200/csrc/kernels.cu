@@ -220,6 +220,128 @@ __device__ __forceinline__ c128 det_lu_reg(const c128* tl, const Idx<N>& ix) {
     return det;
 }
 
+// Hybrid elimination (N = 5..8): N-4 steps of left-looking LU with partial pivoting, multipliers in
+// registers, then the closed form of the 4x4 Schur complement ("up to 4x4 analytic, LU above",
+// PAPER.md:203, applied to the trailing block as well).  det = (+-) piv_0 ... piv_{K-1} det4(S).
+// Rows are exchanged only during the K pivot steps; the 4 trailing rows keep whatever order the
+// pivoting left them in (det4 is evaluated in that order, the sign is already in `det`).
+// `tb` = shared-memory byte address of tile[0][lane]; rb[i] / cb[j] = byte offsets of row a_i / column b_j.
+template <int N>
+__device__ __forceinline__ c128 det_lu_hybrid(const unsigned char* tb, const uint32_t (&rb0)[N], const uint32_t (&cb)[N]) {
+    constexpr int K = N - 4;
+    uint32_t rb[N];
+#pragma unroll
+    for (int r = 0; r < N; ++r) rb[r] = rb0[r];
+    double Lr[N][K], Li[N][K];         // multipliers; only [r][i] with r > i is used
+    c128 det = make_double2(1.0, 0.0);
+#pragma unroll
+    for (int j = 0; j < K; ++j) {
+        double cr[N], ci[N];
+#pragma unroll
+        for (int r = 0; r < N; ++r) {
+            const c128 v = *reinterpret_cast<const c128*>(tb + (rb[r] + cb[j]));
+            cr[r] = v.x; ci[r] = v.y;
+        }
+#pragma unroll
+        for (int i = 0; i < j; ++i) {
+#pragma unroll
+            for (int r = i + 1; r < N; ++r) {
+                cr[r] = fma(-Lr[r][i], cr[i], fma(Li[r][i], ci[i], cr[r]));
+                ci[r] = fma(-Lr[r][i], ci[i], fma(-Li[r][i], cr[i], ci[r]));
+            }
+        }
+        // pivot = candidate with the largest |re| + |im| (LAPACK izamax rule), first maximum wins
+        int p = j;
+        double best = fabs(cr[j]) + fabs(ci[j]);
+#pragma unroll
+        for (int r = j + 1; r < N; ++r) {
+            const double m = fabs(cr[r]) + fabs(ci[r]);
+            if (m > best) { best = m; p = r; }
+        }
+        // exchange positions j and p: active column, row offsets, multipliers of columns < j
+        double pr = cr[j], pi = ci[j];
+        uint32_t po = rb[j];
+#pragma unroll
+        for (int r = j + 1; r < N; ++r) {
+            const bool hit = (p == r);
+            const double tr = cr[r], ti = ci[r];
+            const uint32_t to = rb[r];
+            cr[r] = hit ? cr[j] : tr; ci[r] = hit ? ci[j] : ti; rb[r] = hit ? rb[j] : to;
+            pr = hit ? tr : pr; pi = hit ? ti : pi; po = hit ? to : po;
+        }
+        rb[j] = po;
+#pragma unroll
+        for (int i = 0; i < j; ++i) {
+            double gr = Lr[j][i], gi = Li[j][i];
+#pragma unroll
+            for (int r = j + 1; r < N; ++r) {
+                const bool hit = (p == r);
+                const double ar = Lr[r][i], ai = Li[r][i];
+                Lr[r][i] = hit ? Lr[j][i] : ar; Li[r][i] = hit ? Li[j][i] : ai;
+                gr = hit ? ar : gr; gi = hit ? ai : gi;
+            }
+            Lr[j][i] = gr; Li[j][i] = gi;
+        }
+        const c128 piv = make_double2(pr, pi);
+        det = (j == 0) ? piv : cmul(det, piv);
+        if (p != j) { det.x = -det.x; det.y = -det.y; }
+        const c128 inv = crecip(piv);
+#pragma unroll
+        for (int r = j + 1; r < N; ++r) {
+            Lr[r][j] = cr[r] * inv.x - ci[r] * inv.y;
+            Li[r][j] = cr[r] * inv.y + ci[r] * inv.x;
+        }
+    }
+    // trailing columns: apply the K eliminations, keep the last 4 entries; Laplace along column pairs
+    c128 s[6];
+#pragma unroll
+    for (int h = 0; h < 2; ++h) {
+        double tr[2][4], ti[2][4];
+#pragma unroll
+        for (int q = 0; q < 2; ++q) {
+            const int j = K + 2 * h + q;
+            double cr[N], ci[N];
+#pragma unroll
+            for (int r = 0; r < N; ++r) {
+                const c128 v = *reinterpret_cast<const c128*>(tb + (rb[r] + cb[j]));
+                cr[r] = v.x; ci[r] = v.y;
+            }
+#pragma unroll
+            for (int i = 0; i < K; ++i) {
+#pragma unroll
+                for (int r = i + 1; r < N; ++r) {
+                    cr[r] = fma(-Lr[r][i], cr[i], fma(Li[r][i], ci[i], cr[r]));
+                    ci[r] = fma(-Lr[r][i], ci[i], fma(-Li[r][i], cr[i], ci[r]));
+                }
+            }
+#pragma unroll
+            for (int r = 0; r < 4; ++r) { tr[q][r] = cr[K + r]; ti[q][r] = ci[K + r]; }
+        }
+        c128 d2[6];
+        int k = 0;
+#pragma unroll
+        for (int a = 0; a < 4; ++a)
+#pragma unroll
+            for (int b = a + 1; b < 4; ++b)
+                d2[k++] = det2(make_double2(tr[0][a], ti[0][a]), make_double2(tr[1][a], ti[1][a]),
+                               make_double2(tr[0][b], ti[0][b]), make_double2(tr[1][b], ti[1][b]));
+        if (h == 0) {
+#pragma unroll
+            for (int q = 0; q < 6; ++q) s[q] = d2[q];
+        } else {
+            // pairs in order (01,02,03,12,13,23); complement of pair q is pair 5-q; signs + - + + - +
+            c128 d = cmul(s[0], d2[5]);
+            d = cfnma(s[1], d2[4], d);
+            d = cfma(s[2], d2[3], d);
+            d = cfma(s[3], d2[2], d);
+            d = cfnma(s[4], d2[1], d);
+            d = cfma(s[5], d2[0], d);
+            det = cmul(det, d);
+        }
+    }
+    return det;
+}
+
 // Same algorithm with the multipliers in shared memory (N = 9..12: N(N-1)/2 complex numbers do not
 // fit one thread's registers).  Ls points at this thread's slot; entry (r, i), r > i, lives at
 // Ls[(r(r-1)/2 + i) * NT] so that consecutive lanes hit consecutive 16-byte words (conflict free,
@@ -293,7 +415,7 @@ __device__ __forceinline__ c128 det_lu_smem(const c128* tl, c128* Ls, const Idx<
 template <int N> struct MinorCfg {
     static constexpr bool kSmemL = (N >= 9);
     static constexpr int kThreads = kSmemL ? 128 : 256;
-    static constexpr int kMinBlocks = (N <= 4) ? 2 : 1;
+    static constexpr int kMinBlocks = (N <= 6) ? 2 : 1;
     static constexpr size_t kSmem = size_t(TILE_BYTES) + (kSmemL ? size_t(N * (N - 1) / 2) * 16 * kThreads : 0);
 };
 
@@ -327,7 +449,12 @@ minors_kernel(const c128* __restrict__ P, int64_t st0, int64_t n_st_total, int S
         }
         c128 det;
         if constexpr (N <= 4) det = det_small<N>(tl, ix);
-        else if constexpr (!MinorCfg<N>::kSmemL) det = det_lu_reg<N>(tl, ix);
+        else if constexpr (!MinorCfg<N>::kSmemL) {
+            uint32_t rb[N], cb[N];
+#pragma unroll
+            for (int i = 0; i < N; ++i) { rb[i] = uint32_t(ix.re[i]) * (GROUP * 16); cb[i] = uint32_t(ix.ce[i]) * (GROUP * 16); }
+            det = det_lu_hybrid<N>(reinterpret_cast<const unsigned char*>(tl), rb, cb);
+        }
         else det = det_lu_smem<N, NT>(tl, tile + TILE_ELEMS + threadIdx.x, ix);
         if (valid) out[int64_t(m) * S_b + int64_t(g) * GROUP + lane] = det;
     }
