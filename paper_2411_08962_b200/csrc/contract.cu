@@ -46,17 +46,20 @@ struct BlobBuilder {
     }
 };
 
-// tuple table -> [n][16] bytes: scale * index, zero padded
-std::vector<uint8_t> elem_table(const std::vector<uint16_t>& masks, int scale) {
-    std::vector<uint8_t> out(masks.size() * 16, 0);
-    for (size_t i = 0; i < masks.size(); ++i) {
-        int k = 0;
-        for (int b = 0; b < 12; ++b)
-            if (masks[i] & (1u << b)) out[i * 16 + k++] = uint8_t(b * scale);
-    }
-    return out;
+// index set (12-bit mask) -> its indices as 4-bit fields, ascending
+uint64_t nibbles_of_mask(uint16_t mask) {
+    uint64_t w = 0;
+    int k = 0;
+    for (int b = 0; b < 12; ++b)
+        if (mask & (1u << b)) w |= uint64_t(b) << (4 * k++);
+    return w;
 }
 
+// minor descriptors for launch_minors (kernels.cu: struct Desc)
+void pack_minor_desc(int n, uint64_t rows, uint64_t cols, uint64_t* out) {
+    if (minor_desc_words(n) == 1) out[0] = (rows & 0xffffffffull) | (cols << 32);
+    else { out[0] = rows; out[1] = cols; }
+}
 
 // Connected components of the bipartite graph (qu -- qd) of a factor list.  Physical sink lists are
 // block diagonal (He-4: 199 blocks of at most 15 x 15 tuples), so the factorised reduction
@@ -168,16 +171,15 @@ int upload_tables(const wick_terms* t, cudaStream_t stream) {
     if (d.blob && d.device == dev) return WICK_OK;
     if (d.blob) { set_error("wick_terms handle was first used on another device"); return WICK_ERR_ARG; }
     BlobBuilder bb;
-    size_t o_row[2], o_col[2], o_rc[2];
+    size_t o_desc[2];
     for (int f = 0; f < 2; ++f) {
         const FlavourTables& ft = t->f[f];
-        if (ft.rows.size() > 65535 || ft.cols.size() > 65535) { set_error("more than 65535 distinct tuples"); return WICK_ERR_UNSUPPORTED; }
-        std::vector<uint8_t> re = elem_table(ft.rows, 12), ce = elem_table(ft.cols, 1);
-        std::vector<uint32_t> rc(ft.minor_row.size());
-        for (size_t m = 0; m < rc.size(); ++m) rc[m] = uint32_t(ft.minor_row[m]) | (uint32_t(ft.minor_col[m]) << 16);
-        o_row[f] = bb.add(re.data(), re.size());
-        o_col[f] = bb.add(ce.data(), ce.size());
-        o_rc[f] = bb.add(rc.data(), rc.size() * 4);
+        const int words = minor_desc_words(ft.n);
+        std::vector<uint64_t> desc(ft.minor_row.size() * size_t(words));
+        for (size_t m = 0; m < ft.minor_row.size(); ++m)
+            pack_minor_desc(ft.n, nibbles_of_mask(ft.rows[size_t(ft.minor_row[m])]), nibbles_of_mask(ft.cols[size_t(ft.minor_col[m])]),
+                            desc.data() + m * size_t(words));
+        o_desc[f] = bb.add(desc.data(), desc.size() * 8);
     }
     size_t o_sp = 0, o_srd = 0, o_sc = 0, o_qp = 0, o_qcu = 0, o_qc = 0;
     size_t o_srdoff = 0, o_rup = 0, o_rul = 0, o_cdp = 0, o_cdl = 0, o_binp = 0, o_items = 0;
@@ -224,11 +226,7 @@ int upload_tables(const wick_terms* t, cudaStream_t stream) {
     if (e == cudaSuccess) e = cudaStreamSynchronize(stream);   // bb.host dies at scope exit
     if (e != cudaSuccess) { cudaFree(blob); set_error(std::string("table upload: ") + cudaGetErrorString(e)); return WICK_ERR_CUDA; }
     unsigned char* b = static_cast<unsigned char*>(blob);
-    for (int f = 0; f < 2; ++f) {
-        d.row_elem[f] = b + o_row[f];
-        d.col_elem[f] = b + o_col[f];
-        d.minor_rc[f] = reinterpret_cast<const uint32_t*>(b + o_rc[f]);
-    }
+    for (int f = 0; f < 2; ++f) d.minor_desc[f] = b + o_desc[f];
     if (t->outer) {
         d.sink_ptr = reinterpret_cast<const int32_t*>(b + o_sp);
         d.sink_rd = reinterpret_cast<const int32_t*>(b + o_srd);
@@ -377,8 +375,8 @@ extern "C" int wick_contract(const void* U_dev, const void* D_dev, const wick_te
     for (int64_t st0 = 0; st0 < p.n_st; st0 += S_b) {
         const int64_t n_valid = std::min<int64_t>(S_b, p.n_st - st0);
         const int n_groups = int((n_valid + GROUP - 1) / GROUP);
-        WICK_CUDA(launch_minors(t->n_u, U, st0, p.n_st, n_groups, S_b, d.row_elem[0], d.col_elem[0], d.minor_rc[0], nmu, MU, PROF_MINORS_U, stream));
-        WICK_CUDA(launch_minors(t->n_d, D, st0, p.n_st, n_groups, S_b, d.row_elem[1], d.col_elem[1], d.minor_rc[1], nmd, MD, PROF_MINORS_D, stream));
+        WICK_CUDA(launch_minors(t->n_u, U, st0, p.n_st, n_groups, S_b, d.minor_desc[0], nmu, MU, PROF_MINORS_U, stream));
+        WICK_CUDA(launch_minors(t->n_d, D, st0, p.n_st, n_groups, S_b, d.minor_desc[1], nmd, MD, PROF_MINORS_D, stream));
         int n_chunks = 1;
         if (t->n_terms == 0) {
             WICK_CUDA(cudaMemsetAsync(sigma + st0, 0, size_t(n_valid) * 16, stream));
@@ -491,16 +489,14 @@ extern "C" int wick_minor_dets(const void* P_dev, int64_t n_sites, int n, const 
     if (rc != WICK_OK) return rc;
     const int64_t n_pad = (n_sites + GROUP - 1) / GROUP * GROUP;
     const bool direct = (n_pad == n_sites);                   // out[m][s] has row length n_sites: usable as S_b only if padded
-    // tables: one row tuple and one column tuple per minor, processed in slabs of 32768 minors
+    // descriptors built from the caller's tuples (any order, repeats allowed), in slabs of 32768 minors
     const int64_t slab = 32768;
-    std::vector<uint8_t> re(size_t(std::min(slab, n_minors)) * 16), ce(re.size());
-    std::vector<uint32_t> rcv(size_t(std::min(slab, n_minors)));
-    void *d_re = nullptr, *d_ce = nullptr, *d_rc = nullptr, *d_tmp = nullptr;
-    auto cleanup = [&]() { cudaFree(d_re); cudaFree(d_ce); cudaFree(d_rc); cudaFree(d_tmp); };
+    const int words = minor_desc_words(n);
+    std::vector<uint64_t> desc(size_t(std::min(slab, n_minors)) * size_t(words));
+    void *d_desc = nullptr, *d_tmp = nullptr;
+    auto cleanup = [&]() { cudaFree(d_desc); cudaFree(d_tmp); };
 #define WICK_CUDA_M(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) { set_error(std::string(#call) + ": " + cudaGetErrorString(e_)); cleanup(); return WICK_ERR_CUDA; } } while (0)
-    WICK_CUDA_M(cudaMalloc(&d_re, re.size()));
-    WICK_CUDA_M(cudaMalloc(&d_ce, ce.size()));
-    WICK_CUDA_M(cudaMalloc(&d_rc, rcv.size() * 4));
+    WICK_CUDA_M(cudaMalloc(&d_desc, desc.size() * 8));
     // site batches so that the padded staging buffer stays small when n_sites is not a multiple of 32
     const int64_t S_b = direct ? n_sites : std::min<int64_t>(n_pad, 4096);
     if (!direct) WICK_CUDA_M(cudaMalloc(&d_tmp, size_t(std::min(slab, n_minors)) * size_t(S_b) * 16));
@@ -508,33 +504,29 @@ extern "C" int wick_minor_dets(const void* P_dev, int64_t n_sites, int n, const 
         cleanup(); set_error("wick_minor_dets: n_sites too large for one call (max 2^22)"); return WICK_ERR_UNSUPPORTED; }
     for (int64_t m0 = 0; m0 < n_minors; m0 += slab) {
         const int64_t nm = std::min(slab, n_minors - m0);
-        std::fill(re.begin(), re.end(), 0); std::fill(ce.begin(), ce.end(), 0);
         for (int64_t m = 0; m < nm; ++m) {
+            uint64_t rw = 0, cw = 0;
             for (int i = 0; i < n; ++i) {
-                re[size_t(m) * 16 + i] = uint8_t(rows[(m0 + m) * n + i] * 12);
-                ce[size_t(m) * 16 + i] = cols[(m0 + m) * n + i];
+                rw |= uint64_t(rows[(m0 + m) * n + i]) << (4 * i);
+                cw |= uint64_t(cols[(m0 + m) * n + i]) << (4 * i);
             }
-            rcv[size_t(m)] = uint32_t(m) | (uint32_t(m) << 16);
+            pack_minor_desc(n, rw, cw, desc.data() + size_t(m) * size_t(words));
         }
-        WICK_CUDA_M(cudaMemcpyAsync(d_re, re.data(), size_t(nm) * 16, cudaMemcpyHostToDevice, stream));
-        WICK_CUDA_M(cudaMemcpyAsync(d_ce, ce.data(), size_t(nm) * 16, cudaMemcpyHostToDevice, stream));
-        WICK_CUDA_M(cudaMemcpyAsync(d_rc, rcv.data(), size_t(nm) * 4, cudaMemcpyHostToDevice, stream));
+        WICK_CUDA_M(cudaMemcpyAsync(d_desc, desc.data(), size_t(nm) * size_t(words) * 8, cudaMemcpyHostToDevice, stream));
         double2* out = static_cast<double2*>(out_dev) + m0 * n_sites;
         if (direct) {
             WICK_CUDA_M(launch_minors(n, static_cast<const double2*>(P_dev), 0, n_sites, int(n_sites / GROUP), int(S_b),
-                                      static_cast<const uint8_t*>(d_re), static_cast<const uint8_t*>(d_ce),
-                                      static_cast<const uint32_t*>(d_rc), nm, out, PROF_MINORS_U, stream));
+                                      d_desc, nm, out, PROF_MINORS_U, stream));
         } else {
             for (int64_t s0 = 0; s0 < n_sites; s0 += S_b) {
                 const int64_t nv = std::min(S_b, n_sites - s0);
                 WICK_CUDA_M(launch_minors(n, static_cast<const double2*>(P_dev), s0, n_sites, int((nv + GROUP - 1) / GROUP), int(S_b),
-                                          static_cast<const uint8_t*>(d_re), static_cast<const uint8_t*>(d_ce),
-                                          static_cast<const uint32_t*>(d_rc), nm, static_cast<double2*>(d_tmp), PROF_MINORS_U, stream));
+                                          d_desc, nm, static_cast<double2*>(d_tmp), PROF_MINORS_U, stream));
                 WICK_CUDA_M(cudaMemcpy2DAsync(out + s0, size_t(n_sites) * 16, d_tmp, size_t(S_b) * 16, size_t(nv) * 16, size_t(nm),
                                               cudaMemcpyDeviceToDevice, stream));
             }
         }
-        WICK_CUDA_M(cudaStreamSynchronize(stream));           // host tables are reused by the next slab
+        WICK_CUDA_M(cudaStreamSynchronize(stream));           // the host descriptor slab is reused by the next one
     }
     cleanup();
 #undef WICK_CUDA_M

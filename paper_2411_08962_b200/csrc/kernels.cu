@@ -138,13 +138,26 @@ __device__ __forceinline__ c128 det_small(const c128* tl, const Idx<N>& ix) {
     return d;
 }
 
-// reciprocal of a pivot: 1/(x + i y) = (x - i y) / (x^2 + y^2); an exactly zero pivot (singular
-// column: every candidate was 0) gives multipliers 0 so that det stays exactly 0 instead of NaN
+// reciprocal of a pivot: 1/(x + i y) = (x - i y) / (x^2 + y^2).  The real reciprocal is MUFU.RCP64H
+// (rcp.approx.ftz.f64, ~20 bits) plus two Newton steps (relative error ~1e-16 for normal d); an exactly
+// zero pivot (singular column: every candidate was 0) gives multipliers 0, so det stays exactly 0, not NaN.
+// |pivot|^2 must be a normal double (|pivot| in ~[1e-154, 1e154]); outside, det over/underflows anyway.
 __device__ __forceinline__ c128 crecip(c128 p) {
     const double d = fma(p.x, p.x, p.y * p.y);
-    const double r = d > 0.0 ? 1.0 / d : 0.0;
+    double r;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(d));
+    double e = fma(-d, r, 1.0);
+    r = fma(r, e, r);
+    e = fma(-d, r, 1.0);
+    r = fma(r, e, r);
+    r = d > 0.0 ? r : 0.0;
     return make_double2(p.x * r, -p.y * r);
 }
+
+// pivot key: high word of |re| + |im| (>= 0, so the integer order is the floating-point order up to
+// the 2^-20 of the dropped low word): near-maximal pivots are as good as the maximal one for stability,
+// and integer compares keep the argmax chain off the FP64 pipe
+__device__ __forceinline__ int pivot_key(double re, double im) { return __double2hiint(fabs(re) + fabs(im)); }
 
 // Left-looking LU with partial pivoting, multipliers L in registers (N = 5..8).
 // Pivot = candidate with the largest |re| + |im| (the LAPACK izamax / cabs1 rule), first maximum wins.
@@ -250,12 +263,12 @@ __device__ __forceinline__ c128 det_lu_hybrid(const unsigned char* tb, const uin
                 ci[r] = fma(-Lr[r][i], ci[i], fma(-Li[r][i], cr[i], ci[r]));
             }
         }
-        // pivot = candidate with the largest |re| + |im| (LAPACK izamax rule), first maximum wins
+        // pivot = candidate with the largest |re| + |im| (LAPACK izamax rule) to 2^-20, first maximum wins
         int p = j;
-        double best = fabs(cr[j]) + fabs(ci[j]);
+        int best = pivot_key(cr[j], ci[j]);
 #pragma unroll
         for (int r = j + 1; r < N; ++r) {
-            const double m = fabs(cr[r]) + fabs(ci[r]);
+            const int m = pivot_key(cr[r], ci[r]);
             if (m > best) { best = m; p = r; }
         }
         // exchange positions j and p: active column, row offsets, multipliers of columns < j
@@ -419,51 +432,75 @@ template <int N> struct MinorCfg {
     static constexpr size_t kSmem = size_t(TILE_BYTES) + (kSmemL ? size_t(N * (N - 1) / 2) * 16 * kThreads : 0);
 };
 
+// Minor descriptor (built on the host, contract.cu: pack_minor_desc): the row and column indices as
+// 4-bit fields, ascending.  n <= 8: one 64-bit word (rows in the low half, columns in the high half);
+// n >= 9: two 64-bit words (rows, columns).  One load per minor, no dependent second load.
+template <int N> struct Desc {
+    static constexpr int kWords = (N <= 8) ? 1 : 2;
+    unsigned long long w[kWords];
+    __device__ __forceinline__ static Desc load(const unsigned long long* tab, int m) {
+        Desc d;
+        if constexpr (kWords == 1) d.w[0] = __ldg(tab + m);
+        else { const ulonglong2 v = __ldg(reinterpret_cast<const ulonglong2*>(tab) + m); d.w[0] = v.x; d.w[1] = v.y; }
+        return d;
+    }
+    __device__ __forceinline__ uint32_t row(int i) const {
+        if constexpr (kWords == 1) return (uint32_t(w[0]) >> (4 * i)) & 15u;
+        else return uint32_t(w[0] >> (4 * i)) & 15u;
+    }
+    __device__ __forceinline__ uint32_t col(int i) const {
+        if constexpr (kWords == 1) return (uint32_t(w[0] >> 32) >> (4 * i)) & 15u;
+        else return uint32_t(w[1] >> (4 * i)) & 15u;
+    }
+};
+
 template <int N>
 __global__ void __launch_bounds__(MinorCfg<N>::kThreads, MinorCfg<N>::kMinBlocks)
 minors_kernel(const c128* __restrict__ P, int64_t st0, int64_t n_st_total, int S_b,
-              const uint8_t* __restrict__ row_elem, const uint8_t* __restrict__ col_elem,
-              const uint32_t* __restrict__ minor_rc, int n_minors, int chunk, c128* __restrict__ out) {
+              const unsigned long long* __restrict__ desc, int n_minors, int chunk, c128* __restrict__ out) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     c128* tile = reinterpret_cast<c128*>(smem_raw);
     constexpr int NT = MinorCfg<N>::kThreads;
     const int g = blockIdx.x;
     const int64_t st_first = st0 + int64_t(g) * GROUP;
-    stage_tile(tile, P, st_first, n_st_total, NT);
-    __syncthreads();
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const c128* tl = tile + lane;
-    const bool valid = st_first + lane < n_st_total;
     const int m_begin = blockIdx.y * chunk;
     const int m_end = min(n_minors, m_begin + chunk);
-    for (int m = m_begin + warp; m < m_end; m += NT / 32) {
-        const uint32_t rc = __ldg(minor_rc + m);
-        const uint4 rw = __ldg(reinterpret_cast<const uint4*>(row_elem) + (rc & 0xffffu));
-        const uint4 cw = __ldg(reinterpret_cast<const uint4*>(col_elem) + (rc >> 16));
-        const uint32_t rws[4] = {rw.x, rw.y, rw.z, rw.w}, cws[4] = {cw.x, cw.y, cw.z, cw.w};
-        Idx<N> ix;
-#pragma unroll
-        for (int i = 0; i < N; ++i) {
-            ix.re[i] = (rws[i >> 2] >> (8 * (i & 3))) & 0xff;
-            ix.ce[i] = (cws[i >> 2] >> (8 * (i & 3))) & 0xff;
-        }
+    int m = m_begin + warp;
+    Desc<N> dn;                                                // descriptor of the next minor, fetched one iteration ahead
+    if (m < m_end) dn = Desc<N>::load(desc, m);
+    stage_tile(tile, P, st_first, n_st_total, NT);
+    __syncthreads();
+    const c128* tl = tile + lane;
+    const bool valid = st_first + lane < n_st_total;
+    c128* outp = out + int64_t(g) * GROUP + lane;
+    for (; m < m_end; m += NT / 32) {
+        const Desc<N> dc = dn;
+        if (m + NT / 32 < m_end) dn = Desc<N>::load(desc, m + NT / 32);
         c128 det;
-        if constexpr (N <= 4) det = det_small<N>(tl, ix);
-        else if constexpr (!MinorCfg<N>::kSmemL) {
+        if constexpr (N <= 4) {
+            Idx<N> ix;
+#pragma unroll
+            for (int i = 0; i < N; ++i) { ix.re[i] = int(dc.row(i)) * 12; ix.ce[i] = int(dc.col(i)); }
+            det = det_small<N>(tl, ix);
+        } else if constexpr (!MinorCfg<N>::kSmemL) {
             uint32_t rb[N], cb[N];
 #pragma unroll
-            for (int i = 0; i < N; ++i) { rb[i] = uint32_t(ix.re[i]) * (GROUP * 16); cb[i] = uint32_t(ix.ce[i]) * (GROUP * 16); }
+            for (int i = 0; i < N; ++i) { rb[i] = dc.row(i) * (12 * GROUP * 16); cb[i] = dc.col(i) * (GROUP * 16); }
             det = det_lu_hybrid<N>(reinterpret_cast<const unsigned char*>(tl), rb, cb);
+        } else {
+            Idx<N> ix;
+#pragma unroll
+            for (int i = 0; i < N; ++i) { ix.re[i] = int(dc.row(i)) * 12; ix.ce[i] = int(dc.col(i)); }
+            det = det_lu_smem<N, NT>(tl, tile + TILE_ELEMS + threadIdx.x, ix);
         }
-        else det = det_lu_smem<N, NT>(tl, tile + TILE_ELEMS + threadIdx.x, ix);
-        if (valid) out[int64_t(m) * S_b + int64_t(g) * GROUP + lane] = det;
+        if (valid) outp[int64_t(m) * S_b] = det;
     }
 }
 
 template <int N>
 static cudaError_t launch_minors_n(const c128* P, int64_t st0, int64_t n_st_total, int n_groups, int S_b,
-                                   const uint8_t* row_elem, const uint8_t* col_elem, const uint32_t* minor_rc,
-                                   int64_t n_minors, c128* out, int prof_cls, cudaStream_t stream) {
+                                   const void* desc, int64_t n_minors, c128* out, int prof_cls, cudaStream_t stream) {
     constexpr int NT = MinorCfg<N>::kThreads;
     constexpr int warps = NT / 32;
     // enough CTAs for ~4 waves on 148 SMs, but at least 2 minors per warp per CTA
@@ -477,17 +514,18 @@ static cudaError_t launch_minors_n(const c128* P, int64_t st0, int64_t n_st_tota
     chunks = int((n_minors + chunk - 1) / chunk);
     dim3 grid(n_groups, chunks);
     ProfScope prof(prof_cls, stream);
-    minors_kernel<N><<<grid, NT, MinorCfg<N>::kSmem, stream>>>(P, st0, n_st_total, S_b, row_elem, col_elem,
-                                                             minor_rc, int(n_minors), chunk, out);
+    minors_kernel<N><<<grid, NT, MinorCfg<N>::kSmem, stream>>>(P, st0, n_st_total, S_b,
+                                                             static_cast<const unsigned long long*>(desc), int(n_minors), chunk, out);
     ++g_launches;
     return cudaGetLastError();
 }
 
+int minor_desc_words(int n) { return n <= 8 ? 1 : 2; }
+
 cudaError_t launch_minors(int n, const double2* P, int64_t st0, int64_t n_st_total, int n_groups, int S_b,
-                          const uint8_t* row_elem, const uint8_t* col_elem, const uint32_t* minor_rc,
-                          int64_t n_minors, double2* out, int prof_cls, cudaStream_t stream) {
+                          const void* desc, int64_t n_minors, double2* out, int prof_cls, cudaStream_t stream) {
     if (n_minors == 0 || n_groups == 0) return cudaSuccess;
-#define WICK_CASE(N) case N: return launch_minors_n<N>(P, st0, n_st_total, n_groups, S_b, row_elem, col_elem, minor_rc, n_minors, out, prof_cls, stream);
+#define WICK_CASE(N) case N: return launch_minors_n<N>(P, st0, n_st_total, n_groups, S_b, desc, n_minors, out, prof_cls, stream);
     switch (n) {
         WICK_CASE(0) WICK_CASE(1) WICK_CASE(2) WICK_CASE(3) WICK_CASE(4) WICK_CASE(5) WICK_CASE(6)
         WICK_CASE(7) WICK_CASE(8) WICK_CASE(9) WICK_CASE(10) WICK_CASE(11) WICK_CASE(12)

@@ -28,9 +28,7 @@ struct FactorTerm { int32_t qu, qd; cplx c; };
 struct DeviceTables {
     int device = -1;
     void* blob = nullptr;                       // one allocation holding the minor tables + factor lists
-    const uint8_t* row_elem[2] = {nullptr, nullptr};   // [n_rows][16]: a_i * 12 (element offset of row a_i), zero padded
-    const uint8_t* col_elem[2] = {nullptr, nullptr};   // [n_cols][16]: b_j
-    const uint32_t* minor_rc[2] = {nullptr, nullptr};  // [n_minors]: row id | col id << 16
+    const void* minor_desc[2] = {nullptr, nullptr};     // [n_minors] packed (row indices, column indices), kernels.cu: struct Desc
     // factorised reduction: sink CSR over u row-tuple id, source CSR over d column-tuple id
     const int32_t* sink_ptr = nullptr;          // [n_rows_u + 1]
     const int32_t* sink_rd = nullptr;           // [n_sink]   d row-tuple id
