@@ -159,94 +159,37 @@ __device__ __forceinline__ c128 crecip(c128 p) {
 // and integer compares keep the argmax chain off the FP64 pipe
 __device__ __forceinline__ int pivot_key(double re, double im) { return __double2hiint(fabs(re) + fabs(im)); }
 
-// Left-looking LU with partial pivoting, multipliers L in registers (N = 5..8).
-// Pivot = candidate with the largest |re| + |im| (the LAPACK izamax / cabs1 rule), first maximum wins.
-template <int N>
-__device__ __forceinline__ c128 det_lu_reg(const c128* tl, const Idx<N>& ix) {
-    int roff[N];                       // per-lane row order: element offset of the row at position r
-#pragma unroll
-    for (int r = 0; r < N; ++r) roff[r] = ix.re[r];
-    double Lr[N][N], Li[N][N];         // multipliers; only [r][i] with r > i is used
-    c128 det = make_double2(1.0, 0.0);
-#pragma unroll
-    for (int j = 0; j < N; ++j) {
-        double cr[N], ci[N];
-#pragma unroll
-        for (int r = 0; r < N; ++r) {
-            const c128 v = ld(tl, roff[r], ix.ce[j]);
-            cr[r] = v.x; ci[r] = v.y;
-        }
-        // apply the eliminations of columns i < j to the new column
-#pragma unroll
-        for (int i = 0; i < j; ++i) {
-#pragma unroll
-            for (int r = i + 1; r < N; ++r) {
-                cr[r] = fma(-Lr[r][i], cr[i], fma(Li[r][i], ci[i], cr[r]));
-                ci[r] = fma(-Lr[r][i], ci[i], fma(-Li[r][i], cr[i], ci[r]));
-            }
-        }
-        if (j < N - 1) {
-            int p = j;
-            double best = fabs(cr[j]) + fabs(ci[j]);
-#pragma unroll
-            for (int r = j + 1; r < N; ++r) {
-                const double m = fabs(cr[r]) + fabs(ci[r]);
-                if (m > best) { best = m; p = r; }
-            }
-            // exchange positions j and p: active column, row order, multipliers of columns < j
-            double pr = cr[j], pi = ci[j];
-            int po = roff[j];
-#pragma unroll
-            for (int r = j + 1; r < N; ++r) {
-                const bool hit = (p == r);
-                const double tr = cr[r], ti = ci[r];
-                const int to = roff[r];
-                cr[r] = hit ? cr[j] : tr; ci[r] = hit ? ci[j] : ti; roff[r] = hit ? roff[j] : to;
-                pr = hit ? tr : pr; pi = hit ? ti : pi; po = hit ? to : po;
-            }
-            cr[j] = pr; ci[j] = pi; roff[j] = po;
-#pragma unroll
-            for (int i = 0; i < j; ++i) {
-                double gr = Lr[j][i], gi = Li[j][i];
-#pragma unroll
-                for (int r = j + 1; r < N; ++r) {
-                    const bool hit = (p == r);
-                    const double tr = Lr[r][i], ti = Li[r][i];
-                    Lr[r][i] = hit ? Lr[j][i] : tr; Li[r][i] = hit ? Li[j][i] : ti;
-                    gr = hit ? tr : gr; gi = hit ? ti : gi;
-                }
-                Lr[j][i] = gr; Li[j][i] = gi;
-            }
-            const c128 piv = make_double2(pr, pi);
-            det = cmul(det, piv);
-            if (p != j) { det.x = -det.x; det.y = -det.y; }
-            const c128 inv = crecip(piv);
-#pragma unroll
-            for (int r = j + 1; r < N; ++r) {
-                Lr[r][j] = cr[r] * inv.x - ci[r] * inv.y;
-                Li[r][j] = cr[r] * inv.y + ci[r] * inv.x;
-            }
-        } else {
-            det = cmul(det, make_double2(cr[N - 1], ci[N - 1]));
-        }
-    }
-    return det;
-}
+// number of multipliers in the first i columns of L (column c holds rows c+1 .. N-1)
+template <int N> __host__ __device__ constexpr int lcol_base(int i) { return i * (N - 1) - i * (i - 1) / 2; }
 
-// Hybrid elimination (N = 5..8): N-4 steps of left-looking LU with partial pivoting, multipliers in
-// registers, then the closed form of the 4x4 Schur complement ("up to 4x4 analytic, LU above",
-// PAPER.md:203, applied to the trailing block as well).  det = (+-) piv_0 ... piv_{K-1} det4(S).
+// Hybrid elimination (N >= 5): K = N-4 steps of LEFT-LOOKING LU with partial pivoting, then the closed
+// form of the 4x4 Schur complement ("up to 4x4 analytic, LU above", applied to the
+// trailing block as well).  det = (+-) piv_0 ... piv_{K-1} det4(S).  Left-looking: column j of the minor
+// is gathered from shared memory only after the pivots of columns < j are known, in the lane's current
+// row order, so the only data ever exchanged is the active column and the multipliers.
+// The multipliers of columns < R live in shared memory (Ls: this thread's slot, entry e at Ls[e * NT],
+// conflict free also for the per-lane dynamic row of the exchange), those of columns R..K-1 in registers.
 // Rows are exchanged only during the K pivot steps; the 4 trailing rows keep whatever order the
 // pivoting left them in (det4 is evaluated in that order, the sign is already in `det`).
-// `tb` = shared-memory byte address of tile[0][lane]; rb[i] / cb[j] = byte offsets of row a_i / column b_j.
-template <int N>
-__device__ __forceinline__ c128 det_lu_hybrid(const unsigned char* tb, const uint32_t (&rb0)[N], const uint32_t (&cb)[N]) {
+// `tb` = byte address of tile[0][lane]; rb0[i] / cb[j] = byte offsets of row a_i / column b_j.
+template <int N, int R, int NT>
+__device__ __forceinline__ c128 det_lu_hybrid(const unsigned char* tb, c128* Ls, const uint32_t (&rb0)[N], const uint32_t (&cb)[N]) {
     constexpr int K = N - 4;
+    constexpr int KR = (K - R > 0) ? K - R : 1;
     uint32_t rb[N];
 #pragma unroll
     for (int r = 0; r < N; ++r) rb[r] = rb0[r];
-    double Lr[N][K], Li[N][K];         // multipliers; only [r][i] with r > i is used
+    double Lr[N][KR], Li[N][KR];       // register multipliers: column i >= R at [r][i - R], r > i
     c128 det = make_double2(1.0, 0.0);
+    // c[r] -= L[r][i] c[i] for r > i: the elimination of column i applied to the active column
+#define WICK_APPLY_COLUMN(i)                                                                   \
+    _Pragma("unroll") for (int r = (i) + 1; r < N; ++r) {                                      \
+        double lr, li;                                                                         \
+        if ((i) < R) { const c128 l = Ls[(lcol_base<N>(i) + r - (i) - 1) * NT]; lr = l.x; li = l.y; } \
+        else { lr = Lr[r][(i) >= R ? (i) - R : 0]; li = Li[r][(i) >= R ? (i) - R : 0]; }        \
+        cr[r] = fma(-lr, cr[i], fma(li, ci[i], cr[r]));                                        \
+        ci[r] = fma(-lr, ci[i], fma(-li, cr[i], ci[r]));                                       \
+    }
 #pragma unroll
     for (int j = 0; j < K; ++j) {
         double cr[N], ci[N];
@@ -256,13 +199,7 @@ __device__ __forceinline__ c128 det_lu_hybrid(const unsigned char* tb, const uin
             cr[r] = v.x; ci[r] = v.y;
         }
 #pragma unroll
-        for (int i = 0; i < j; ++i) {
-#pragma unroll
-            for (int r = i + 1; r < N; ++r) {
-                cr[r] = fma(-Lr[r][i], cr[i], fma(Li[r][i], ci[i], cr[r]));
-                ci[r] = fma(-Lr[r][i], ci[i], fma(-Li[r][i], cr[i], ci[r]));
-            }
-        }
+        for (int i = 0; i < j; ++i) { WICK_APPLY_COLUMN(i) }
         // pivot = candidate with the largest |re| + |im| (LAPACK izamax rule) to 2^-20, first maximum wins
         int p = j;
         int best = pivot_key(cr[j], ci[j]);
@@ -283,17 +220,26 @@ __device__ __forceinline__ c128 det_lu_hybrid(const unsigned char* tb, const uin
             pr = hit ? tr : pr; pi = hit ? ti : pi; po = hit ? to : po;
         }
         rb[j] = po;
+        if (R > 0 && j > 0 && p != j) {                         // shared-memory columns: swap rows j and p
 #pragma unroll
-        for (int i = 0; i < j; ++i) {
-            double gr = Lr[j][i], gi = Li[j][i];
+            for (int i = 0; i < (j < R ? j : R); ++i) {
+                c128* ej = Ls + (lcol_base<N>(i) + j - i - 1) * NT;
+                c128* ep = Ls + (lcol_base<N>(i) + p - i - 1) * NT;
+                const c128 a = *ej, b = *ep;
+                *ej = b; *ep = a;
+            }
+        }
+#pragma unroll
+        for (int i = R; i < j; ++i) {                           // register columns: exchange by selects
+            double gr = Lr[j][i - R], gi = Li[j][i - R];
 #pragma unroll
             for (int r = j + 1; r < N; ++r) {
                 const bool hit = (p == r);
-                const double ar = Lr[r][i], ai = Li[r][i];
-                Lr[r][i] = hit ? Lr[j][i] : ar; Li[r][i] = hit ? Li[j][i] : ai;
+                const double ar = Lr[r][i - R], ai = Li[r][i - R];
+                Lr[r][i - R] = hit ? Lr[j][i - R] : ar; Li[r][i - R] = hit ? Li[j][i - R] : ai;
                 gr = hit ? ar : gr; gi = hit ? ai : gi;
             }
-            Lr[j][i] = gr; Li[j][i] = gi;
+            Lr[j][i - R] = gr; Li[j][i - R] = gi;
         }
         const c128 piv = make_double2(pr, pi);
         det = (j == 0) ? piv : cmul(det, piv);
@@ -301,8 +247,9 @@ __device__ __forceinline__ c128 det_lu_hybrid(const unsigned char* tb, const uin
         const c128 inv = crecip(piv);
 #pragma unroll
         for (int r = j + 1; r < N; ++r) {
-            Lr[r][j] = cr[r] * inv.x - ci[r] * inv.y;
-            Li[r][j] = cr[r] * inv.y + ci[r] * inv.x;
+            const double lr = cr[r] * inv.x - ci[r] * inv.y, li = cr[r] * inv.y + ci[r] * inv.x;
+            if (j < R) Ls[(lcol_base<N>(j) + r - j - 1) * NT] = make_double2(lr, li);
+            else { Lr[r][j >= R ? j - R : 0] = lr; Li[r][j >= R ? j - R : 0] = li; }
         }
     }
     // trailing columns: apply the K eliminations, keep the last 4 entries; Laplace along column pairs
@@ -320,13 +267,7 @@ __device__ __forceinline__ c128 det_lu_hybrid(const unsigned char* tb, const uin
                 cr[r] = v.x; ci[r] = v.y;
             }
 #pragma unroll
-            for (int i = 0; i < K; ++i) {
-#pragma unroll
-                for (int r = i + 1; r < N; ++r) {
-                    cr[r] = fma(-Lr[r][i], cr[i], fma(Li[r][i], ci[i], cr[r]));
-                    ci[r] = fma(-Lr[r][i], ci[i], fma(-Li[r][i], cr[i], ci[r]));
-                }
-            }
+            for (int i = 0; i < K; ++i) { WICK_APPLY_COLUMN(i) }
 #pragma unroll
             for (int r = 0; r < 4; ++r) { tr[q][r] = cr[K + r]; ti[q][r] = ci[K + r]; }
         }
@@ -355,81 +296,14 @@ __device__ __forceinline__ c128 det_lu_hybrid(const unsigned char* tb, const uin
     return det;
 }
 
-// Same algorithm with the multipliers in shared memory (N = 9..12: N(N-1)/2 complex numbers do not
-// fit one thread's registers).  Ls points at this thread's slot; entry (r, i), r > i, lives at
-// Ls[(r(r-1)/2 + i) * NT] so that consecutive lanes hit consecutive 16-byte words (conflict free,
-// also for the per-lane dynamic row p of the exchange).
-template <int N, int NT>
-__device__ __forceinline__ c128 det_lu_smem(const c128* tl, c128* Ls, const Idx<N>& ix) {
-    int roff[N];
-#pragma unroll
-    for (int r = 0; r < N; ++r) roff[r] = ix.re[r];
-    c128 det = make_double2(1.0, 0.0);
-#pragma unroll
-    for (int j = 0; j < N; ++j) {
-        double cr[N], ci[N];
-#pragma unroll
-        for (int r = 0; r < N; ++r) {
-            const c128 v = ld(tl, roff[r], ix.ce[j]);
-            cr[r] = v.x; ci[r] = v.y;
-        }
-#pragma unroll
-        for (int i = 0; i < j; ++i) {
-#pragma unroll
-            for (int r = i + 1; r < N; ++r) {
-                const c128 l = Ls[(r * (r - 1) / 2 + i) * NT];
-                cr[r] = fma(-l.x, cr[i], fma(l.y, ci[i], cr[r]));
-                ci[r] = fma(-l.x, ci[i], fma(-l.y, cr[i], ci[r]));
-            }
-        }
-        if (j < N - 1) {
-            int p = j;
-            double best = fabs(cr[j]) + fabs(ci[j]);
-#pragma unroll
-            for (int r = j + 1; r < N; ++r) {
-                const double m = fabs(cr[r]) + fabs(ci[r]);
-                if (m > best) { best = m; p = r; }
-            }
-            double pr = cr[j], pi = ci[j];
-            int po = roff[j];
-#pragma unroll
-            for (int r = j + 1; r < N; ++r) {
-                const bool hit = (p == r);
-                const double tr = cr[r], ti = ci[r];
-                const int to = roff[r];
-                cr[r] = hit ? cr[j] : tr; ci[r] = hit ? ci[j] : ti; roff[r] = hit ? roff[j] : to;
-                pr = hit ? tr : pr; pi = hit ? ti : pi; po = hit ? to : po;
-            }
-            cr[j] = pr; ci[j] = pi; roff[j] = po;
-            if (p != j) {                                   // exchange multiplier rows j and p (columns < j)
-                const int pb = p * (p - 1) / 2;
-#pragma unroll
-                for (int i = 0; i < j; ++i) {
-                    const c128 a = Ls[(j * (j - 1) / 2 + i) * NT];
-                    const c128 b = Ls[(pb + i) * NT];
-                    Ls[(j * (j - 1) / 2 + i) * NT] = b;
-                    Ls[(pb + i) * NT] = a;
-                }
-            }
-            const c128 piv = make_double2(pr, pi);
-            det = cmul(det, piv);
-            if (p != j) { det.x = -det.x; det.y = -det.y; }
-            const c128 inv = crecip(piv);
-#pragma unroll
-            for (int r = j + 1; r < N; ++r)
-                Ls[(r * (r - 1) / 2 + j) * NT] = make_double2(cr[r] * inv.x - ci[r] * inv.y, cr[r] * inv.y + ci[r] * inv.x);
-        } else {
-            det = cmul(det, make_double2(cr[N - 1], ci[N - 1]));
-        }
-    }
-    return det;
-}
+#undef WICK_APPLY_COLUMN
 
 template <int N> struct MinorCfg {
-    static constexpr bool kSmemL = (N >= 9);
-    static constexpr int kThreads = kSmemL ? 128 : 256;
+    // columns of L kept in shared memory (the rest of the N-4 columns are registers)
+    static constexpr int kSmemCols = (N <= 10) ? 0 : (N == 11 ? 3 : 5);
+    static constexpr int kThreads = (N <= 11) ? 256 : 128;
     static constexpr int kMinBlocks = (N <= 6) ? 2 : 1;
-    static constexpr size_t kSmem = size_t(TILE_BYTES) + (kSmemL ? size_t(N * (N - 1) / 2) * 16 * kThreads : 0);
+    static constexpr size_t kSmem = size_t(TILE_BYTES) + size_t(lcol_base<(N > 1 ? N : 2)>(kSmemCols)) * 16 * kThreads;
 };
 
 // Minor descriptor (built on the host, contract.cu: pack_minor_desc): the row and column indices as
@@ -483,16 +357,12 @@ minors_kernel(const c128* __restrict__ P, int64_t st0, int64_t n_st_total, int S
 #pragma unroll
             for (int i = 0; i < N; ++i) { ix.re[i] = int(dc.row(i)) * 12; ix.ce[i] = int(dc.col(i)); }
             det = det_small<N>(tl, ix);
-        } else if constexpr (!MinorCfg<N>::kSmemL) {
+        } else {
             uint32_t rb[N], cb[N];
 #pragma unroll
             for (int i = 0; i < N; ++i) { rb[i] = dc.row(i) * (12 * GROUP * 16); cb[i] = dc.col(i) * (GROUP * 16); }
-            det = det_lu_hybrid<N>(reinterpret_cast<const unsigned char*>(tl), rb, cb);
-        } else {
-            Idx<N> ix;
-#pragma unroll
-            for (int i = 0; i < N; ++i) { ix.re[i] = int(dc.row(i)) * 12; ix.ce[i] = int(dc.col(i)); }
-            det = det_lu_smem<N, NT>(tl, tile + TILE_ELEMS + threadIdx.x, ix);
+            det = det_lu_hybrid<N, MinorCfg<N>::kSmemCols, NT>(reinterpret_cast<const unsigned char*>(tl),
+                                                               tile + TILE_ELEMS + threadIdx.x, rb, cb);
         }
         if (valid) outp[int64_t(m) * S_b] = det;
     }
