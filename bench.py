@@ -279,6 +279,11 @@ def main():
         "reduce": {"ms_per_step": ms_reduce, "tflops": st_per_step * info.n_terms * FLOPS_PER_TERM / (ms_reduce * 1e-3) / 1e12
                    if ms_reduce > 0 else None, "share_of_step": ms_reduce / ms_step},
         "project_ms_per_step": ms_project,
+        "per_flavour": {
+            q: {"n": n, "ms_per_step": prof[k][0] / args.steps,
+                "frac": (st_per_step * nm * flops_lu(n) / (prof[k][0] / args.steps * 1e-3) / 1e12 / FP64_PEAK_DERIVED_TFLOPS)
+                if prof[k][0] > 0 else None}
+            for q, k, n, nm in (("u", "minors_u", info.n_u, info.n_minors_u), ("d", "minors_d", info.n_d, info.n_minors_d))},
         "whole_step_tflops": (flop_minors + st_per_step * info.n_terms * FLOPS_PER_TERM) / (ms_step * 1e-3) / 1e12,
     }
 

@@ -300,7 +300,7 @@ __device__ __forceinline__ c128 det_lu_hybrid(const unsigned char* tb, c128* Ls,
 
 template <int N> struct MinorCfg {
     // columns of L kept in shared memory (the rest of the N-4 columns are registers)
-    static constexpr int kSmemCols = (N <= 10) ? 0 : (N == 11 ? 3 : 5);
+    static constexpr int kSmemCols = (N <= 10) ? 0 : (N == 11 ? 2 : 5);
     static constexpr int kThreads = (N <= 11) ? 256 : 128;
     static constexpr int kMinBlocks = (N <= 6) ? 2 : 1;
     static constexpr size_t kSmem = size_t(TILE_BYTES) + size_t(lcol_base<(N > 1 ? N : 2)>(kSmemCols)) * 16 * kThreads;
