@@ -167,111 +167,130 @@ template <int N> __host__ __device__ constexpr int lcol_base(int i) { return i *
 // trailing block as well).  det = (+-) piv_0 ... piv_{K-1} det4(S).  Left-looking: column j of the minor
 // is gathered from shared memory only after the pivots of columns < j are known, in the lane's current
 // row order, so the only data ever exchanged is the active column and the multipliers.
+//
+// The state of the K pivot steps (row order, multipliers, pivot product) depends only on the row tuple
+// and the first K columns, and the six 2x2 minors of trailing columns (K, K+1) only on those and the
+// two columns.  Minors are stored row tuple by row tuple with column tuples in lexicographic order
+// (term_builder.cpp), so consecutive minors of a warp share these prefixes and the state is kept in
+// registers across them (minors_kernel); a minor whose prefix differs starts a fresh elimination.
+// Every minor is still the pivoted LU of its own matrix: identical leading work is not repeated.
+//
 // The multipliers of columns < R live in shared memory (Ls: this thread's slot, entry e at Ls[e * NT],
 // conflict free also for the per-lane dynamic row of the exchange), those of columns R..K-1 in registers.
 // Rows are exchanged only during the K pivot steps; the 4 trailing rows keep whatever order the
-// pivoting left them in (det4 is evaluated in that order, the sign is already in `det`).
-// `tb` = byte address of tile[0][lane]; rb0[i] / cb[j] = byte offsets of row a_i / column b_j.
+// pivoting left them in (det4 is evaluated in that order, the sign is already in `detp`).
+// `tb` = byte address of tile[0][lane]; row / column byte offsets are 12 * a_i * 512 and b_j * 512.
 template <int N, int R, int NT>
-__device__ __forceinline__ c128 det_lu_hybrid(const unsigned char* tb, c128* Ls, const uint32_t (&rb0)[N], const uint32_t (&cb)[N]) {
-    constexpr int K = N - 4;
-    constexpr int KR = (K - R > 0) ? K - R : 1;
-    uint32_t rb[N];
-#pragma unroll
-    for (int r = 0; r < N; ++r) rb[r] = rb0[r];
+struct LuState {
+    static constexpr int K = N - 4;
+    static constexpr int KR = (K - R > 0) ? K - R : 1;
+    uint32_t rb[N];                    // byte offset of the row at position r (per-lane order)
     double Lr[N][KR], Li[N][KR];       // register multipliers: column i >= R at [r][i - R], r > i
-    c128 det = make_double2(1.0, 0.0);
+    c128 detp;                         // (+-) product of the K pivots
+    c128 s[6];                         // 2x2 minors of trailing columns (K, K+1), row pairs 01 02 03 12 13 23
+
     // c[r] -= L[r][i] c[i] for r > i: the elimination of column i applied to the active column
-#define WICK_APPLY_COLUMN(i)                                                                   \
-    _Pragma("unroll") for (int r = (i) + 1; r < N; ++r) {                                      \
-        double lr, li;                                                                         \
-        if ((i) < R) { const c128 l = Ls[(lcol_base<N>(i) + r - (i) - 1) * NT]; lr = l.x; li = l.y; } \
-        else { lr = Lr[r][(i) >= R ? (i) - R : 0]; li = Li[r][(i) >= R ? (i) - R : 0]; }        \
-        cr[r] = fma(-lr, cr[i], fma(li, ci[i], cr[r]));                                        \
-        ci[r] = fma(-lr, ci[i], fma(-li, cr[i], ci[r]));                                       \
-    }
+    template <int I>
+    __device__ __forceinline__ void apply_column(const c128* Ls, double (&cr)[N], double (&ci)[N]) const {
 #pragma unroll
-    for (int j = 0; j < K; ++j) {
-        double cr[N], ci[N];
+        for (int r = I + 1; r < N; ++r) {
+            double lr, li;
+            if constexpr (I < R) { const c128 l = Ls[(lcol_base<N>(I) + r - I - 1) * NT]; lr = l.x; li = l.y; }
+            else { lr = Lr[r][I - R]; li = Li[r][I - R]; }
+            cr[r] = fma(-lr, cr[I], fma(li, ci[I], cr[r]));
+            ci[r] = fma(-lr, ci[I], fma(-li, cr[I], ci[r]));
+        }
+    }
+    template <int I, int J>
+    __device__ __forceinline__ void apply_columns_below(const c128* Ls, double (&cr)[N], double (&ci)[N]) const {
+        if constexpr (I < J) { apply_column<I>(Ls, cr, ci); apply_columns_below<I + 1, J>(Ls, cr, ci); }
+    }
+    __device__ __forceinline__ void load_column(const unsigned char* tb, uint32_t cbj, double (&cr)[N], double (&ci)[N]) const {
 #pragma unroll
         for (int r = 0; r < N; ++r) {
-            const c128 v = *reinterpret_cast<const c128*>(tb + (rb[r] + cb[j]));
+            const c128 v = *reinterpret_cast<const c128*>(tb + (rb[r] + cbj));
             cr[r] = v.x; ci[r] = v.y;
         }
-#pragma unroll
-        for (int i = 0; i < j; ++i) { WICK_APPLY_COLUMN(i) }
+    }
+    // pivot step J on column offset cbj (rows in the order left by steps < J)
+    template <int J>
+    __device__ __forceinline__ void pivot_step(const unsigned char* tb, c128* Ls, uint32_t cbj) {
+        double cr[N], ci[N];
+        load_column(tb, cbj, cr, ci);
+        apply_columns_below<0, J>(Ls, cr, ci);
         // pivot = candidate with the largest |re| + |im| (LAPACK izamax rule) to 2^-20, first maximum wins
-        int p = j;
-        int best = pivot_key(cr[j], ci[j]);
+        int p = J;
+        int best = pivot_key(cr[J], ci[J]);
 #pragma unroll
-        for (int r = j + 1; r < N; ++r) {
+        for (int r = J + 1; r < N; ++r) {
             const int m = pivot_key(cr[r], ci[r]);
             if (m > best) { best = m; p = r; }
         }
-        // exchange positions j and p: active column, row offsets, multipliers of columns < j
-        double pr = cr[j], pi = ci[j];
-        uint32_t po = rb[j];
+        // exchange positions J and p: active column, row offsets, multipliers of columns < J
+        double pr = cr[J], pi = ci[J];
+        uint32_t po = rb[J];
 #pragma unroll
-        for (int r = j + 1; r < N; ++r) {
+        for (int r = J + 1; r < N; ++r) {
             const bool hit = (p == r);
             const double tr = cr[r], ti = ci[r];
             const uint32_t to = rb[r];
-            cr[r] = hit ? cr[j] : tr; ci[r] = hit ? ci[j] : ti; rb[r] = hit ? rb[j] : to;
+            cr[r] = hit ? cr[J] : tr; ci[r] = hit ? ci[J] : ti; rb[r] = hit ? rb[J] : to;
             pr = hit ? tr : pr; pi = hit ? ti : pi; po = hit ? to : po;
         }
-        rb[j] = po;
-        if (R > 0 && j > 0 && p != j) {                         // shared-memory columns: swap rows j and p
+        rb[J] = po;
+        if (R > 0 && J > 0 && p != J) {                         // shared-memory columns: swap rows J and p
 #pragma unroll
-            for (int i = 0; i < (j < R ? j : R); ++i) {
-                c128* ej = Ls + (lcol_base<N>(i) + j - i - 1) * NT;
+            for (int i = 0; i < (J < R ? J : R); ++i) {
+                c128* ej = Ls + (lcol_base<N>(i) + J - i - 1) * NT;
                 c128* ep = Ls + (lcol_base<N>(i) + p - i - 1) * NT;
                 const c128 a = *ej, b = *ep;
                 *ej = b; *ep = a;
             }
         }
 #pragma unroll
-        for (int i = R; i < j; ++i) {                           // register columns: exchange by selects
-            double gr = Lr[j][i - R], gi = Li[j][i - R];
+        for (int i = R; i < J; ++i) {                           // register columns: exchange by selects
+            double gr = Lr[J][i - R], gi = Li[J][i - R];
 #pragma unroll
-            for (int r = j + 1; r < N; ++r) {
+            for (int r = J + 1; r < N; ++r) {
                 const bool hit = (p == r);
                 const double ar = Lr[r][i - R], ai = Li[r][i - R];
-                Lr[r][i - R] = hit ? Lr[j][i - R] : ar; Li[r][i - R] = hit ? Li[j][i - R] : ai;
+                Lr[r][i - R] = hit ? Lr[J][i - R] : ar; Li[r][i - R] = hit ? Li[J][i - R] : ai;
                 gr = hit ? ar : gr; gi = hit ? ai : gi;
             }
-            Lr[j][i - R] = gr; Li[j][i - R] = gi;
+            Lr[J][i - R] = gr; Li[J][i - R] = gi;
         }
         const c128 piv = make_double2(pr, pi);
-        det = (j == 0) ? piv : cmul(det, piv);
-        if (p != j) { det.x = -det.x; det.y = -det.y; }
+        detp = (J == 0) ? piv : cmul(detp, piv);
+        if (p != J) { detp.x = -detp.x; detp.y = -detp.y; }
         const c128 inv = crecip(piv);
 #pragma unroll
-        for (int r = j + 1; r < N; ++r) {
+        for (int r = J + 1; r < N; ++r) {
             const double lr = cr[r] * inv.x - ci[r] * inv.y, li = cr[r] * inv.y + ci[r] * inv.x;
-            if (j < R) Ls[(lcol_base<N>(j) + r - j - 1) * NT] = make_double2(lr, li);
-            else { Lr[r][j >= R ? j - R : 0] = lr; Li[r][j >= R ? j - R : 0] = li; }
+            if constexpr (J < R) Ls[(lcol_base<N>(J) + r - J - 1) * NT] = make_double2(lr, li);
+            else { Lr[r][J - R] = lr; Li[r][J - R] = li; }
         }
     }
-    // trailing columns: apply the K eliminations, keep the last 4 entries; Laplace along column pairs
-    c128 s[6];
+    template <int J>
+    __device__ __forceinline__ void pivot_steps(const unsigned char* tb, c128* Ls, const uint32_t (&cb)[N]) {
+        if constexpr (J < K) { pivot_step<J>(tb, Ls, cb[J]); pivot_steps<J + 1>(tb, Ls, cb); }
+    }
+    // the K pivot steps of a new (row tuple, leading K columns)
+    __device__ __forceinline__ void start(const unsigned char* tb, c128* Ls, const uint32_t (&rb0)[N], const uint32_t (&cb)[N]) {
 #pragma unroll
-    for (int h = 0; h < 2; ++h) {
+        for (int r = 0; r < N; ++r) rb[r] = rb0[r];
+        pivot_steps<0>(tb, Ls, cb);
+    }
+    // two trailing columns: apply the K eliminations, keep the last 4 entries, return their six 2x2 minors
+    __device__ __forceinline__ void column_pair(const unsigned char* tb, const c128* Ls, uint32_t cba, uint32_t cbb, c128 (&d2)[6]) const {
         double tr[2][4], ti[2][4];
 #pragma unroll
         for (int q = 0; q < 2; ++q) {
-            const int j = K + 2 * h + q;
             double cr[N], ci[N];
-#pragma unroll
-            for (int r = 0; r < N; ++r) {
-                const c128 v = *reinterpret_cast<const c128*>(tb + (rb[r] + cb[j]));
-                cr[r] = v.x; ci[r] = v.y;
-            }
-#pragma unroll
-            for (int i = 0; i < K; ++i) { WICK_APPLY_COLUMN(i) }
+            load_column(tb, q == 0 ? cba : cbb, cr, ci);
+            apply_columns_below<0, K>(Ls, cr, ci);
 #pragma unroll
             for (int r = 0; r < 4; ++r) { tr[q][r] = cr[K + r]; ti[q][r] = ci[K + r]; }
         }
-        c128 d2[6];
         int k = 0;
 #pragma unroll
         for (int a = 0; a < 4; ++a)
@@ -279,24 +298,24 @@ __device__ __forceinline__ c128 det_lu_hybrid(const unsigned char* tb, c128* Ls,
             for (int b = a + 1; b < 4; ++b)
                 d2[k++] = det2(make_double2(tr[0][a], ti[0][a]), make_double2(tr[1][a], ti[1][a]),
                                make_double2(tr[0][b], ti[0][b]), make_double2(tr[1][b], ti[1][b]));
-        if (h == 0) {
-#pragma unroll
-            for (int q = 0; q < 6; ++q) s[q] = d2[q];
-        } else {
-            // pairs in order (01,02,03,12,13,23); complement of pair q is pair 5-q; signs + - + + - +
-            c128 d = cmul(s[0], d2[5]);
-            d = cfnma(s[1], d2[4], d);
-            d = cfma(s[2], d2[3], d);
-            d = cfma(s[3], d2[2], d);
-            d = cfnma(s[4], d2[1], d);
-            d = cfma(s[5], d2[0], d);
-            det = cmul(det, d);
-        }
     }
-    return det;
-}
-
-#undef WICK_APPLY_COLUMN
+    __device__ __forceinline__ void first_pair(const unsigned char* tb, const c128* Ls, uint32_t cba, uint32_t cbb) {
+        column_pair(tb, Ls, cba, cbb, s);
+    }
+    // Laplace expansion of the 4x4 Schur complement along its column pairs (01 | 23):
+    // pairs in order (01,02,03,12,13,23); the complement of pair q is pair 5-q; signs + - + + - +
+    __device__ __forceinline__ c128 finish(const unsigned char* tb, const c128* Ls, uint32_t cba, uint32_t cbb) const {
+        c128 d2[6];
+        column_pair(tb, Ls, cba, cbb, d2);
+        c128 d = cmul(s[0], d2[5]);
+        d = cfnma(s[1], d2[4], d);
+        d = cfma(s[2], d2[3], d);
+        d = cfma(s[3], d2[2], d);
+        d = cfnma(s[4], d2[1], d);
+        d = cfma(s[5], d2[0], d);
+        return cmul(detp, d);
+    }
+};
 
 template <int N> struct MinorCfg {
     // columns of L kept in shared memory (the rest of the N-4 columns are registers)
@@ -318,6 +337,8 @@ template <int N> struct Desc {
         else { const ulonglong2 v = __ldg(reinterpret_cast<const ulonglong2*>(tab) + m); d.w[0] = v.x; d.w[1] = v.y; }
         return d;
     }
+    __device__ __forceinline__ unsigned long long rows_bits() const { return kWords == 1 ? (w[0] & 0xffffffffull) : w[0]; }
+    __device__ __forceinline__ unsigned long long cols_bits() const { return kWords == 1 ? (w[0] >> 32) : w[kWords - 1]; }
     __device__ __forceinline__ uint32_t row(int i) const {
         if constexpr (kWords == 1) return (uint32_t(w[0]) >> (4 * i)) & 15u;
         else return uint32_t(w[0] >> (4 * i)) & 15u;
@@ -340,31 +361,52 @@ minors_kernel(const c128* __restrict__ P, int64_t st0, int64_t n_st_total, int S
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int m_begin = blockIdx.y * chunk;
     const int m_end = min(n_minors, m_begin + chunk);
-    int m = m_begin + warp;
+    // N <= 4: warp w takes minors m_begin + w, + NT/32, ...; N >= 5: a contiguous piece of the chunk, so
+    // that consecutive minors share their row tuple and leading columns (see LuState)
+    constexpr int kStride = (N <= 4) ? NT / 32 : 1;
+    int m = (N <= 4) ? m_begin + warp : m_begin + warp * (chunk / (NT / 32));
+    const int m_stop = (N <= 4) ? m_end : min(m_end, m + chunk / (NT / 32));
     Desc<N> dn;                                                // descriptor of the next minor, fetched one iteration ahead
-    if (m < m_end) dn = Desc<N>::load(desc, m);
+    if (m < m_stop) dn = Desc<N>::load(desc, m);
     stage_tile(tile, P, st_first, n_st_total, NT);
     __syncthreads();
     const c128* tl = tile + lane;
     const bool valid = st_first + lane < n_st_total;
     c128* outp = out + int64_t(g) * GROUP + lane;
-    for (; m < m_end; m += NT / 32) {
-        const Desc<N> dc = dn;
-        if (m + NT / 32 < m_end) dn = Desc<N>::load(desc, m + NT / 32);
-        c128 det;
-        if constexpr (N <= 4) {
+    if constexpr (N <= 4) {
+        for (; m < m_stop; m += kStride) {
+            const Desc<N> dc = dn;
+            if (m + kStride < m_stop) dn = Desc<N>::load(desc, m + kStride);
             Idx<N> ix;
 #pragma unroll
             for (int i = 0; i < N; ++i) { ix.re[i] = int(dc.row(i)) * 12; ix.ce[i] = int(dc.col(i)); }
-            det = det_small<N>(tl, ix);
-        } else {
-            uint32_t rb[N], cb[N];
-#pragma unroll
-            for (int i = 0; i < N; ++i) { rb[i] = dc.row(i) * (12 * GROUP * 16); cb[i] = dc.col(i) * (GROUP * 16); }
-            det = det_lu_hybrid<N, MinorCfg<N>::kSmemCols, NT>(reinterpret_cast<const unsigned char*>(tl),
-                                                               tile + TILE_ELEMS + threadIdx.x, rb, cb);
+            const c128 det = det_small<N>(tl, ix);
+            if (valid) outp[int64_t(m) * S_b] = det;
         }
-        if (valid) outp[int64_t(m) * S_b] = det;
+    } else {
+        constexpr int K = N - 4;
+        constexpr uint32_t kRowStep = 12 * GROUP * 16, kColStep = GROUP * 16;
+        constexpr unsigned long long kLead = (1ull << (4 * K)) - 1, kLeadPair = (1ull << (4 * (K + 2))) - 1;
+        const unsigned char* tb = reinterpret_cast<const unsigned char*>(tl);
+        c128* Ls = tile + TILE_ELEMS + threadIdx.x;
+        LuState<N, MinorCfg<N>::kSmemCols, NT> lu;
+        unsigned long long prow = ~0ull, pcol = 0;              // no index set has all 64 bits set: the first minor starts fresh
+        for (; m < m_stop; ++m) {
+            const Desc<N> dc = dn;
+            if (m + 1 < m_stop) dn = Desc<N>::load(desc, m + 1);
+            const unsigned long long rws = dc.rows_bits(), diff = dc.cols_bits() ^ pcol;
+            const bool fresh = (rws != prow) || (diff & kLead) != 0;
+            if (fresh) {
+                uint32_t rb[N], cb[N];
+#pragma unroll
+                for (int i = 0; i < N; ++i) { rb[i] = dc.row(i) * kRowStep; cb[i] = dc.col(i) * kColStep; }
+                lu.start(tb, Ls, rb, cb);
+            }
+            if (fresh || (diff & kLeadPair) != 0) lu.first_pair(tb, Ls, dc.col(K) * kColStep, dc.col(K + 1) * kColStep);
+            const c128 det = lu.finish(tb, Ls, dc.col(K + 2) * kColStep, dc.col(K + 3) * kColStep);
+            prow = rws; pcol = dc.cols_bits();
+            if (valid) outp[int64_t(m) * S_b] = det;
+        }
     }
 }
 
