@@ -4,6 +4,7 @@
 #include <algorithm>
 #include <cstdio>
 #include <cstring>
+#include <map>
 #include <string>
 #include <vector>
 
@@ -246,6 +247,162 @@ int upload_tables(const wick_terms* t, cudaStream_t stream) {
     return WICK_OK;
 }
 
+// ---- staged factorised reduction: host schedule (kernels.cu: reduce_staged_kernel) --------------
+// Tuples grouped by block: ru_list / rd_list by sink block, cu_list / cd_list by source block.
+// Batches = (source block k', d-column piece) x (run of sink blocks) with at most STG_MD_CAP MD elements;
+// batches are assigned to n_bins CTAs by longest-processing-time, each bin keeps a fixed order.
+// Returns 1 and fills `out` when the list is eligible, 0 when a block is too large (caller falls back
+// to reduce_outer_kernel), negative on error.
+int ensure_staged(const wick_terms* t, int n_bins, cudaStream_t stream, StagedTables* out) {
+    std::lock_guard<std::mutex> lock(t->mu);
+    DeviceTables& d = t->dev;
+    if (d.staged_state < 0) return 0;
+    const int nru = int(t->f[0].rows.size()), nrd = int(t->f[1].rows.size());
+    const int ncu = int(t->f[0].cols.size()), ncd = int(t->f[1].cols.size());
+    auto fill = [&](const StagedDev& sd) {
+        out->n_cols_u = ncu; out->n_cols_d = ncd; out->n_bins = sd.n_bins;
+        out->sink_ptr = sd.sink_ptr; out->sink_rdpos = sd.sink_rdpos; out->sink_c = reinterpret_cast<const double2*>(sd.sink_c);
+        out->src_ptr = sd.src_ptr; out->src_cupos = sd.src_cupos; out->src_c = reinterpret_cast<const double2*>(sd.src_c);
+        out->ru_list = sd.ru_list; out->rd_list = sd.rd_list; out->cu_list = sd.cu_list; out->cd_list = sd.cd_list;
+        out->bin_ptr = sd.bin_ptr; out->batches = static_cast<const StagedBatch*>(sd.batches);
+    };
+    auto hit = d.staged.find(n_bins);
+    if (hit != d.staged.end()) { fill(hit->second); return 1; }
+
+    const Components cs = factor_components(nru, nrd, t->sink);
+    const Components cq = factor_components(ncu, ncd, t->source);
+    auto group = [](const std::vector<int>& comp_of, int n_comp, std::vector<int32_t>& ptr, std::vector<int32_t>& list, std::vector<int32_t>& pos) {
+        ptr.assign(size_t(n_comp) + 1, 0);
+        for (int c : comp_of) if (c >= 0) ptr[size_t(c) + 1]++;
+        for (int c = 0; c < n_comp; ++c) ptr[size_t(c) + 1] += ptr[size_t(c)];
+        list.resize(size_t(ptr[size_t(n_comp)]));
+        pos.assign(comp_of.size(), -1);
+        std::vector<int32_t> next(ptr.begin(), ptr.end() - 1);
+        for (size_t x = 0; x < comp_of.size(); ++x)
+            if (comp_of[x] >= 0) { pos[x] = next[size_t(comp_of[x])]++; list[size_t(pos[x])] = int32_t(x); }
+    };
+    std::vector<int32_t> ru_ptr, ru_list, ru_pos, rd_ptr, rd_list, rd_pos, cu_ptr, cu_list, cu_pos, cd_ptr, cd_list, cd_pos;
+    group(cs.of_u, cs.n, ru_ptr, ru_list, ru_pos);
+    group(cs.of_d, cs.n, rd_ptr, rd_list, rd_pos);
+    group(cq.of_u, cq.n, cu_ptr, cu_list, cu_pos);
+    group(cq.of_d, cq.n, cd_ptr, cd_list, cd_pos);
+    int max_rd = 1, max_cu = 1;
+    for (int k = 0; k < cs.n; ++k) max_rd = std::max(max_rd, rd_ptr[size_t(k) + 1] - rd_ptr[size_t(k)]);
+    for (int k = 0; k < cq.n; ++k) max_cu = std::max(max_cu, cu_ptr[size_t(k) + 1] - cu_ptr[size_t(k)]);
+    if (max_rd > STG_MD_CAP || max_cu > STG_ROW_CAP || cs.n == 0 || cq.n == 0) { d.staged_state = -1; return 0; }
+
+    // coefficient lists regrouped by list position, so that a batch's entries are contiguous:
+    // sink entries by position of ru in ru_list, source entries by position of cd in cd_list
+    std::vector<int32_t> sink_ptr(size_t(nru) + 1, 0), src_ptr(size_t(ncd) + 1, 0);
+    for (const FactorTerm& f : t->sink) sink_ptr[size_t(ru_pos[size_t(f.qu)]) + 1]++;
+    for (const FactorTerm& f : t->source) src_ptr[size_t(cd_pos[size_t(f.qd)]) + 1]++;
+    for (int r = 0; r < nru; ++r) sink_ptr[size_t(r) + 1] += sink_ptr[size_t(r)];
+    for (int c = 0; c < ncd; ++c) src_ptr[size_t(c) + 1] += src_ptr[size_t(c)];
+    std::vector<int32_t> sink_rdpos(t->sink.size()), src_cupos(t->source.size());
+    std::vector<double> sink_c(2 * t->sink.size()), src_c(2 * t->source.size());
+    {
+        std::vector<int32_t> next(sink_ptr.begin(), sink_ptr.end() - 1);
+        for (const FactorTerm& f : t->sink) {                  // t->sink is sorted by (ru, rd): order within a row is kept
+            const size_t e = size_t(next[size_t(ru_pos[size_t(f.qu)])]++);
+            sink_rdpos[e] = rd_pos[size_t(f.qd)]; sink_c[2 * e] = f.c.real(); sink_c[2 * e + 1] = f.c.imag();
+        }
+        std::vector<FactorTerm> src = t->source;
+        std::stable_sort(src.begin(), src.end(), [](const FactorTerm& a, const FactorTerm& b) {
+            return a.qd != b.qd ? a.qd < b.qd : a.qu < b.qu; });
+        std::vector<int32_t> nextq(src_ptr.begin(), src_ptr.end() - 1);
+        for (const FactorTerm& f : src) {
+            const size_t e = size_t(nextq[size_t(cd_pos[size_t(f.qd)])]++);
+            src_cupos[e] = cu_pos[size_t(f.qu)]; src_c[2 * e] = f.c.real(); src_c[2 * e + 1] = f.c.imag();
+        }
+    }
+    // a single u-row tuple or a single d column must fit the entry buffers
+    for (int r = 0; r < nru; ++r) if (sink_ptr[size_t(r) + 1] - sink_ptr[size_t(r)] > STG_SINK_CAP) { d.staged_state = -1; return 0; }
+    for (int c = 0; c < ncd; ++c) if (src_ptr[size_t(c) + 1] - src_ptr[size_t(c)] > STG_SRC_CAP) { d.staged_state = -1; return 0; }
+    for (int k = 0; k < cs.n; ++k)                              // one sink block must fit a batch on its own
+        if (ru_ptr[size_t(k) + 1] - ru_ptr[size_t(k)] > STG_ROWS_CAP ||
+            sink_ptr[size_t(ru_ptr[size_t(k) + 1])] - sink_ptr[size_t(ru_ptr[size_t(k)])] > STG_SINK_CAP) { d.staged_state = -1; return 0; }
+    d.staged_state = 1;
+
+    struct Item { int64_t cost; StagedBatch b; };
+    std::vector<Item> items;
+    for (int kp = 0; kp < cq.n; ++kp) {
+        const int cdA = cd_ptr[size_t(kp)], cdB = cd_ptr[size_t(kp) + 1];
+        const int cuA = cu_ptr[size_t(kp)], cuB = cu_ptr[size_t(kp) + 1];
+        // equal pieces of the block's d columns, each small enough for the largest sink block
+        const int piece_max = std::max(1, std::min(std::min(cdB - cdA, STG_NCD_CAP), STG_MD_CAP / max_rd));
+        const int n_pieces = (cdB - cdA + piece_max - 1) / piece_max;
+        const int piece = (cdB - cdA + n_pieces - 1) / n_pieces;
+        for (int ca = cdA; ca < cdB;) {
+            int cb = std::min(cdB, ca + piece);
+            while (cb > ca + 1 && src_ptr[size_t(cb)] - src_ptr[size_t(ca)] > STG_SRC_CAP) --cb;   // source entries of the piece
+            const int n_cd = cb - ca;
+            const int64_t src_work = (src_ptr[size_t(cb)] - src_ptr[size_t(ca)]) + n_cd;
+            int ka = 0;
+            while (ka < cs.n) {
+                int kb = ka, n_rd = 0;
+                while (kb < cs.n) {
+                    const int n_rd2 = n_rd + rd_ptr[size_t(kb) + 1] - rd_ptr[size_t(kb)];
+                    const int rows2 = ru_ptr[size_t(kb) + 1] - ru_ptr[size_t(ka)];
+                    const int ent2 = sink_ptr[size_t(ru_ptr[size_t(kb) + 1])] - sink_ptr[size_t(ru_ptr[size_t(ka)])];
+                    if (kb > ka && (n_rd2 * n_cd > STG_MD_CAP || rows2 > STG_ROWS_CAP || ent2 > STG_SINK_CAP)) break;
+                    n_rd = n_rd2;
+                    ++kb;
+                }
+                Item it;
+                it.b = StagedBatch{ca, cb, cuA, cuB, rd_ptr[size_t(ka)], rd_ptr[size_t(kb)], ru_ptr[size_t(ka)], ru_ptr[size_t(kb)]};
+                const int rows = ru_ptr[size_t(kb)] - ru_ptr[size_t(ka)];
+                const int ent = sink_ptr[size_t(ru_ptr[size_t(kb)])] - sink_ptr[size_t(ru_ptr[size_t(ka)])];
+                it.cost = int64_t(n_rd) * n_cd + 16 + int64_t(rows) * ((cuB - cuA) + src_work + 4) + int64_t(ent) * n_cd;
+                items.push_back(it);
+                ka = kb;
+            }
+            ca = cb;
+        }
+    }
+    std::stable_sort(items.begin(), items.end(), [](const Item& a, const Item& b) { return a.cost > b.cost; });
+    std::vector<std::vector<StagedBatch>> bins(static_cast<size_t>(n_bins));
+    std::vector<std::pair<int64_t, int>> heap;
+    for (int b = 0; b < n_bins; ++b) heap.push_back({0, b});
+    auto cmp = [](const std::pair<int64_t, int>& a, const std::pair<int64_t, int>& b) { return a > b; };
+    std::make_heap(heap.begin(), heap.end(), cmp);
+    for (const Item& it : items) {
+        std::pop_heap(heap.begin(), heap.end(), cmp);
+        bins[size_t(heap.back().second)].push_back(it.b);
+        heap.back().first += it.cost;
+        std::push_heap(heap.begin(), heap.end(), cmp);
+    }
+    std::vector<int32_t> bin_ptr(size_t(n_bins) + 1, 0);
+    std::vector<StagedBatch> batches;
+    for (int b = 0; b < n_bins; ++b) {
+        batches.insert(batches.end(), bins[size_t(b)].begin(), bins[size_t(b)].end());
+        bin_ptr[size_t(b) + 1] = int32_t(batches.size());
+    }
+    BlobBuilder bb;
+    const size_t o_srp = bb.add(sink_rdpos.data(), sink_rdpos.size() * 4), o_scp = bb.add(src_cupos.data(), src_cupos.size() * 4);
+    const size_t o_sp = bb.add(sink_ptr.data(), sink_ptr.size() * 4), o_qp = bb.add(src_ptr.data(), src_ptr.size() * 4);
+    const size_t o_sc = bb.add(sink_c.data(), sink_c.size() * 8), o_qc = bb.add(src_c.data(), src_c.size() * 8);
+    const size_t o_ru = bb.add(ru_list.data(), ru_list.size() * 4), o_rd = bb.add(rd_list.data(), rd_list.size() * 4);
+    const size_t o_cu = bb.add(cu_list.data(), cu_list.size() * 4), o_cd = bb.add(cd_list.data(), cd_list.size() * 4);
+    const size_t o_bp = bb.add(bin_ptr.data(), bin_ptr.size() * 4), o_ba = bb.add(batches.data(), batches.size() * sizeof(StagedBatch));
+    void* blob = nullptr;
+    WICK_CUDA(cudaMalloc(&blob, std::max<size_t>(bb.host.size(), 256)));
+    cudaError_t e = cudaMemcpyAsync(blob, bb.host.data(), bb.host.size(), cudaMemcpyHostToDevice, stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(stream);   // bb.host dies at scope exit
+    if (e != cudaSuccess) { cudaFree(blob); set_error(std::string("staged schedule upload: ") + cudaGetErrorString(e)); return WICK_ERR_CUDA; }
+    unsigned char* b = static_cast<unsigned char*>(blob);
+    StagedDev sd;
+    sd.blob = blob; sd.n_bins = n_bins;
+    sd.sink_rdpos = reinterpret_cast<const int32_t*>(b + o_srp); sd.src_cupos = reinterpret_cast<const int32_t*>(b + o_scp);
+    sd.sink_ptr = reinterpret_cast<const int32_t*>(b + o_sp); sd.src_ptr = reinterpret_cast<const int32_t*>(b + o_qp);
+    sd.sink_c = reinterpret_cast<const double*>(b + o_sc); sd.src_c = reinterpret_cast<const double*>(b + o_qc);
+    sd.ru_list = reinterpret_cast<const int32_t*>(b + o_ru); sd.rd_list = reinterpret_cast<const int32_t*>(b + o_rd);
+    sd.cu_list = reinterpret_cast<const int32_t*>(b + o_cu); sd.cd_list = reinterpret_cast<const int32_t*>(b + o_cd);
+    sd.bin_ptr = reinterpret_cast<const int32_t*>(b + o_bp); sd.batches = b + o_ba;
+    d.staged[n_bins] = sd;
+    fill(sd);
+    return 1;
+}
+
 int upload_flat(const wick_terms* t, cudaStream_t stream) {
     try { t->ensure_flat(); } catch (const std::bad_alloc&) { set_error("flat term list: out of host memory"); return WICK_ERR_NOMEM; }
     std::lock_guard<std::mutex> lock(t->mu);
@@ -300,6 +457,15 @@ bool make_plan(const wick_terms* t, int L, int T, int n_mom, size_t workspace_by
     sb = std::min<int64_t>(sb, n_st_pad);
     sb = std::min<int64_t>(sb, int64_t(1) << 22);             // keeps grid.x and 32-bit site offsets small
     if (want_max) sb = std::max<int64_t>(sb, GROUP);
+    // the staged reduction runs n_groups x floor(148 / n_groups) CTAs (or n_groups when >= 148), one per SM:
+    // shrink the batch until that grid fills at least 90 % of its last wave
+    auto wave_fill = [](int64_t g) {
+        if (g < 148) return double(g * (148 / g)) / 148.0;
+        return double(g) / double((g + 147) / 148 * 148);
+    };
+    int64_t g = sb / GROUP;
+    while (g > 1 && wave_fill(g) < 0.9) --g;
+    sb = g * GROUP;
     p->S_b = sb;
     return true;
 }
@@ -311,6 +477,7 @@ size_t plan_bytes(const Plan& p, int64_t S_b) { return p.sigma_bytes + 1024 + si
 extern "C" void wick_terms_release_device(DeviceTables* d) {
     if (d->blob) cudaFree(d->blob);
     if (d->flat_blob) cudaFree(d->flat_blob);
+    for (auto& kv : d->staged) cudaFree(kv.second.blob);
     *d = DeviceTables();
 }
 
@@ -372,6 +539,17 @@ extern "C" int wick_contract(const void* U_dev, const void* D_dev, const wick_te
     const double2* U = static_cast<const double2*>(U_dev);
     const double2* D = static_cast<const double2*>(D_dev);
 
+    // staged factorised reduction: one CTA per SM, n_groups x n_bins CTAs ~ one wave of 148
+    StagedTables stg;
+    bool have_staged = false;
+    if (use_outer && t->n_terms > 0 && !(flags & WICK_CONTRACT_NO_STAGED) &&
+        std::max(nmu, nmd) * int64_t(S_b) < (int64_t(1) << 31)) {   // the staged kernel keeps 32-bit element offsets
+        const int groups_full = int(std::min<int64_t>(S_b, (p.n_st + GROUP - 1) / GROUP * GROUP) / GROUP);
+        const int n_bins = std::max(1, std::min(MAX_CHUNKS, 148 * STG_CTAS_PER_SM / std::max(1, groups_full)));
+        rc = ensure_staged(t, n_bins, stream, &stg);
+        if (rc < 0) return rc;
+        have_staged = (rc == 1);
+    }
     for (int64_t st0 = 0; st0 < p.n_st; st0 += S_b) {
         const int64_t n_valid = std::min<int64_t>(S_b, p.n_st - st0);
         const int n_groups = int((n_valid + GROUP - 1) / GROUP);
@@ -381,7 +559,9 @@ extern "C" int wick_contract(const void* U_dev, const void* D_dev, const wick_te
         if (t->n_terms == 0) {
             WICK_CUDA(cudaMemsetAsync(sigma + st0, 0, size_t(n_valid) * 16, stream));
         } else {
-            if (use_outer) {
+            if (use_outer && have_staged) {
+                WICK_CUDA(launch_reduce_staged(MU, MD, n_groups, S_b, stg, partial, &n_chunks, stream));
+            } else if (use_outer) {
                 OuterTables ot;
                 ot.n_cols_u = int(t->f[0].cols.size()); ot.n_cols_d = int(t->f[1].cols.size());
                 ot.sink_ptr = d.sink_ptr; ot.sink_rdoff = d.sink_rdoff; ot.sink_c = reinterpret_cast<const double2*>(d.sink_c);

@@ -446,19 +446,6 @@ cudaError_t launch_minors(int n, const double2* P, int64_t st0, int64_t n_st_tot
 #undef WICK_CASE
 }
 
-template <int N> static cudaError_t set_smem_attr() {
-    return cudaFuncSetAttribute(minors_kernel<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(MinorCfg<N>::kSmem));
-}
-
-cudaError_t configure_kernels() {
-    cudaError_t e;
-#define WICK_ATTR(N) if ((e = set_smem_attr<N>()) != cudaSuccess) return e;
-    WICK_ATTR(0) WICK_ATTR(1) WICK_ATTR(2) WICK_ATTR(3) WICK_ATTR(4) WICK_ATTR(5) WICK_ATTR(6)
-    WICK_ATTR(7) WICK_ATTR(8) WICK_ATTR(9) WICK_ATTR(10) WICK_ATTR(11) WICK_ATTR(12)
-#undef WICK_ATTR
-    return cudaSuccess;
-}
-
 // ---------------------------------------------------------------------------------------------
 // a5: weighted bilinear products.  Lane = site; term indices and weights are warp-uniform.
 // Each CTA handles one 32-site group and one chunk of the work; its warps' partial sums are
@@ -536,6 +523,188 @@ reduce_outer_kernel(const c128* __restrict__ MU, const c128* __restrict__ MD, in
         }
     }
     cta_combine_store(acc, partial + int64_t(blockIdx.y) * S_b + int64_t(blockIdx.x) * GROUP);
+}
+
+// ---------------------------------------------------------------------------------------------
+// a5, staged factorised reduction (outer-product lists whose blocks fit the STG_* capacities).
+//   sigma = sum over (sink block k, source block k') of
+//           sum_{ru in k} sum_{cd in k'} ( sum_{j in src[cd]} cbar_j MU[ru, cu_j] ) ( sum_{i in sink[ru]} c_i MD[rd_i, cd] )
+// A batch = (d columns cd_a..cd_b of one source block) x (sink blocks ka..kb).  Per batch the CTA copies
+// into shared memory, once: the MD elements [rd in blocks][cd] (cp.async, 16 B per lane, 512-byte rows)
+// and the two coefficient lists it needs (source entries of the d columns, sink entries of the u-row
+// tuples), so the inner loops touch no global table.  Warp w then takes the u-row tuples ru_a + w, + W, ...:
+// the row MU[ru, cu in k'] goes to its private buffer (the next row is already in flight in registers),
+//   P[cd] = sum_i c_i MD[rd_i, cd]            (cd unrolled: registers, one LDS + 4 DFMA per term)
+//   acc  += sum_cd P[cd] * sum_j cbar_j row[cu_j]
+// Every minor is read from DRAM once per batch that needs it.  Work order is fixed by the host
+// schedule: bit-reproducible.
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ void cp_async16(void* smem_dst, const void* gmem_src) {
+    const uint32_t d = static_cast<uint32_t>(__cvta_generic_to_shared(smem_dst));
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d), "l"(gmem_src) : "memory");
+}
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.commit_group;\n\tcp.async.wait_group 0;" ::: "memory"); }
+
+constexpr int STG_W = STG_THREADS / 32;
+// shared memory map (bytes)
+constexpr size_t STG_OFF_ROWS = size_t(STG_MD_CAP) * GROUP * 16;
+constexpr size_t STG_OFF_SINKC = STG_OFF_ROWS + size_t(STG_W) * STG_ROW_CAP * GROUP * 16;   // c128[STG_SINK_CAP]
+constexpr size_t STG_OFF_SRCC = STG_OFF_SINKC + size_t(STG_SINK_CAP) * 16;                  // c128[STG_SRC_CAP]
+constexpr size_t STG_OFF_SINKO = STG_OFF_SRCC + size_t(STG_SRC_CAP) * 16;                   // int[STG_SINK_CAP] MD element offset
+constexpr size_t STG_OFF_SRCO = STG_OFF_SINKO + size_t(STG_SINK_CAP) * 4;                   // int[STG_SRC_CAP]  row element offset
+constexpr size_t STG_OFF_SINKP = STG_OFF_SRCO + size_t(STG_SRC_CAP) * 4;                    // int[STG_ROWS_CAP + 1] per-row entry ranges
+constexpr size_t STG_OFF_ROWOFF = STG_OFF_SINKP + size_t(STG_ROWS_CAP + 2) * 4;             // int[STG_ROWS_CAP] MU row offsets
+constexpr size_t STG_OFF_SRCP = STG_OFF_ROWOFF + size_t(STG_ROWS_CAP + 2) * 4;              // int[16] per-cd entry ranges, int[16] u column offsets
+constexpr size_t STG_SMEM = STG_OFF_SRCP + 32 * 4;
+
+// All u-row tuples of a batch that belong to this warp.  NCU / NCD = compile-time bounds on the u columns
+// of the source block and on the d columns of the piece (loops over them are unrolled and predicated).
+template <int NCU, int NCD>
+__device__ __forceinline__ c128 staged_rows(const c128* MUs, const c128* MDl, c128* row, int warp, int n_rows, int n_cu, int n_cd,
+                                            const int* rowoff, const int* cuoff, const int* sinkp, const c128* sinkc,
+                                            const int* sinko, const int* srcp, const c128* srcc, const int* srco) {
+    c128 acc = make_double2(0.0, 0.0);
+    c128 X[NCU];
+#pragma unroll
+    for (int c = 0; c < NCU; ++c) X[c] = make_double2(0.0, 0.0);
+    int r = warp;
+    if (r < n_rows) {                                                    // first row: global -> registers
+        const c128* src = MUs + rowoff[r];
+#pragma unroll
+        for (int c = 0; c < NCU; ++c)
+            if (c < n_cu) X[c] = __ldg(src + cuoff[c]);
+    }
+    for (; r < n_rows; r += STG_W) {
+#pragma unroll
+        for (int c = 0; c < NCU; ++c)
+            if (c < n_cu) row[c * GROUP] = X[c];
+        __syncwarp();
+        if (r + STG_W < n_rows) {                                        // next row: in flight during this row's arithmetic
+            const c128* src = MUs + rowoff[r + STG_W];
+#pragma unroll
+            for (int c = 0; c < NCU; ++c)
+                if (c < n_cu) X[c] = __ldg(src + cuoff[c]);
+        }
+        // P[cd] = sum_i c_i MD[rd_i, cd]
+        c128 P[NCD];
+#pragma unroll
+        for (int c = 0; c < NCD; ++c) P[c] = make_double2(0.0, 0.0);
+        const int i0 = sinkp[r], i1 = sinkp[r + 1];
+        for (int i = i0; i < i1; ++i) {
+            const c128 a = sinkc[i];
+            const c128* md = MDl + sinko[i];                     // element (rd_i, first cd of the piece), this lane
+#pragma unroll
+            for (int c = 0; c < NCD; ++c)
+                if (c < n_cd) P[c] = cfma(a, md[c * GROUP], P[c]);
+        }
+        // acc += sum_cd P[cd] * sum_j cbar_j MU[ru, cu_j]
+#pragma unroll
+        for (int c = 0; c < NCD; ++c) {
+            if (c < n_cd) {
+                const int j0 = srcp[c], j1 = srcp[c + 1];
+                c128 q = make_double2(0.0, 0.0);
+                for (int j = j0; j < j1; ++j) q = cfma(srcc[j], row[srco[j]], q);
+                acc = cfma(q, P[c], acc);
+            }
+        }
+        __syncwarp();                                                    // all lanes have read the row buffer
+    }
+    return acc;
+}
+
+template <int NCU>
+__device__ __forceinline__ c128 staged_rows_ncd(const c128* MUs, const c128* MDl, c128* row, int warp, int n_rows, int n_cu, int n_cd,
+                                                const int* rowoff, const int* cuoff, const int* sinkp, const c128* sinkc,
+                                                const int* sinko, const int* srcp, const c128* srcc, const int* srco) {
+#define WICK_STG_CALL(NCD) staged_rows<NCU, NCD>(MUs, MDl, row, warp, n_rows, n_cu, n_cd, rowoff, cuoff, sinkp, sinkc, sinko, srcp, srcc, srco)
+    if (n_cd <= 1) return WICK_STG_CALL(1);
+    if (n_cd <= 2) return WICK_STG_CALL(2);
+    if (n_cd <= 4) return WICK_STG_CALL(4);
+    return WICK_STG_CALL(STG_NCD_CAP);
+#undef WICK_STG_CALL
+}
+
+__global__ void __launch_bounds__(STG_THREADS, STG_CTAS_PER_SM)
+reduce_staged_kernel(const c128* __restrict__ MU, const c128* __restrict__ MD, int S_b, StagedTables st,
+                     c128* __restrict__ partial) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    c128* MDs = reinterpret_cast<c128*>(smem_raw);                       // [element][lane]
+    c128* sinkc = reinterpret_cast<c128*>(smem_raw + STG_OFF_SINKC);
+    c128* srcc = reinterpret_cast<c128*>(smem_raw + STG_OFF_SRCC);
+    int* sinko = reinterpret_cast<int*>(smem_raw + STG_OFF_SINKO);
+    int* srco = reinterpret_cast<int*>(smem_raw + STG_OFF_SRCO);
+    int* sinkp = reinterpret_cast<int*>(smem_raw + STG_OFF_SINKP);        // [0..rows]: sink entry ranges
+    int* rowoff = reinterpret_cast<int*>(smem_raw + STG_OFF_ROWOFF);      // [rows]: element offset of MU[ru, 0]
+    int* srcp = reinterpret_cast<int*>(smem_raw + STG_OFF_SRCP);          // [0..n_cd]: source entry ranges
+    int* cuoff = srcp + 16;                                               // [n_cu]: element offset of u column tuple
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    c128* row = reinterpret_cast<c128*>(smem_raw + STG_OFF_ROWS) + warp * STG_ROW_CAP * GROUP + lane;
+    const c128* MDl = MDs + lane;
+    const int64_t s = int64_t(blockIdx.x) * GROUP + lane;
+    const c128* MUs = MU + s;
+    const c128* MDg = MD + s;
+    c128 acc = make_double2(0.0, 0.0);
+    const int b0 = __ldg(st.bin_ptr + blockIdx.y), b1 = __ldg(st.bin_ptr + blockIdx.y + 1);
+    for (int b = b0; b < b1; ++b) {
+        const int4 v0 = __ldg(reinterpret_cast<const int4*>(st.batches + b));
+        const int4 v1 = __ldg(reinterpret_cast<const int4*>(st.batches + b) + 1);
+        const int cd_a = v0.x, n_cd = v0.y - v0.x, cu_a = v0.z, n_cu = v0.w - v0.z;
+        const int rd_a = v1.x, n_rd = v1.y - v1.x, ru_a = v1.z, n_rows = v1.w - v1.z;
+        __syncthreads();                                                 // every warp is done with the previous batch
+        for (int e = warp; e < n_rd * n_cd; e += STG_W) {
+            const int rdi = e / n_cd, cdi = e - rdi * n_cd;
+            const int id = __ldg(st.rd_list + rd_a + rdi) * st.n_cols_d + __ldg(st.cd_list + cd_a + cdi);
+            cp_async16(MDs + e * GROUP + lane, MDg + int64_t(id) * S_b);
+        }
+        // coefficient lists of the batch -> shared memory, offsets already in elements of the staged buffers
+        const int sp0 = __ldg(st.sink_ptr + ru_a), sp1 = __ldg(st.sink_ptr + ru_a + n_rows);
+        for (int e = threadIdx.x; e < sp1 - sp0; e += STG_THREADS) {
+            sinkc[e] = __ldg(st.sink_c + sp0 + e);
+            sinko[e] = (__ldg(st.sink_rdpos + sp0 + e) - rd_a) * n_cd * GROUP;
+        }
+        for (int r = threadIdx.x; r <= n_rows; r += STG_THREADS) {
+            sinkp[r] = __ldg(st.sink_ptr + ru_a + r) - sp0;
+            if (r < n_rows) rowoff[r] = __ldg(st.ru_list + ru_a + r) * st.n_cols_u * S_b;
+        }
+        const int q0 = __ldg(st.src_ptr + cd_a), q1 = __ldg(st.src_ptr + cd_a + n_cd);
+        for (int e = threadIdx.x; e < q1 - q0; e += STG_THREADS) {
+            srcc[e] = __ldg(st.src_c + q0 + e);
+            srco[e] = (__ldg(st.src_cupos + q0 + e) - cu_a) * GROUP;
+        }
+        if (threadIdx.x <= n_cd) srcp[threadIdx.x] = __ldg(st.src_ptr + cd_a + threadIdx.x) - q0;
+        if (threadIdx.x >= 32 && threadIdx.x < 32 + n_cu) cuoff[threadIdx.x - 32] = __ldg(st.cu_list + cu_a + threadIdx.x - 32) * S_b;
+        cp_async_wait_all();
+        __syncthreads();
+#define WICK_STG_CALL(NCU) staged_rows_ncd<NCU>(MUs, MDl, row, warp, n_rows, n_cu, n_cd, rowoff, cuoff, sinkp, sinkc, sinko, srcp, srcc, srco)
+        c128 v;
+        if (n_cu <= 1) v = WICK_STG_CALL(1);
+        else if (n_cu <= 2) v = WICK_STG_CALL(2);
+        else if (n_cu <= 4) v = WICK_STG_CALL(4);
+        else if (n_cu <= 8) v = WICK_STG_CALL(8);
+        else v = WICK_STG_CALL(STG_ROW_CAP);
+#undef WICK_STG_CALL
+        acc = cadd(acc, v);
+    }
+    // fixed-order combination of the warps -> partial[bin][site]
+    __syncthreads();
+    MDs[threadIdx.x] = acc;
+    __syncthreads();
+    if (threadIdx.x < GROUP) {
+        c128 t = MDs[threadIdx.x];
+#pragma unroll
+        for (int w = 1; w < STG_W; ++w) t = cadd(t, MDs[w * 32 + threadIdx.x]);
+        partial[int64_t(blockIdx.y) * S_b + int64_t(blockIdx.x) * GROUP + threadIdx.x] = t;
+    }
+}
+
+cudaError_t launch_reduce_staged(const double2* MU, const double2* MD, int n_groups, int S_b, const StagedTables& st,
+                                 double2* partial, int* n_chunks_out, cudaStream_t stream) {
+    dim3 grid(n_groups, st.n_bins);
+    ProfScope prof(PROF_REDUCE, stream);
+    reduce_staged_kernel<<<grid, STG_THREADS, STG_SMEM, stream>>>(MU, MD, S_b, st, partial);
+    ++g_launches;
+    *n_chunks_out = st.n_bins;
+    return cudaGetLastError();
 }
 
 cudaError_t launch_reduce_flat(const double2* MU, const double2* MD, int n_groups, int S_b,
@@ -676,6 +845,20 @@ cudaError_t measure_fp64_peak(double* tflops, cudaStream_t stream) {
     cudaFree(d);
     *tflops = best;
     return e;
+}
+
+template <int N> static cudaError_t set_smem_attr() {
+    return cudaFuncSetAttribute(minors_kernel<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(MinorCfg<N>::kSmem));
+}
+
+cudaError_t configure_kernels() {
+    cudaError_t e;
+    if ((e = cudaFuncSetAttribute(reduce_staged_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, int(STG_SMEM))) != cudaSuccess) return e;
+#define WICK_ATTR(N) if ((e = set_smem_attr<N>()) != cudaSuccess) return e;
+    WICK_ATTR(0) WICK_ATTR(1) WICK_ATTR(2) WICK_ATTR(3) WICK_ATTR(4) WICK_ATTR(5) WICK_ATTR(6)
+    WICK_ATTR(7) WICK_ATTR(8) WICK_ATTR(9) WICK_ATTR(10) WICK_ATTR(11) WICK_ATTR(12)
+#undef WICK_ATTR
+    return cudaSuccess;
 }
 
 }  // namespace wick

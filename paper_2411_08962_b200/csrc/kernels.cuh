@@ -43,6 +43,28 @@ struct OuterTables {
 };
 cudaError_t launch_reduce_outer(const double2* MU, const double2* MD, int n_groups, int S_b, const OuterTables& ot,
                                 double2* partial, int* n_chunks_out, cudaStream_t stream);
+// Staged factorised reduction (reduce_staged_kernel): a CTA walks batches = (one source block's d-column
+// range) x (a run of sink blocks); the MD elements of a batch sit in shared memory once, every warp
+// streams its u-row tuples' MU rows through a private buffer.  All lists hold positions in the
+// block-grouped tuple lists ru_list / rd_list / cu_list / cd_list.
+constexpr int STG_THREADS = 192;          // 6 warps, two CTAs per SM (one loads while the other computes)
+constexpr int STG_CTAS_PER_SM = 2;
+constexpr int STG_MD_CAP = 96;            // MD elements (512 B each) of a batch
+constexpr int STG_ROW_CAP = 15;           // MU elements of one (u-row tuple, source block) row
+constexpr int STG_NCD_CAP = 8;            // d columns of a batch piece
+constexpr int STG_SINK_CAP = 512;         // sink entries of a batch's u-row tuples
+constexpr int STG_SRC_CAP = 256;          // source entries of a batch piece's d columns
+constexpr int STG_ROWS_CAP = STG_MD_CAP;  // u-row tuples of a batch
+struct StagedBatch { int32_t cd_a, cd_b, cu_a, cu_b, rd_a, rd_b, ru_a, ru_b; };
+struct StagedTables {
+    int n_cols_u, n_cols_d, n_bins;
+    const int32_t *sink_ptr, *sink_rdpos; const double2* sink_c;   // CSR over POSITION in ru_list: (position of rd in rd_list, c_i)
+    const int32_t *src_ptr, *src_cupos; const double2* src_c;      // CSR over POSITION in cd_list: (position of cu in cu_list, conj c_j)
+    const int32_t *ru_list, *rd_list, *cu_list, *cd_list;
+    const int32_t* bin_ptr; const StagedBatch* batches;            // per CTA bin: its batches, fixed order
+};
+cudaError_t launch_reduce_staged(const double2* MU, const double2* MD, int n_groups, int S_b, const StagedTables& st,
+                                 double2* partial, int* n_chunks_out, cudaStream_t stream);
 cudaError_t launch_finalize_sigma(const double2* partial, int n_chunks, int S_b, int64_t n_valid,
                                   double2* sigma_batch, cudaStream_t stream);
 cudaError_t launch_project(const double2* sigma, int L, int T, const MomentumList& mom, double2* C_out,

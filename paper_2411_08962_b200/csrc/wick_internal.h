@@ -3,6 +3,7 @@
 // builder compiles as plain C++.
 #pragma once
 #include <complex>
+#include <map>
 #include <cstdint>
 #include <mutex>
 #include <string>
@@ -23,6 +24,17 @@ struct FlavourTables {
 
 // Factor of an outer-product list.  Sink: (row-tuple ids, c_i).  Source: (column-tuple ids, conj c_j).
 struct FactorTerm { int32_t qu, qd; cplx c; };
+
+// Schedule of the staged factorised reduction for one CTA-bin count (contract.cu: ensure_staged)
+struct StagedDev {
+    void* blob = nullptr;
+    int n_bins = 0;
+    const int32_t *sink_ptr = nullptr, *sink_rdpos = nullptr, *src_ptr = nullptr, *src_cupos = nullptr;   // CSR by list position
+    const double *sink_c = nullptr, *src_c = nullptr;
+    const int32_t *ru_list = nullptr, *rd_list = nullptr, *cu_list = nullptr, *cd_list = nullptr;
+    const int32_t* bin_ptr = nullptr;
+    const void* batches = nullptr;
+};
 
 // Device-resident copies, created by the first device call that needs them (contract.cu).
 struct DeviceTables {
@@ -46,6 +58,8 @@ struct DeviceTables {
     const int32_t* red_bin_ptr = nullptr;       // [n_red_bins + 1]
     const int32_t* red_items = nullptr;         // [n_items][2]  (sink component, source component)
     int n_red_bins = 0;
+    int staged_state = 0;                       // 0 = not checked, 1 = eligible, -1 = blocks too large for the staged kernel
+    std::map<int, StagedDev> staged;            // by number of CTA bins
     // flat list (uploaded only when the flat path runs)
     void* flat_blob = nullptr;
     const int32_t* t_uid = nullptr;
