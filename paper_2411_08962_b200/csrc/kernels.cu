@@ -188,6 +188,7 @@ struct LuState {
     double Lr[N][KR], Li[N][KR];       // register multipliers: column i >= R at [r][i - R], r > i
     c128 detp;                         // (+-) product of the K pivots
     c128 s[6];                         // 2x2 minors of trailing columns (K, K+1), row pairs 01 02 03 12 13 23
+    c128 c3[4];                        // signed 3x3 minors of trailing columns (K, K+1, K+2)
 
     // c[r] -= L[r][i] c[i] for r > i: the elimination of column i applied to the active column
     template <int I>
@@ -280,40 +281,44 @@ struct LuState {
         for (int r = 0; r < N; ++r) rb[r] = rb0[r];
         pivot_steps<0>(tb, Ls, cb);
     }
-    // two trailing columns: apply the K eliminations, keep the last 4 entries, return their six 2x2 minors
-    __device__ __forceinline__ void column_pair(const unsigned char* tb, const c128* Ls, uint32_t cba, uint32_t cbb, c128 (&d2)[6]) const {
-        double tr[2][4], ti[2][4];
+    // one trailing column: apply the K eliminations, keep the last 4 entries (the column of the Schur complement)
+    __device__ __forceinline__ void schur_column(const unsigned char* tb, const c128* Ls, uint32_t cbj, c128 (&t)[4]) const {
+        double cr[N], ci[N];
+        load_column(tb, cbj, cr, ci);
+        apply_columns_below<0, K>(Ls, cr, ci);
 #pragma unroll
-        for (int q = 0; q < 2; ++q) {
-            double cr[N], ci[N];
-            load_column(tb, q == 0 ? cba : cbb, cr, ci);
-            apply_columns_below<0, K>(Ls, cr, ci);
-#pragma unroll
-            for (int r = 0; r < 4; ++r) { tr[q][r] = cr[K + r]; ti[q][r] = ci[K + r]; }
-        }
+        for (int r = 0; r < 4; ++r) t[r] = make_double2(cr[K + r], ci[K + r]);
+    }
+    // level 1: columns K, K+1 of the minor -> s = 2x2 minors of Schur columns 0, 1 over the row pairs
+    __device__ __forceinline__ void first_pair(const unsigned char* tb, const c128* Ls, uint32_t cba, uint32_t cbb) {
+        c128 t0[4], t1[4];
+        schur_column(tb, Ls, cba, t0);
+        schur_column(tb, Ls, cbb, t1);
         int k = 0;
 #pragma unroll
         for (int a = 0; a < 4; ++a)
 #pragma unroll
-            for (int b = a + 1; b < 4; ++b)
-                d2[k++] = det2(make_double2(tr[0][a], ti[0][a]), make_double2(tr[1][a], ti[1][a]),
-                               make_double2(tr[0][b], ti[0][b]), make_double2(tr[1][b], ti[1][b]));
+            for (int b = a + 1; b < 4; ++b) s[k++] = det2(t0[a], t1[a], t0[b], t1[b]);
     }
-    __device__ __forceinline__ void first_pair(const unsigned char* tb, const c128* Ls, uint32_t cba, uint32_t cbb) {
-        column_pair(tb, Ls, cba, cbb, s);
+    // level 2: column K+2 -> signed 3x3 minors of Schur columns 0..2: c3[r] = (-1)^(r+3) det(rows != r),
+    // each expanded along its last column in the 2x2 minors s
+    __device__ __forceinline__ void third_column(const unsigned char* tb, const c128* Ls, uint32_t cbj) {
+        c128 t[4];
+        schur_column(tb, Ls, cbj, t);
+        const c128 m0 = cfma(t[3], s[3], cfnma(t[2], s[4], cmul(t[1], s[5])));   // rows 1,2,3
+        const c128 m1 = cfma(t[3], s[1], cfnma(t[2], s[2], cmul(t[0], s[5])));   // rows 0,2,3
+        const c128 m2 = cfma(t[3], s[0], cfnma(t[1], s[2], cmul(t[0], s[4])));   // rows 0,1,3
+        const c128 m3 = cfma(t[2], s[0], cfnma(t[1], s[1], cmul(t[0], s[3])));   // rows 0,1,2
+        c3[0] = make_double2(-m0.x, -m0.y); c3[1] = m1; c3[2] = make_double2(-m2.x, -m2.y); c3[3] = m3;
     }
-    // Laplace expansion of the 4x4 Schur complement along its column pairs (01 | 23):
-    // pairs in order (01,02,03,12,13,23); the complement of pair q is pair 5-q; signs + - + + - +
-    __device__ __forceinline__ c128 finish(const unsigned char* tb, const c128* Ls, uint32_t cba, uint32_t cbb) const {
-        c128 d2[6];
-        column_pair(tb, Ls, cba, cbb, d2);
-        c128 d = cmul(s[0], d2[5]);
-        d = cfnma(s[1], d2[4], d);
-        d = cfma(s[2], d2[3], d);
-        d = cfma(s[3], d2[2], d);
-        d = cfnma(s[4], d2[1], d);
-        d = cfma(s[5], d2[0], d);
-        return cmul(detp, d);
+    // level 3: last column -> det = detp * sum_r S[r][3] c3[r]  (Laplace expansion of the 4x4 Schur
+    // complement along its last column); two independent partial sums keep the dependency chain short
+    __device__ __forceinline__ c128 finish(const unsigned char* tb, const c128* Ls, uint32_t cbj) const {
+        c128 t[4];
+        schur_column(tb, Ls, cbj, t);
+        const c128 e0 = cfma(t[1], c3[1], cmul(t[0], c3[0]));
+        const c128 e1 = cfma(t[3], c3[3], cmul(t[2], c3[2]));
+        return cmul(detp, cadd(e0, e1));
     }
 };
 
@@ -386,7 +391,8 @@ minors_kernel(const c128* __restrict__ P, int64_t st0, int64_t n_st_total, int S
     } else {
         constexpr int K = N - 4;
         constexpr uint32_t kRowStep = 12 * GROUP * 16, kColStep = GROUP * 16;
-        constexpr unsigned long long kLead = (1ull << (4 * K)) - 1, kLeadPair = (1ull << (4 * (K + 2))) - 1;
+        constexpr unsigned long long kLead = (1ull << (4 * K)) - 1, kLeadPair = (1ull << (4 * (K + 2))) - 1,
+                                     kLead3 = (1ull << (4 * (K + 3))) - 1;
         const unsigned char* tb = reinterpret_cast<const unsigned char*>(tl);
         c128* Ls = tile + TILE_ELEMS + threadIdx.x;
         LuState<N, MinorCfg<N>::kSmemCols, NT> lu;
@@ -402,8 +408,10 @@ minors_kernel(const c128* __restrict__ P, int64_t st0, int64_t n_st_total, int S
                 for (int i = 0; i < N; ++i) { rb[i] = dc.row(i) * kRowStep; cb[i] = dc.col(i) * kColStep; }
                 lu.start(tb, Ls, rb, cb);
             }
-            if (fresh || (diff & kLeadPair) != 0) lu.first_pair(tb, Ls, dc.col(K) * kColStep, dc.col(K + 1) * kColStep);
-            const c128 det = lu.finish(tb, Ls, dc.col(K + 2) * kColStep, dc.col(K + 3) * kColStep);
+            const bool new_pair = fresh || (diff & kLeadPair) != 0;
+            if (new_pair) lu.first_pair(tb, Ls, dc.col(K) * kColStep, dc.col(K + 1) * kColStep);
+            if (new_pair || (diff & kLead3) != 0) lu.third_column(tb, Ls, dc.col(K + 2) * kColStep);
+            const c128 det = lu.finish(tb, Ls, dc.col(K + 3) * kColStep);
             prow = rws; pcol = dc.cols_bits();
             if (valid) outp[int64_t(m) * S_b] = det;
         }
