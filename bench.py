@@ -43,6 +43,29 @@ def flops_lu(n: int) -> float:
         return 220.0
     return 8.0 * (n - 1) * n * (2 * n - 1) / 6 + 6.0 * n * (n - 1) / 2 + 15.0 * (n - 1) + 3.0 * (n * (n + 1) / 2 - 1)
 
+def executed_flops_per_site(n: int, rows: np.ndarray, cols: np.ndarray, minor_row: np.ndarray, minor_col: np.ndarray) -> float:
+    """Flops the minors kernel actually executes per site for one flavour: the pivoted-LU
+    state is kept across consecutive minors that share the row tuple and leading columns, so the K = n-4
+    pivot steps run once per (row tuple, first K columns), the 2x2 / 3x3 minors of the Schur complement
+    once per (.., first K+2 / K+3 columns), and only the last column once per minor."""
+    nm = len(minor_row)
+    if n <= 4 or nm == 0:
+        return nm * flops_lu(n)
+    K = n - 4
+    f_col = 8.0 * sum(n - 1 - i for i in range(K))
+    f_start = sum(8.0 * sum(n - 1 - i for i in range(J)) + (n - J) + 14.0 + 6.0 * (n - 1 - J) + (6.0 if J else 0.0)
+                  for J in range(K))
+    f_pair, f_third, f_finish = 2 * f_col + 84.0, f_col + 88.0, f_col + 36.0
+    c = cols[minor_col]                                            # [nm][n] column tuples in minor order
+    same_row = minor_row[1:] == minor_row[:-1]
+    def same_lead(k):
+        return same_row & np.all(c[1:, :k] == c[:-1, :k], axis=1)
+    n_fresh = 1 + int(np.count_nonzero(~same_lead(K)))
+    n_pair = 1 + int(np.count_nonzero(~same_lead(K + 2)))
+    n_third = 1 + int(np.count_nonzero(~same_lead(K + 3)))
+    return n_fresh * f_start + n_pair * f_pair + n_third * f_third + nm * f_finish
+
+
 FLOPS_PER_TERM = 14.0
 FP64_PEAK_DERIVED_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12     # 148 SMs x 64 DFMA lanes x 2 flop x 1.965 GHz = 37.2
 
@@ -260,6 +283,11 @@ def main():
     ms_project = prof["project"][0] / args.steps
     n_minor_launches = (prof["minors_u"][1] + prof["minors_d"][1]) // args.steps
     achieved_tf = flop_minors / (ms_minors * 1e-3) / 1e12
+    tu_rows, tu_cols, td_rows, td_cols = terms.tuples()
+    mu_row, mu_col, md_row, md_col = terms.minors()
+    exec_site = (executed_flops_per_site(info.n_u, tu_rows, tu_cols, mu_row, mu_col),
+                 executed_flops_per_site(info.n_d, td_rows, td_cols, md_row, md_col))
+    executed_tf = st_per_step * sum(exec_site) / (ms_minors * 1e-3) / 1e12
     traffic = None
     try:
         with open(os.path.join(ROOT, "profiles", "roofline_traffic.json")) as f:
@@ -271,6 +299,10 @@ def main():
         "achieved": achieved_tf, "peak": FP64_PEAK_DERIVED_TFLOPS, "unit": "TFLOP/s",
         "frac": achieved_tf / FP64_PEAK_DERIVED_TFLOPS,
         "peak_source": "derived: 148 SMs x 64 FP64 lanes x 2 flop x 1.965 GHz (MEASURED_PEAKS.json has no FP64 entry)",
+        "executed": {"tflops": executed_tf, "frac": executed_tf / FP64_PEAK_DERIVED_TFLOPS,
+                     "flops_per_minor": {"u": exec_site[0] / max(info.n_minors_u, 1), "d": exec_site[1] / max(info.n_minors_d, 1)},
+                     "note": "flops the kernel issues: LU state shared by minors with equal row tuple and leading columns "
+                             "(DESIGN.md 6b); `achieved`/`frac` count one full LU per unique minor (SURVEY 8d) and can exceed 1"},
         "peak_measured_dfma_probe": fp64_probe, "frac_of_dfma_probe": achieved_tf / fp64_probe if fp64_probe else None,
         "traffic": traffic, "launches_per_step": int(n_minor_launches),
         "avg_launch_ms": ms_minors / max(n_minor_launches, 1),

@@ -270,7 +270,16 @@ int ensure_staged(const wick_terms* t, int n_bins, cudaStream_t stream, StagedTa
     if (hit != d.staged.end()) { fill(hit->second); return 1; }
 
     const Components cs = factor_components(nru, nrd, t->sink);
-    const Components cq = factor_components(ncu, ncd, t->source);
+    Components cq = factor_components(ncu, ncd, t->source);
+    {   // source blocks relabelled by decreasing number of d columns, so that small blocks are neighbours and can share a piece
+        std::vector<int> n_cd_of(size_t(cq.n), 0), order(size_t(cq.n)), relabel(size_t(cq.n));
+        for (int c : cq.of_d) if (c >= 0) n_cd_of[size_t(c)]++;
+        for (int k = 0; k < cq.n; ++k) order[size_t(k)] = k;
+        std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return n_cd_of[size_t(a)] > n_cd_of[size_t(b)]; });
+        for (int k = 0; k < cq.n; ++k) relabel[size_t(order[size_t(k)])] = k;
+        for (int& c : cq.of_u) if (c >= 0) c = relabel[size_t(c)];
+        for (int& c : cq.of_d) if (c >= 0) c = relabel[size_t(c)];
+    }
     auto group = [](const std::vector<int>& comp_of, int n_comp, std::vector<int32_t>& ptr, std::vector<int32_t>& list, std::vector<int32_t>& pos) {
         ptr.assign(size_t(n_comp) + 1, 0);
         for (int c : comp_of) if (c >= 0) ptr[size_t(c) + 1]++;
@@ -325,16 +334,35 @@ int ensure_staged(const wick_terms* t, int n_bins, cudaStream_t stream, StagedTa
 
     struct Item { int64_t cost; StagedBatch b; };
     std::vector<Item> items;
-    for (int kp = 0; kp < cq.n; ++kp) {
+    // pieces of the d-column list: a large source block is cut into equal pieces small enough for the largest
+    // sink block; neighbouring small blocks share a piece (their union is just a block-diagonal source block)
+    struct Piece { int ca, cb, cuA, cuB; };
+    std::vector<Piece> pieces;
+    const int piece_max = std::max(1, std::min(STG_NCD_CAP, STG_MD_CAP / max_rd));
+    for (int kp = 0; kp < cq.n;) {
         const int cdA = cd_ptr[size_t(kp)], cdB = cd_ptr[size_t(kp) + 1];
-        const int cuA = cu_ptr[size_t(kp)], cuB = cu_ptr[size_t(kp) + 1];
-        // equal pieces of the block's d columns, each small enough for the largest sink block
-        const int piece_max = std::max(1, std::min(std::min(cdB - cdA, STG_NCD_CAP), STG_MD_CAP / max_rd));
-        const int n_pieces = (cdB - cdA + piece_max - 1) / piece_max;
-        const int piece = (cdB - cdA + n_pieces - 1) / n_pieces;
-        for (int ca = cdA; ca < cdB;) {
-            int cb = std::min(cdB, ca + piece);
-            while (cb > ca + 1 && src_ptr[size_t(cb)] - src_ptr[size_t(ca)] > STG_SRC_CAP) --cb;   // source entries of the piece
+        const int cuA = cu_ptr[size_t(kp)];
+        if (cdB - cdA >= piece_max) {
+            const int n_pieces = (cdB - cdA + piece_max - 1) / piece_max;
+            const int piece = (cdB - cdA + n_pieces - 1) / n_pieces;
+            for (int ca = cdA; ca < cdB;) {
+                int cb = std::min(cdB, ca + piece);
+                while (cb > ca + 1 && src_ptr[size_t(cb)] - src_ptr[size_t(ca)] > STG_SRC_CAP) --cb;
+                pieces.push_back({ca, cb, cuA, cu_ptr[size_t(kp) + 1]});
+                ca = cb;
+            }
+            ++kp;
+        } else {
+            int ke = kp + 1;
+            while (ke < cq.n && cd_ptr[size_t(ke) + 1] - cdA <= piece_max && cu_ptr[size_t(ke) + 1] - cuA <= STG_ROW_CAP &&
+                   src_ptr[size_t(cd_ptr[size_t(ke) + 1])] - src_ptr[size_t(cdA)] <= STG_SRC_CAP) ++ke;
+            pieces.push_back({cdA, cd_ptr[size_t(ke)], cuA, cu_ptr[size_t(ke)]});
+            kp = ke;
+        }
+    }
+    for (const Piece& pc : pieces) {
+        {
+            const int ca = pc.ca, cb = pc.cb, cuA = pc.cuA, cuB = pc.cuB;
             const int n_cd = cb - ca;
             const int64_t src_work = (src_ptr[size_t(cb)] - src_ptr[size_t(ca)]) + n_cd;
             int ka = 0;
@@ -356,7 +384,6 @@ int ensure_staged(const wick_terms* t, int n_bins, cudaStream_t stream, StagedTa
                 items.push_back(it);
                 ka = kb;
             }
-            ca = cb;
         }
     }
     std::stable_sort(items.begin(), items.end(), [](const Item& a, const Item& b) { return a.cost > b.cost; });
