@@ -49,15 +49,18 @@ def executed_flops_per_site(n: int, rows: np.ndarray, cols: np.ndarray, minor_ro
     pivot steps run once per (row tuple, first K columns), the 2x2 / 3x3 minors of the Schur complement
     once per (.., first K+2 / K+3 columns), and only the last column once per minor."""
     nm = len(minor_row)
-    if n <= 4 or nm == 0:
+    if n <= 2 or nm == 0:
         return nm * flops_lu(n)
+    c = cols[minor_col]                                            # [nm][n] column tuples in minor order
+    same_row = minor_row[1:] == minor_row[:-1]
+    if n == 3:                                                     # cofactors of the last column per (rows, b0, b1)
+        n_pair = 1 + int(np.count_nonzero(~(same_row & np.all(c[1:, :2] == c[:-1, :2], axis=1))))
+        return n_pair * 42.0 + nm * 22.0
     K = n - 4
     f_col = 8.0 * sum(n - 1 - i for i in range(K))
     f_start = sum(8.0 * sum(n - 1 - i for i in range(J)) + (n - J) + 14.0 + 6.0 * (n - 1 - J) + (6.0 if J else 0.0)
                   for J in range(K))
     f_pair, f_third, f_finish = 2 * f_col + 84.0, f_col + 88.0, f_col + 36.0
-    c = cols[minor_col]                                            # [nm][n] column tuples in minor order
-    same_row = minor_row[1:] == minor_row[:-1]
     def same_lead(k):
         return same_row & np.all(c[1:, :k] == c[:-1, :k], axis=1)
     n_fresh = 1 + int(np.count_nonzero(~same_lead(K)))

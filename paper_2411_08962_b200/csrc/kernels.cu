@@ -1,8 +1,9 @@
 // Device kernels of the hot path, sm_100a.  See kernels.cuh for the on-chip layout.
 //
 //  a3  stage_tile          : propagators of 32 site-times -> shared memory, element-major / lane-minor
-//  a4  minors_kernel<N>    : one unique minor per (warp iteration, lane = site).  N <= 4: analytic
-//                            expression; N >= 5: LU with partial pivoting.  The LU is
+//  a4  minors_kernel<N>    : one unique minor per (warp iteration, lane = site).  N <= 3: analytic
+//                            expression; N >= 4: N-4 steps of LU with partial pivoting, then the analytic 4x4
+//                            expression of the Schur complement.  The LU is
 //                            LEFT-LOOKING: column j of the minor is gathered from shared memory only
 //                            after the pivots of columns < j are known, in the lane's current row
 //                            order, so the only data that ever has to be exchanged in registers is
@@ -162,7 +163,7 @@ __device__ __forceinline__ int pivot_key(double re, double im) { return __double
 // number of multipliers in the first i columns of L (column c holds rows c+1 .. N-1)
 template <int N> __host__ __device__ constexpr int lcol_base(int i) { return i * (N - 1) - i * (i - 1) / 2; }
 
-// Hybrid elimination (N >= 5): K = N-4 steps of LEFT-LOOKING LU with partial pivoting, then the closed
+// Hybrid elimination (N >= 4): K = N-4 steps of LEFT-LOOKING LU with partial pivoting, then the closed
 // form of the 4x4 Schur complement ("up to 4x4 analytic, LU above", applied to the
 // trailing block as well).  det = (+-) piv_0 ... piv_{K-1} det4(S).  Left-looking: column j of the minor
 // is gathered from shared memory only after the pivots of columns < j are known, in the lane's current
@@ -279,6 +280,7 @@ struct LuState {
     __device__ __forceinline__ void start(const unsigned char* tb, c128* Ls, const uint32_t (&rb0)[N], const uint32_t (&cb)[N]) {
 #pragma unroll
         for (int r = 0; r < N; ++r) rb[r] = rb0[r];
+        detp = make_double2(1.0, 0.0);                          // N = 4: no pivot step, the minor is its own Schur complement
         pivot_steps<0>(tb, Ls, cb);
     }
     // one trailing column: apply the K eliminations, keep the last 4 entries (the column of the Schur complement)
@@ -366,11 +368,11 @@ minors_kernel(const c128* __restrict__ P, int64_t st0, int64_t n_st_total, int S
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int m_begin = blockIdx.y * chunk;
     const int m_end = min(n_minors, m_begin + chunk);
-    // N <= 4: warp w takes minors m_begin + w, + NT/32, ...; N >= 5: a contiguous piece of the chunk, so
+    // N <= 2: warp w takes minors m_begin + w, + NT/32, ...; N >= 3: a contiguous piece of the chunk, so
     // that consecutive minors share their row tuple and leading columns (see LuState)
-    constexpr int kStride = (N <= 4) ? NT / 32 : 1;
-    int m = (N <= 4) ? m_begin + warp : m_begin + warp * (chunk / (NT / 32));
-    const int m_stop = (N <= 4) ? m_end : min(m_end, m + chunk / (NT / 32));
+    constexpr int kStride = (N <= 2) ? NT / 32 : 1;
+    int m = (N <= 2) ? m_begin + warp : m_begin + warp * (chunk / (NT / 32));
+    const int m_stop = (N <= 2) ? m_end : min(m_end, m + chunk / (NT / 32));
     Desc<N> dn;                                                // descriptor of the next minor, fetched one iteration ahead
     if (m < m_stop) dn = Desc<N>::load(desc, m);
     stage_tile(tile, P, st_first, n_st_total, NT);
@@ -378,7 +380,32 @@ minors_kernel(const c128* __restrict__ P, int64_t st0, int64_t n_st_total, int S
     const c128* tl = tile + lane;
     const bool valid = st_first + lane < n_st_total;
     c128* outp = out + int64_t(g) * GROUP + lane;
-    if constexpr (N <= 4) {
+    if constexpr (N == 3) {
+        // 3x3: the cofactors of the last column depend on (row tuple, first two columns) only and are kept
+        // across consecutive minors; per minor 3 loads and 3 complex multiply-adds
+        c128 cof[3];
+        unsigned long long prow = ~0ull, pcol = 0;
+        for (; m < m_stop; ++m) {
+            const Desc<N> dc = dn;
+            if (m + 1 < m_stop) dn = Desc<N>::load(desc, m + 1);
+            const unsigned long long rws = dc.rows_bits(), cls = dc.cols_bits();
+            int re[3];
+#pragma unroll
+            for (int i = 0; i < 3; ++i) re[i] = int(dc.row(i)) * 12;
+            if (rws != prow || ((cls ^ pcol) & 0xffull) != 0) {
+                const int c0 = int(dc.col(0)), c1 = int(dc.col(1));
+                const c128 a0 = ld(tl, re[0], c0), a1 = ld(tl, re[1], c0), a2 = ld(tl, re[2], c0);
+                const c128 b0 = ld(tl, re[0], c1), b1 = ld(tl, re[1], c1), b2 = ld(tl, re[2], c1);
+                cof[0] = det2(a1, b1, a2, b2);                   // rows 1,2
+                cof[1] = det2(a2, b2, a0, b0);                   // -(rows 0,2)
+                cof[2] = det2(a0, b0, a1, b1);                   // rows 0,1
+            }
+            const int c2 = int(dc.col(2));
+            const c128 det = cfma(ld(tl, re[2], c2), cof[2], cfma(ld(tl, re[1], c2), cof[1], cmul(ld(tl, re[0], c2), cof[0])));
+            prow = rws; pcol = cls;
+            if (valid) outp[int64_t(m) * S_b] = det;
+        }
+    } else if constexpr (N <= 2) {
         for (; m < m_stop; m += kStride) {
             const Desc<N> dc = dn;
             if (m + kStride < m_stop) dn = Desc<N>::load(desc, m + kStride);
