@@ -47,6 +47,7 @@ extern "C" {
                                      /* test then evaluates both flavours on the SAME random matrix          */
 /* wick_contract flags */
 #define WICK_CONTRACT_FORCE_FLAT 1u  /* use the flat (uid, did, w) term list even if a factorised form exists */
+#define WICK_CONTRACT_COMPLEX_COEFFS 4u /* staged reduction: do not use the cheaper entries for all-real factor coefficients */
 #define WICK_CONTRACT_NO_STAGED  2u  /* factorised lists: walk the block items from L1/L2 instead of staging them in shared memory */
 
 #define WICK_NUCLEON_PROTON  0

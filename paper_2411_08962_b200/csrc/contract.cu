@@ -261,6 +261,9 @@ int ensure_staged(const wick_terms* t, int n_bins, cudaStream_t stream, StagedTa
     const int ncu = int(t->f[0].cols.size()), ncd = int(t->f[1].cols.size());
     auto fill = [&](const StagedDev& sd) {
         out->n_cols_u = ncu; out->n_cols_d = ncd; out->n_bins = sd.n_bins;
+        out->real_coeffs = true;
+        for (const FactorTerm& f : t->sink) if (f.c.imag() != 0.0) out->real_coeffs = false;
+        for (const FactorTerm& f : t->source) if (f.c.imag() != 0.0) out->real_coeffs = false;
         out->sink_ptr = sd.sink_ptr; out->sink_rdpos = sd.sink_rdpos; out->sink_c = reinterpret_cast<const double2*>(sd.sink_c);
         out->src_ptr = sd.src_ptr; out->src_cupos = sd.src_cupos; out->src_c = reinterpret_cast<const double2*>(sd.src_c);
         out->ru_list = sd.ru_list; out->rd_list = sd.rd_list; out->cu_list = sd.cu_list; out->cd_list = sd.cd_list;
@@ -576,6 +579,7 @@ extern "C" int wick_contract(const void* U_dev, const void* D_dev, const wick_te
         rc = ensure_staged(t, n_bins, stream, &stg);
         if (rc < 0) return rc;
         have_staged = (rc == 1);
+        if (flags & WICK_CONTRACT_COMPLEX_COEFFS) stg.real_coeffs = false;
     }
     for (int64_t st0 = 0; st0 < p.n_st; st0 += S_b) {
         const int64_t n_valid = std::min<int64_t>(S_b, p.n_st - st0);

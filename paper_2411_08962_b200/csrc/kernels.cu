@@ -592,10 +592,12 @@ constexpr size_t STG_OFF_ROWOFF = STG_OFF_SINKP + size_t(STG_ROWS_CAP + 2) * 4; 
 constexpr size_t STG_OFF_SRCP = STG_OFF_ROWOFF + size_t(STG_ROWS_CAP + 2) * 4;              // int[16] per-cd entry ranges, int[16] u column offsets
 constexpr size_t STG_SMEM = STG_OFF_SRCP + 32 * 4;
 
-// All u-row tuples of a batch that belong to this warp.  NCU / NCD = compile-time bounds on the u columns
-// of the source block and on the d columns of the piece (loops over them are unrolled and predicated).
-template <int NCU, int NCD>
-__device__ __forceinline__ c128 staged_rows(const c128* MUs, const c128* MDl, c128* row, int warp, int n_rows, int n_cu, int n_cd,
+// All u-row tuples of a batch that belong to this warp.  NCU = compile-time bound on the u columns of the
+// piece (loads / stores of the row are unrolled and predicated), NCD = its number of d columns (exact).
+// REAL: every coefficient of the factor lists is real (all interpolator products of wick_build_terms): a list
+// entry is one 16-byte record {coefficient, element offset} and a term costs 2 DFMA instead of 4.
+template <int NCU, int NCD, bool REAL>
+__device__ __forceinline__ c128 staged_rows(const c128* MUs, const c128* MDl, c128* row, int warp, int n_rows, int n_cu,
                                             const int* rowoff, const int* cuoff, const int* sinkp, const c128* sinkc,
                                             const int* sinko, const int* srcp, const c128* srcc, const int* srco) {
     c128 acc = make_double2(0.0, 0.0);
@@ -625,40 +627,54 @@ __device__ __forceinline__ c128 staged_rows(const c128* MUs, const c128* MDl, c1
 #pragma unroll
         for (int c = 0; c < NCD; ++c) P[c] = make_double2(0.0, 0.0);
         const int i0 = sinkp[r], i1 = sinkp[r + 1];
+#pragma unroll 2
         for (int i = i0; i < i1; ++i) {
             const c128 a = sinkc[i];
-            const c128* md = MDl + sinko[i];                     // element (rd_i, first cd of the piece), this lane
+            const c128* md = MDl + (REAL ? __double2loint(a.y) : sinko[i]);   // element (rd_i, first cd of the piece), this lane
 #pragma unroll
-            for (int c = 0; c < NCD; ++c)
-                if (c < n_cd) P[c] = cfma(a, md[c * GROUP], P[c]);
+            for (int c = 0; c < NCD; ++c) {
+                const c128 v = md[c * GROUP];
+                if (REAL) { P[c].x = fma(a.x, v.x, P[c].x); P[c].y = fma(a.x, v.y, P[c].y); }
+                else P[c] = cfma(a, v, P[c]);
+            }
         }
         // acc += sum_cd P[cd] * sum_j cbar_j MU[ru, cu_j]
 #pragma unroll
         for (int c = 0; c < NCD; ++c) {
-            if (c < n_cd) {
-                const int j0 = srcp[c], j1 = srcp[c + 1];
-                c128 q = make_double2(0.0, 0.0);
-                for (int j = j0; j < j1; ++j) q = cfma(srcc[j], row[srco[j]], q);
-                acc = cfma(q, P[c], acc);
+            const int j0 = srcp[c], j1 = srcp[c + 1];
+            c128 q = make_double2(0.0, 0.0);
+#pragma unroll 2
+            for (int j = j0; j < j1; ++j) {
+                const c128 b = srcc[j];
+                const c128 x = row[REAL ? __double2loint(b.y) : srco[j]];
+                if (REAL) { q.x = fma(b.x, x.x, q.x); q.y = fma(b.x, x.y, q.y); }
+                else q = cfma(b, x, q);
             }
+            acc = cfma(q, P[c], acc);
         }
         __syncwarp();                                                    // all lanes have read the row buffer
     }
     return acc;
 }
 
-template <int NCU>
+template <int NCU, bool REAL>
 __device__ __forceinline__ c128 staged_rows_ncd(const c128* MUs, const c128* MDl, c128* row, int warp, int n_rows, int n_cu, int n_cd,
                                                 const int* rowoff, const int* cuoff, const int* sinkp, const c128* sinkc,
                                                 const int* sinko, const int* srcp, const c128* srcc, const int* srco) {
-#define WICK_STG_CALL(NCD) staged_rows<NCU, NCD>(MUs, MDl, row, warp, n_rows, n_cu, n_cd, rowoff, cuoff, sinkp, sinkc, sinko, srcp, srcc, srco)
-    if (n_cd <= 1) return WICK_STG_CALL(1);
-    if (n_cd <= 2) return WICK_STG_CALL(2);
-    if (n_cd <= 4) return WICK_STG_CALL(4);
-    return WICK_STG_CALL(STG_NCD_CAP);
+#define WICK_STG_CALL(NCD) staged_rows<NCU, NCD, REAL>(MUs, MDl, row, warp, n_rows, n_cu, rowoff, cuoff, sinkp, sinkc, sinko, srcp, srcc, srco)
+    static_assert(STG_NCD_CAP == 6, "one case per d-column count");
+    switch (n_cd) {
+        case 1: return WICK_STG_CALL(1);
+        case 2: return WICK_STG_CALL(2);
+        case 3: return WICK_STG_CALL(3);
+        case 4: return WICK_STG_CALL(4);
+        case 5: return WICK_STG_CALL(5);
+        default: return WICK_STG_CALL(6);
+    }
 #undef WICK_STG_CALL
 }
 
+template <bool REAL>
 __global__ void __launch_bounds__(STG_THREADS, STG_CTAS_PER_SM)
 reduce_staged_kernel(const c128* __restrict__ MU, const c128* __restrict__ MD, int S_b, StagedTables st,
                      c128* __restrict__ partial) {
@@ -694,8 +710,10 @@ reduce_staged_kernel(const c128* __restrict__ MU, const c128* __restrict__ MD, i
         // coefficient lists of the batch -> shared memory, offsets already in elements of the staged buffers
         const int sp0 = __ldg(st.sink_ptr + ru_a), sp1 = __ldg(st.sink_ptr + ru_a + n_rows);
         for (int e = threadIdx.x; e < sp1 - sp0; e += STG_THREADS) {
-            sinkc[e] = __ldg(st.sink_c + sp0 + e);
-            sinko[e] = (__ldg(st.sink_rdpos + sp0 + e) - rd_a) * n_cd * GROUP;
+            const c128 cf = __ldg(st.sink_c + sp0 + e);
+            const int off = (__ldg(st.sink_rdpos + sp0 + e) - rd_a) * n_cd * GROUP;
+            sinkc[e] = REAL ? make_double2(cf.x, __hiloint2double(0, off)) : cf;
+            sinko[e] = off;
         }
         for (int r = threadIdx.x; r <= n_rows; r += STG_THREADS) {
             sinkp[r] = __ldg(st.sink_ptr + ru_a + r) - sp0;
@@ -703,17 +721,18 @@ reduce_staged_kernel(const c128* __restrict__ MU, const c128* __restrict__ MD, i
         }
         const int q0 = __ldg(st.src_ptr + cd_a), q1 = __ldg(st.src_ptr + cd_a + n_cd);
         for (int e = threadIdx.x; e < q1 - q0; e += STG_THREADS) {
-            srcc[e] = __ldg(st.src_c + q0 + e);
-            srco[e] = (__ldg(st.src_cupos + q0 + e) - cu_a) * GROUP;
+            const c128 cf = __ldg(st.src_c + q0 + e);
+            const int off = (__ldg(st.src_cupos + q0 + e) - cu_a) * GROUP;
+            srcc[e] = REAL ? make_double2(cf.x, __hiloint2double(0, off)) : cf;
+            srco[e] = off;
         }
         if (threadIdx.x <= n_cd) srcp[threadIdx.x] = __ldg(st.src_ptr + cd_a + threadIdx.x) - q0;
         if (threadIdx.x >= 32 && threadIdx.x < 32 + n_cu) cuoff[threadIdx.x - 32] = __ldg(st.cu_list + cu_a + threadIdx.x - 32) * S_b;
         cp_async_wait_all();
         __syncthreads();
-#define WICK_STG_CALL(NCU) staged_rows_ncd<NCU>(MUs, MDl, row, warp, n_rows, n_cu, n_cd, rowoff, cuoff, sinkp, sinkc, sinko, srcp, srcc, srco)
+#define WICK_STG_CALL(NCU) staged_rows_ncd<NCU, REAL>(MUs, MDl, row, warp, n_rows, n_cu, n_cd, rowoff, cuoff, sinkp, sinkc, sinko, srcp, srcc, srco)
         c128 v;
-        if (n_cu <= 1) v = WICK_STG_CALL(1);
-        else if (n_cu <= 2) v = WICK_STG_CALL(2);
+        if (n_cu <= 2) v = WICK_STG_CALL(2);
         else if (n_cu <= 4) v = WICK_STG_CALL(4);
         else if (n_cu <= 8) v = WICK_STG_CALL(8);
         else v = WICK_STG_CALL(STG_ROW_CAP);
@@ -736,7 +755,8 @@ cudaError_t launch_reduce_staged(const double2* MU, const double2* MD, int n_gro
                                  double2* partial, int* n_chunks_out, cudaStream_t stream) {
     dim3 grid(n_groups, st.n_bins);
     ProfScope prof(PROF_REDUCE, stream);
-    reduce_staged_kernel<<<grid, STG_THREADS, STG_SMEM, stream>>>(MU, MD, S_b, st, partial);
+    if (st.real_coeffs) reduce_staged_kernel<true><<<grid, STG_THREADS, STG_SMEM, stream>>>(MU, MD, S_b, st, partial);
+    else reduce_staged_kernel<false><<<grid, STG_THREADS, STG_SMEM, stream>>>(MU, MD, S_b, st, partial);
     ++g_launches;
     *n_chunks_out = st.n_bins;
     return cudaGetLastError();
@@ -888,7 +908,8 @@ template <int N> static cudaError_t set_smem_attr() {
 
 cudaError_t configure_kernels() {
     cudaError_t e;
-    if ((e = cudaFuncSetAttribute(reduce_staged_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, int(STG_SMEM))) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(reduce_staged_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(STG_SMEM))) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(reduce_staged_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(STG_SMEM))) != cudaSuccess) return e;
 #define WICK_ATTR(N) if ((e = set_smem_attr<N>()) != cudaSuccess) return e;
     WICK_ATTR(0) WICK_ATTR(1) WICK_ATTR(2) WICK_ATTR(3) WICK_ATTR(4) WICK_ATTR(5) WICK_ATTR(6)
     WICK_ATTR(7) WICK_ATTR(8) WICK_ATTR(9) WICK_ATTR(10) WICK_ATTR(11) WICK_ATTR(12)

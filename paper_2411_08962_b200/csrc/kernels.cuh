@@ -51,13 +51,14 @@ constexpr int STG_THREADS = 192;          // 6 warps, two CTAs per SM (one loads
 constexpr int STG_CTAS_PER_SM = 2;
 constexpr int STG_MD_CAP = 96;            // MD elements (512 B each) of a batch
 constexpr int STG_ROW_CAP = 15;           // MU elements of one (u-row tuple, source block) row
-constexpr int STG_NCD_CAP = 8;            // d columns of a batch piece
+constexpr int STG_NCD_CAP = 6;            // d columns of a batch piece (one template instance per count)
 constexpr int STG_SINK_CAP = 512;         // sink entries of a batch's u-row tuples
 constexpr int STG_SRC_CAP = 256;          // source entries of a batch piece's d columns
 constexpr int STG_ROWS_CAP = STG_MD_CAP;  // u-row tuples of a batch
 struct StagedBatch { int32_t cd_a, cd_b, cu_a, cu_b, rd_a, rd_b, ru_a, ru_b; };
 struct StagedTables {
     int n_cols_u, n_cols_d, n_bins;
+    bool real_coeffs;                                              // all c_i, cbar_j real: 16-byte {coefficient, offset} entries, 2 DFMA per term
     const int32_t *sink_ptr, *sink_rdpos; const double2* sink_c;   // CSR over POSITION in ru_list: (position of rd in rd_list, c_i)
     const int32_t *src_ptr, *src_cupos; const double2* src_c;      // CSR over POSITION in cd_list: (position of cu in cu_list, conj c_j)
     const int32_t *ru_list, *rd_list, *cu_list, *cd_list;

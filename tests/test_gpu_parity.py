@@ -103,7 +103,7 @@ def _check_C(C_gpu, C_ref, sabs_t):
     assert np.all(err <= REL_TOL * sabs_t[None, :]), (err / sabs_t[None, :]).max()
 
 
-@pytest.mark.parametrize("flags", [0, wk.CONTRACT_FORCE_FLAT, wk.CONTRACT_NO_STAGED])
+@pytest.mark.parametrize("flags", [0, wk.CONTRACT_FORCE_FLAT, wk.CONTRACT_NO_STAGED, wk.CONTRACT_COMPLEX_COEFFS])
 def test_cfg0_proton_full_lattice(flags, cuda_device):
     c = CONFIGS["cfg0"]
     U, D = make_propagators_numpy(c.seed, c.L, c.T)
@@ -141,9 +141,10 @@ def test_shrunken_lattice_full_term_list(cfg, cuda_device):
     Cr, sr, sabs = _oracle_lattice(cfg, U, D, mom, L)
     assert np.all(np.abs(sg - sr) <= REL_TOL * sabs), (np.abs(sg - sr) / sabs).max()
     _check_C(Cg, Cr, sabs.sum(axis=1))
-    if cfg in ("cfg1", "cfg2", "cfg4"):                         # the unstaged factorised kernel on the same list
-        Cn = wk.contract(_dev(U, cuda_device), _dev(D, cuda_device), t, mom, L, T, flags=wk.CONTRACT_NO_STAGED)
-        _check_C(Cn.cpu().numpy(), Cr, sabs.sum(axis=1))
+    if cfg in ("cfg1", "cfg2", "cfg4"):                         # the unstaged factorised kernel / general complex entries
+        for fl in (wk.CONTRACT_NO_STAGED, wk.CONTRACT_COMPLEX_COEFFS):
+            Cn = wk.contract(_dev(U, cuda_device), _dev(D, cuda_device), t, mom, L, T, flags=fl)
+            _check_C(Cn.cpu().numpy(), Cr, sabs.sum(axis=1))
     if cfg in ("cfg1", "cfg4"):                                 # the flat path on the same list
         Cf = wk.contract(_dev(U, cuda_device), _dev(D, cuda_device), t, mom, L, T, flags=wk.CONTRACT_FORCE_FLAT)
         _check_C(Cf.cpu().numpy(), Cr, sabs.sum(axis=1))
