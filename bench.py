@@ -179,6 +179,9 @@ def main():
     ap.add_argument("--cpu-baseline-sites", type=int, default=2)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--isospin", action="store_true",
+                    help="side measurement, not the headline: one propagator for both flavours (the paper's m_u = m_d, "
+                         "PAPER.md:518); flavours with equal unique-minor tables then share one evaluation")
     args = ap.parse_args()
     cfg = CONFIGS[args.workload]
     if args.impl == "reference":
@@ -212,6 +215,8 @@ def main():
     # weak scaling: every rank owns its own block of Tb timeslices (shard by timeslice, no exchange)
     t0_slice = (rank * Tb) % max(cfg.T - Tb + 1, 1)
     U, D = make_propagators_torch(cfg.seed, cfg.L, cfg.T, dev, t0=t0_slice, nt=Tb)
+    if args.isospin:
+        D = U
     ws = torch.empty(wk.contract_workspace_bytes(terms, cfg.L, Tb, n_mom), dtype=torch.uint8, device=dev)
     Cout = torch.empty((n_mom, Tb), dtype=torch.complex128, device=dev)
 
@@ -280,7 +285,8 @@ def main():
     # ---- roofline of the dominant kernel (a4: minors_kernel<n_u>, minors_kernel<n_d>) ----
     st_per_step = Tb * cfg.volume
     minors_per_st = info.n_minors_u + info.n_minors_d
-    flop_minors = st_per_step * (info.n_minors_u * flops_lu(info.n_u) + info.n_minors_d * flops_lu(info.n_d))
+    d_runs = 1.0 if prof["minors_d"][1] > 0 else 0.0           # isospin: the d minors may be served by the u table
+    flop_minors = st_per_step * (info.n_minors_u * flops_lu(info.n_u) + d_runs * info.n_minors_d * flops_lu(info.n_d))
     ms_minors = (prof["minors_u"][0] + prof["minors_d"][0]) / args.steps
     ms_reduce = prof["reduce"][0] / args.steps
     ms_project = prof["project"][0] / args.steps
@@ -290,7 +296,7 @@ def main():
     mu_row, mu_col, md_row, md_col = terms.minors()
     exec_site = (executed_flops_per_site(info.n_u, tu_rows, tu_cols, mu_row, mu_col),
                  executed_flops_per_site(info.n_d, td_rows, td_cols, md_row, md_col))
-    executed_tf = st_per_step * sum(exec_site) / (ms_minors * 1e-3) / 1e12
+    executed_tf = st_per_step * (exec_site[0] + d_runs * exec_site[1]) / (ms_minors * 1e-3) / 1e12
     traffic = None
     try:
         with open(os.path.join(ROOT, "profiles", "roofline_traffic.json")) as f:
@@ -335,11 +341,11 @@ def main():
         "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms_step,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64 (complex128)", "data": "synthetic",
         "config": {"workload": cfg.name, "L": cfg.L, "T": cfg.T, "timeslices_per_step": Tb, "n_u": info.n_u, "n_d": info.n_d,
-                   "n_terms": int(info.n_terms), "unique_minors_per_site": int(minors_per_st), "n_momenta": n_mom,
+                   "isospin_u_equals_d": bool(args.isospin), "n_terms": int(info.n_terms), "unique_minors_per_site": int(minors_per_st), "n_momenta": n_mom,
                    "l2_policy": "inputs_larger_than_l2" if 2 * U.numel() * 16 > 126e6 else "working_set_larger_than_l2",
                    "parallelism": f"timeslice shards x{world}, no collective on the data path"},
         "minor_dets_per_s": world * st_per_step * minors_per_st / (ms_step * 1e-3),
-        "minor_dets_per_s_kernel_only": st_per_step * minors_per_st / (ms_minors * 1e-3),
+        "minor_dets_per_s_kernel_only": st_per_step * (info.n_minors_u + d_runs * info.n_minors_d) / (ms_minors * 1e-3),
         "roofline": roofline, "cpu_baseline": cpu_baseline, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
         "hbm_peak_gbs_measured": read_measured_peaks().get("hbm_gbs"),
         "propagator_read_gbs": st_per_step * 4608 / (ms_step * 1e-3) / 1e9,

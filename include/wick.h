@@ -134,7 +134,8 @@ size_t wick_contract_workspace_bytes(const wick_terms* terms, int L, int T, int 
 
 /* C[p][t] = sum_x e^{+2 pi i (n_p . x)/L} sum_k w_k detU detD  for t = 0..T-1 (Eq. 15 / A1 / A2 / A7).
  * U_dev, D_dev : device, complex128 [T][L^3][12][12], site s = x + L*(y + L*z), 16-byte aligned.
- *                U_dev == D_dev is legal.
+ *                U_dev == D_dev is legal (isospin limit); if the two flavours then also share their
+ *                unique-minor table (e.g. deuteron, He-4) the minors are evaluated once and serve both flavours.
  * momenta      : host, int32 [n_mom][3], integer units of 2*pi/L (read before the call returns).
  * C_out_dev    : device, complex128 [n_mom][T].
  * sigma_out_dev: NULL or device complex128 [T][L^3]: sigma(x,t) = sum_k w_k detU detD (Eq. A5 :646).

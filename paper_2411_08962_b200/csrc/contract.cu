@@ -565,6 +565,12 @@ extern "C" int wick_contract(const void* U_dev, const void* D_dev, const wick_te
     double2* sigma = reinterpret_cast<double2*>(ws);
     double2* MU = reinterpret_cast<double2*>(ws + p.sigma_bytes);          // sigma_bytes is a multiple of 256
     double2* MD = MU + nmu * S_b;
+    // isospin limit (the paper's m_u = m_d): one propagator for both flavours.  When the two flavours
+    // also have the same unique-minor table, every d minor IS the u minor with the same id: evaluate them once.
+    const bool shared_minors = (U_dev == D_dev) && t->n_u == t->n_d && t->f[0].rows == t->f[1].rows &&
+                               t->f[0].cols == t->f[1].cols && t->f[0].minor_row == t->f[1].minor_row &&
+                               t->f[0].minor_col == t->f[1].minor_col;
+    if (shared_minors) MD = MU;
     double2* partial = MD + nmd * S_b;
     const double2* U = static_cast<const double2*>(U_dev);
     const double2* D = static_cast<const double2*>(D_dev);
@@ -585,7 +591,8 @@ extern "C" int wick_contract(const void* U_dev, const void* D_dev, const wick_te
         const int64_t n_valid = std::min<int64_t>(S_b, p.n_st - st0);
         const int n_groups = int((n_valid + GROUP - 1) / GROUP);
         WICK_CUDA(launch_minors(t->n_u, U, st0, p.n_st, n_groups, S_b, d.minor_desc[0], nmu, MU, PROF_MINORS_U, stream));
-        WICK_CUDA(launch_minors(t->n_d, D, st0, p.n_st, n_groups, S_b, d.minor_desc[1], nmd, MD, PROF_MINORS_D, stream));
+        if (!shared_minors)
+            WICK_CUDA(launch_minors(t->n_d, D, st0, p.n_st, n_groups, S_b, d.minor_desc[1], nmd, MD, PROF_MINORS_D, stream));
         int n_chunks = 1;
         if (t->n_terms == 0) {
             WICK_CUDA(cudaMemsetAsync(sigma + st0, 0, size_t(n_valid) * 16, stream));

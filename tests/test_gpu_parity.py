@@ -242,6 +242,26 @@ def test_empty_term_list_and_isospin_alias(cuda_device):
     _check_C(C, Cr, sabs.sum(axis=1))
 
 
+def test_isospin_alias_shares_the_minor_table(cuda_device):
+    """U_dev == D_dev with equal flavour tables (deuteron): the d minors are not evaluated a second time and
+    the result has the same bits as the run on two separate buffers holding the same propagator."""
+    c = CONFIGS["cfg1"]
+    L, T, mom = 3, 2, [(0, 0, 0), (1, 0, 2)]
+    U, _ = make_propagators_numpy(c.seed, L, T)
+    t = wk.build_terms(c.nucleus)
+    Ud, Ucopy = _dev(U, cuda_device), _dev(U.copy(), cuda_device)
+    wk.launch_count(reset=True)
+    C_alias, s_alias = wk.contract(Ud, Ud, t, mom, L, T, want_sigma=True)
+    n_alias = wk.launch_count(reset=True)
+    C_two, s_two = wk.contract(Ud, Ucopy, t, mom, L, T, want_sigma=True)
+    n_two = wk.launch_count(reset=True)
+    assert torch.equal(C_alias, C_two) and torch.equal(s_alias, s_two)
+    assert n_alias < n_two
+    Cr, sr, sabs = _oracle_lattice("cfg1", U, U, mom, L)
+    assert np.all(np.abs(s_alias.cpu().numpy() - sr) <= REL_TOL * sabs)
+    _check_C(C_alias.cpu().numpy(), Cr, sabs.sum(axis=1))
+
+
 def test_contract_host_matches_device_call(cuda_device):
     c = CONFIGS["cfg0"]
     U, D = make_propagators_numpy(c.seed, c.L, c.T)
