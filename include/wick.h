@@ -119,6 +119,13 @@ int  wick_terms_export_terms(const wick_terms* terms, int64_t first, int64_t cou
  * Returns WICK_ERR_UNSUPPORTED if !is_outer_product. */
 int  wick_terms_export_factors(const wick_terms* terms, int32_t* sink_ru, int32_t* sink_rd, double* sink_c_reim,
                                int32_t* src_cu, int32_t* src_cd, double* src_c_reim);
+/* Host-only self-check of the schedule of the staged factorised reduction (reduce_staged_kernel) for
+ * n_bins CTA bins: every (u-row tuple, d-column tuple) pair of the factorised sum (PAPER.md Eq. A1-A5 regrouped) is
+ * covered by exactly one batch, every batch fits the shared-memory capacities and every coefficient entry points
+ * inside its staged block.  Outputs (any may be NULL): number of batches, pairs covered, largest MD block, most
+ * u-row tuples in a batch.  WICK_ERR_UNSUPPORTED: not an outer-product list, or a block too large to stage. */
+int  wick_terms_staged_schedule_check(const wick_terms* terms, int n_bins, int64_t* n_batches, int64_t* n_pairs,
+                                      int64_t* max_md_elements, int64_t* max_rows);
 void wick_terms_free(wick_terms* terms);
 
 /* ---------------------------------------------------------------------------------------------

@@ -23,7 +23,8 @@ CONTRACT_COMPLEX_COEFFS = 4
 
 EXPORTED_SYMBOLS = (
     "wick_build_terms", "wick_build_terms_from_list", "wick_terms_get_info", "wick_terms_export_tuples",
-    "wick_terms_export_minors", "wick_terms_export_terms", "wick_terms_export_factors", "wick_terms_free",
+    "wick_terms_export_minors", "wick_terms_export_terms", "wick_terms_export_factors",
+    "wick_terms_staged_schedule_check", "wick_terms_free",
     "wick_contract_min_workspace_bytes", "wick_contract_workspace_bytes", "wick_contract",
     "wick_contract_host", "wick_minor_dets", "wick_launch_count", "wick_launch_count_reset",
     "wick_last_error", "wick_version", "wick_profile_enable", "wick_profile_read", "wick_measure_fp64_peak",
@@ -73,6 +74,7 @@ def load_library():
     lib.wick_terms_export_minors.argtypes = [vp, vp, vp, vp, vp]
     lib.wick_terms_export_terms.argtypes = [vp, i64, i64, vp, vp, vp]
     lib.wick_terms_export_factors.argtypes = [vp, vp, vp, vp, vp, vp, vp]
+    lib.wick_terms_staged_schedule_check.argtypes = [vp, C.c_int, vp, vp, vp, vp]
     lib.wick_terms_free.argtypes = [vp]
     lib.wick_terms_free.restype = None
     for f in (lib.wick_contract_min_workspace_bytes, lib.wick_contract_workspace_bytes):
@@ -146,6 +148,13 @@ class Terms:
         _check(_lib.wick_terms_export_factors(self._h, _np_ptr(sru), _np_ptr(srd), _np_ptr(sc),
                                               _np_ptr(qcu), _np_ptr(qcd), _np_ptr(qc)), "wick_terms_export_factors")
         return sru, srd, sc, qcu, qcd, qc
+
+    def staged_schedule_check(self, n_bins: int):
+        """Host-only self-check of the staged-reduction schedule; returns (batches, pairs covered, max MD block, max rows)."""
+        out = [C.c_int64(0) for _ in range(4)]
+        _check(_lib.wick_terms_staged_schedule_check(self._h, n_bins, *[C.byref(o) for o in out]),
+               "wick_terms_staged_schedule_check")
+        return tuple(int(o.value) for o in out)
 
     def term_tuples(self, first: int = 0, count: Optional[int] = None):
         """Flat terms as index tuples (a_u, b_u, a_d, b_d, w) -- what an oracle consumes."""

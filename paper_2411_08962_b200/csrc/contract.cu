@@ -247,31 +247,18 @@ int upload_tables(const wick_terms* t, cudaStream_t stream) {
     return WICK_OK;
 }
 
-// ---- staged factorised reduction: host schedule (kernels.cu: reduce_staged_kernel) --------------
-// Tuples grouped by block: ru_list / rd_list by sink block, cu_list / cd_list by source block.
-// Batches = (source block k', d-column piece) x (run of sink blocks) with at most STG_MD_CAP MD elements;
-// batches are assigned to n_bins CTAs by longest-processing-time, each bin keeps a fixed order.
-// Returns 1 and fills `out` when the list is eligible, 0 when a block is too large (caller falls back
-// to reduce_outer_kernel), negative on error.
-int ensure_staged(const wick_terms* t, int n_bins, cudaStream_t stream, StagedTables* out) {
-    std::lock_guard<std::mutex> lock(t->mu);
-    DeviceTables& d = t->dev;
-    if (d.staged_state < 0) return 0;
+struct StagedHost {
+    bool ok = false;                                              // false: a block exceeds the staging capacities
+    std::vector<int32_t> sink_ptr, sink_rdpos, src_ptr, src_cupos, ru_list, rd_list, cu_list, cd_list, bin_ptr;
+    std::vector<double> sink_c, src_c;
+    std::vector<StagedBatch> batches;
+};
+
+// Host part of the staged schedule (no CUDA call): also what wick_terms_staged_schedule_check verifies.
+StagedHost build_staged_host(const wick_terms* t, int n_bins) {
+    StagedHost h;
     const int nru = int(t->f[0].rows.size()), nrd = int(t->f[1].rows.size());
     const int ncu = int(t->f[0].cols.size()), ncd = int(t->f[1].cols.size());
-    auto fill = [&](const StagedDev& sd) {
-        out->n_cols_u = ncu; out->n_cols_d = ncd; out->n_bins = sd.n_bins;
-        out->real_coeffs = true;
-        for (const FactorTerm& f : t->sink) if (f.c.imag() != 0.0) out->real_coeffs = false;
-        for (const FactorTerm& f : t->source) if (f.c.imag() != 0.0) out->real_coeffs = false;
-        out->sink_ptr = sd.sink_ptr; out->sink_rdpos = sd.sink_rdpos; out->sink_c = reinterpret_cast<const double2*>(sd.sink_c);
-        out->src_ptr = sd.src_ptr; out->src_cupos = sd.src_cupos; out->src_c = reinterpret_cast<const double2*>(sd.src_c);
-        out->ru_list = sd.ru_list; out->rd_list = sd.rd_list; out->cu_list = sd.cu_list; out->cd_list = sd.cd_list;
-        out->bin_ptr = sd.bin_ptr; out->batches = static_cast<const StagedBatch*>(sd.batches);
-    };
-    auto hit = d.staged.find(n_bins);
-    if (hit != d.staged.end()) { fill(hit->second); return 1; }
-
     const Components cs = factor_components(nru, nrd, t->sink);
     Components cq = factor_components(ncu, ncd, t->source);
     {   // source blocks relabelled by decreasing number of d columns, so that small blocks are neighbours and can share a piece
@@ -301,7 +288,7 @@ int ensure_staged(const wick_terms* t, int n_bins, cudaStream_t stream, StagedTa
     int max_rd = 1, max_cu = 1;
     for (int k = 0; k < cs.n; ++k) max_rd = std::max(max_rd, rd_ptr[size_t(k) + 1] - rd_ptr[size_t(k)]);
     for (int k = 0; k < cq.n; ++k) max_cu = std::max(max_cu, cu_ptr[size_t(k) + 1] - cu_ptr[size_t(k)]);
-    if (max_rd > STG_MD_CAP || max_cu > STG_ROW_CAP || cs.n == 0 || cq.n == 0) { d.staged_state = -1; return 0; }
+    if (max_rd > STG_MD_CAP || max_cu > STG_ROW_CAP || cs.n == 0 || cq.n == 0) return h;
 
     // coefficient lists regrouped by list position, so that a batch's entries are contiguous:
     // sink entries by position of ru in ru_list, source entries by position of cd in cd_list
@@ -328,12 +315,11 @@ int ensure_staged(const wick_terms* t, int n_bins, cudaStream_t stream, StagedTa
         }
     }
     // a single u-row tuple or a single d column must fit the entry buffers
-    for (int r = 0; r < nru; ++r) if (sink_ptr[size_t(r) + 1] - sink_ptr[size_t(r)] > STG_SINK_CAP) { d.staged_state = -1; return 0; }
-    for (int c = 0; c < ncd; ++c) if (src_ptr[size_t(c) + 1] - src_ptr[size_t(c)] > STG_SRC_CAP) { d.staged_state = -1; return 0; }
+    for (int r = 0; r < nru; ++r) if (sink_ptr[size_t(r) + 1] - sink_ptr[size_t(r)] > STG_SINK_CAP) return h;
+    for (int c = 0; c < ncd; ++c) if (src_ptr[size_t(c) + 1] - src_ptr[size_t(c)] > STG_SRC_CAP) return h;
     for (int k = 0; k < cs.n; ++k)                              // one sink block must fit a batch on its own
         if (ru_ptr[size_t(k) + 1] - ru_ptr[size_t(k)] > STG_ROWS_CAP ||
-            sink_ptr[size_t(ru_ptr[size_t(k) + 1])] - sink_ptr[size_t(ru_ptr[size_t(k)])] > STG_SINK_CAP) { d.staged_state = -1; return 0; }
-    d.staged_state = 1;
+            sink_ptr[size_t(ru_ptr[size_t(k) + 1])] - sink_ptr[size_t(ru_ptr[size_t(k)])] > STG_SINK_CAP) return h;
 
     struct Item { int64_t cost; StagedBatch b; };
     std::vector<Item> items;
@@ -407,6 +393,45 @@ int ensure_staged(const wick_terms* t, int n_bins, cudaStream_t stream, StagedTa
         batches.insert(batches.end(), bins[size_t(b)].begin(), bins[size_t(b)].end());
         bin_ptr[size_t(b) + 1] = int32_t(batches.size());
     }
+    h.ok = true;
+    h.sink_ptr = std::move(sink_ptr); h.sink_rdpos = std::move(sink_rdpos); h.src_ptr = std::move(src_ptr); h.src_cupos = std::move(src_cupos);
+    h.ru_list = std::move(ru_list); h.rd_list = std::move(rd_list); h.cu_list = std::move(cu_list); h.cd_list = std::move(cd_list);
+    h.bin_ptr = std::move(bin_ptr); h.sink_c = std::move(sink_c); h.src_c = std::move(src_c); h.batches = std::move(batches);
+    return h;
+}
+
+// ---- staged factorised reduction: host schedule (kernels.cu: reduce_staged_kernel) --------------
+// Tuples grouped by block: ru_list / rd_list by sink block, cu_list / cd_list by source block.
+// Batches = (source block k', d-column piece) x (run of sink blocks) with at most STG_MD_CAP MD elements;
+// batches are assigned to n_bins CTAs by longest-processing-time, each bin keeps a fixed order.
+// Returns 1 and fills `out` when the list is eligible, 0 when a block is too large (caller falls back
+// to reduce_outer_kernel), negative on error.
+int ensure_staged(const wick_terms* t, int n_bins, cudaStream_t stream, StagedTables* out) {
+    std::lock_guard<std::mutex> lock(t->mu);
+    DeviceTables& d = t->dev;
+    if (d.staged_state < 0) return 0;
+    const int nru = int(t->f[0].rows.size()), nrd = int(t->f[1].rows.size());
+    const int ncu = int(t->f[0].cols.size()), ncd = int(t->f[1].cols.size());
+    auto fill = [&](const StagedDev& sd) {
+        out->n_cols_u = ncu; out->n_cols_d = ncd; out->n_bins = sd.n_bins;
+        out->real_coeffs = true;
+        for (const FactorTerm& f : t->sink) if (f.c.imag() != 0.0) out->real_coeffs = false;
+        for (const FactorTerm& f : t->source) if (f.c.imag() != 0.0) out->real_coeffs = false;
+        out->sink_ptr = sd.sink_ptr; out->sink_rdpos = sd.sink_rdpos; out->sink_c = reinterpret_cast<const double2*>(sd.sink_c);
+        out->src_ptr = sd.src_ptr; out->src_cupos = sd.src_cupos; out->src_c = reinterpret_cast<const double2*>(sd.src_c);
+        out->ru_list = sd.ru_list; out->rd_list = sd.rd_list; out->cu_list = sd.cu_list; out->cd_list = sd.cd_list;
+        out->bin_ptr = sd.bin_ptr; out->batches = static_cast<const StagedBatch*>(sd.batches);
+    };
+    auto hit = d.staged.find(n_bins);
+    if (hit != d.staged.end()) { fill(hit->second); return 1; }
+
+    const StagedHost h = build_staged_host(t, n_bins);
+    if (!h.ok) { d.staged_state = -1; return 0; }
+    d.staged_state = 1;
+    const std::vector<int32_t>&sink_rdpos = h.sink_rdpos, &src_cupos = h.src_cupos, &sink_ptr = h.sink_ptr, &src_ptr = h.src_ptr;
+    const std::vector<int32_t>&ru_list = h.ru_list, &rd_list = h.rd_list, &cu_list = h.cu_list, &cd_list = h.cd_list, &bin_ptr = h.bin_ptr;
+    const std::vector<double>&sink_c = h.sink_c, &src_c = h.src_c;
+    const std::vector<StagedBatch>& batches = h.batches;
     BlobBuilder bb;
     const size_t o_srp = bb.add(sink_rdpos.data(), sink_rdpos.size() * 4), o_scp = bb.add(src_cupos.data(), src_cupos.size() * 4);
     const size_t o_sp = bb.add(sink_ptr.data(), sink_ptr.size() * 4), o_qp = bb.add(src_ptr.data(), src_ptr.size() * 4);
@@ -509,6 +534,50 @@ extern "C" void wick_terms_release_device(DeviceTables* d) {
     if (d->flat_blob) cudaFree(d->flat_blob);
     for (auto& kv : d->staged) cudaFree(kv.second.blob);
     *d = DeviceTables();
+}
+
+extern "C" int wick_terms_staged_schedule_check(const wick_terms* t, int n_bins, int64_t* n_batches_out, int64_t* n_pairs_out,
+                                               int64_t* max_md_elements_out, int64_t* max_rows_out) {
+    if (!t || n_bins < 1) { set_error("wick_terms_staged_schedule_check: bad argument"); return WICK_ERR_ARG; }
+    if (!t->outer) { set_error("not an outer-product term list"); return WICK_ERR_UNSUPPORTED; }
+    StagedHost h;
+    try { h = build_staged_host(t, n_bins); } catch (const std::bad_alloc&) { set_error("out of host memory"); return WICK_ERR_NOMEM; }
+    if (!h.ok) { set_error("a block of the factor lists exceeds the staging capacities (the unstaged kernel is used)"); return WICK_ERR_UNSUPPORTED; }
+    const size_t nru = t->f[0].rows.size(), ncd = t->f[1].cols.size();
+    std::vector<uint8_t> covered(nru * ncd, 0);
+    int64_t max_md = 0, max_rows = 0;
+    auto fail = [](const char* what) { set_error(std::string("staged schedule: ") + what); return WICK_ERR_ARG; };
+    if (h.bin_ptr.size() != size_t(n_bins) + 1 || h.bin_ptr.front() != 0 || size_t(h.bin_ptr.back()) != h.batches.size())
+        return fail("bins do not cover the batch list");
+    for (const StagedBatch& b : h.batches) {
+        const int n_cd = b.cd_b - b.cd_a, n_cu = b.cu_b - b.cu_a, n_rd = b.rd_b - b.rd_a, rows = b.ru_b - b.ru_a;
+        if (n_cd < 1 || n_cd > STG_NCD_CAP || n_cu < 1 || n_cu > STG_ROW_CAP || rows < 1 || rows > STG_ROWS_CAP ||
+            int64_t(n_rd) * n_cd > STG_MD_CAP) return fail("a batch exceeds a capacity");
+        if (h.sink_ptr[size_t(b.ru_b)] - h.sink_ptr[size_t(b.ru_a)] > STG_SINK_CAP ||
+            h.src_ptr[size_t(b.cd_b)] - h.src_ptr[size_t(b.cd_a)] > STG_SRC_CAP) return fail("a batch exceeds an entry buffer");
+        max_md = std::max<int64_t>(max_md, int64_t(n_rd) * n_cd);
+        max_rows = std::max<int64_t>(max_rows, rows);
+        for (int r = b.ru_a; r < b.ru_b; ++r) {
+            for (int i = h.sink_ptr[size_t(r)]; i < h.sink_ptr[size_t(r) + 1]; ++i)
+                if (h.sink_rdpos[size_t(i)] < b.rd_a || h.sink_rdpos[size_t(i)] >= b.rd_b) return fail("a sink entry points outside the staged MD block");
+            for (int c = b.cd_a; c < b.cd_b; ++c) {
+                uint8_t& cell = covered[size_t(r) * ncd + size_t(c)];
+                if (cell) return fail("a (u-row tuple, d-column tuple) pair is covered twice");
+                cell = 1;
+            }
+        }
+        for (int c = b.cd_a; c < b.cd_b; ++c)
+            for (int j = h.src_ptr[size_t(c)]; j < h.src_ptr[size_t(c) + 1]; ++j)
+                if (h.src_cupos[size_t(j)] < b.cu_a || h.src_cupos[size_t(j)] >= b.cu_b) return fail("a source entry points outside the staged MU row");
+    }
+    int64_t n_pairs = 0;
+    for (uint8_t c : covered) n_pairs += c;
+    if (n_pairs != int64_t(nru) * int64_t(ncd)) return fail("a (u-row tuple, d-column tuple) pair is not covered");
+    if (n_batches_out) *n_batches_out = int64_t(h.batches.size());
+    if (n_pairs_out) *n_pairs_out = n_pairs;
+    if (max_md_elements_out) *max_md_elements_out = max_md;
+    if (max_rows_out) *max_rows_out = max_rows;
+    return WICK_OK;
 }
 
 extern "C" int64_t wick_launch_count(void) { return launch_counter_get(); }

@@ -92,51 +92,14 @@ __device__ __forceinline__ c128 det2(c128 a, c128 b, c128 c, c128 d) {   // a d 
     return cfnma(b, c, cmul(a, d));
 }
 
+// N <= 2 (N = 3 and up keep state across minors, see minors_kernel / LuState)
 template <int N>
 __device__ __forceinline__ c128 det_small(const c128* tl, const Idx<N>& ix) {
-    if (N == 0) return make_double2(1.0, 0.0);
-    if (N == 1) return ld(tl, ix.re[0], ix.ce[0]);
-    if (N == 2)
-        return det2(ld(tl, ix.re[0], ix.ce[0]), ld(tl, ix.re[0], ix.ce[1]),
-                    ld(tl, ix.re[1], ix.ce[0]), ld(tl, ix.re[1], ix.ce[1]));
-    if (N == 3) {
-        c128 m[3][3];
-#pragma unroll
-        for (int i = 0; i < 3; ++i)
-#pragma unroll
-            for (int j = 0; j < 3; ++j) m[i][j] = ld(tl, ix.re[i], ix.ce[j]);
-        // expansion along the first row
-        c128 d = cmul(m[0][0], det2(m[1][1], m[1][2], m[2][1], m[2][2]));
-        d = cfnma(m[0][1], det2(m[1][0], m[1][2], m[2][0], m[2][2]), d);
-        d = cfma(m[0][2], det2(m[1][0], m[1][1], m[2][0], m[2][1]), d);
-        return d;
-    }
-    // N == 4: Laplace expansion along the first two rows: sum over column pairs of
-    // (2x2 minor of rows 0,1) * (complementary 2x2 minor of rows 2,3) * sign
-    c128 m[4][4];
-#pragma unroll
-    for (int i = 0; i < 4; ++i)
-#pragma unroll
-        for (int j = 0; j < 4; ++j) m[i][j] = ld(tl, ix.re[i], ix.ce[j]);
-    const c128 s01 = det2(m[0][0], m[0][1], m[1][0], m[1][1]);
-    const c128 s02 = det2(m[0][0], m[0][2], m[1][0], m[1][2]);
-    const c128 s03 = det2(m[0][0], m[0][3], m[1][0], m[1][3]);
-    const c128 s12 = det2(m[0][1], m[0][2], m[1][1], m[1][2]);
-    const c128 s13 = det2(m[0][1], m[0][3], m[1][1], m[1][3]);
-    const c128 s23 = det2(m[0][2], m[0][3], m[1][2], m[1][3]);
-    const c128 b01 = det2(m[2][0], m[2][1], m[3][0], m[3][1]);
-    const c128 b02 = det2(m[2][0], m[2][2], m[3][0], m[3][2]);
-    const c128 b03 = det2(m[2][0], m[2][3], m[3][0], m[3][3]);
-    const c128 b12 = det2(m[2][1], m[2][2], m[3][1], m[3][2]);
-    const c128 b13 = det2(m[2][1], m[2][3], m[3][1], m[3][3]);
-    const c128 b23 = det2(m[2][2], m[2][3], m[3][2], m[3][3]);
-    c128 d = cmul(s01, b23);
-    d = cfnma(s02, b13, d);
-    d = cfma(s03, b12, d);
-    d = cfma(s12, b03, d);
-    d = cfnma(s13, b02, d);
-    d = cfma(s23, b01, d);
-    return d;
+    static_assert(N <= 2, "larger minors go through the column trie");
+    if constexpr (N == 0) return make_double2(1.0, 0.0);
+    else if constexpr (N == 1) return ld(tl, ix.re[0], ix.ce[0]);
+    else return det2(ld(tl, ix.re[0], ix.ce[0]), ld(tl, ix.re[0], ix.ce[1]),
+                     ld(tl, ix.re[1], ix.ce[0]), ld(tl, ix.re[1], ix.ce[1]));
 }
 
 // reciprocal of a pivot: 1/(x + i y) = (x - i y) / (x^2 + y^2).  The real reciprocal is MUFU.RCP64H

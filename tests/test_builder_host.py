@@ -204,3 +204,24 @@ def test_workspace_planning():
     assert lo < hi <= (2 << 30) + 64 * 32768 * 16 + 4096
     t0 = wk.build_terms(NUCLEI["cfg0"])
     assert wk.contract_workspace_bytes(t0, 4, 8, 1) >= 512 * 585 * 16
+
+
+# ---------------------------------------------------------------------------------------------
+# schedule of the staged factorised reduction (host logic of contract.cu, no GPU needed)
+# ---------------------------------------------------------------------------------------------
+
+@pytest.mark.parametrize("cfg", ["cfg0", "cfg1", "cfg2", "cfg3", "cfg4"])
+@pytest.mark.parametrize("n_bins", [1, 2, 37, 74])
+def test_staged_schedule_covers_every_pair_once(cfg, n_bins):
+    t = wk.build_terms(CONFIGS[cfg].nucleus)
+    i = t.info
+    batches, pairs, max_md, max_rows = t.staged_schedule_check(n_bins)   # raises if a pair is missed / doubled / out of range
+    assert pairs == i.n_rows_u * i.n_cols_d
+    assert 1 <= batches and 1 <= max_md <= 96 and 1 <= max_rows <= 96
+
+
+def test_staged_schedule_rejects_generic_lists():
+    c = CONFIGS["cfg4b"]
+    t = wk.build_terms_from_list(*make_random_term_list(c.seed, c.n_u, c.n_d, c.n_random_terms))
+    with pytest.raises(wk.WickError):
+        t.staged_schedule_check(4)
