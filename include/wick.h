@@ -189,6 +189,11 @@ int wick_measure_fp64_peak(double* tflops_out, void* cuda_stream);
 int64_t wick_launch_count(void);
 int64_t wick_launch_count_reset(void);
 
+/* wick_contract_host keeps its device buffers (propagator blocks, workspace), two streams and four events per host
+ * thread between calls; this frees them (call it from the thread that made the host calls, with its device current). */
+void wick_release_cached_buffers(void);
+
+/* Message of the last error on this thread (thread-local, never NULL); library version string. */
 const char* wick_last_error(void);
 const char* wick_version(void);
 

@@ -26,7 +26,7 @@ EXPORTED_SYMBOLS = (
     "wick_terms_export_minors", "wick_terms_export_terms", "wick_terms_export_factors",
     "wick_terms_staged_schedule_check", "wick_terms_free",
     "wick_contract_min_workspace_bytes", "wick_contract_workspace_bytes", "wick_contract",
-    "wick_contract_host", "wick_minor_dets", "wick_launch_count", "wick_launch_count_reset",
+    "wick_contract_host", "wick_release_cached_buffers", "wick_minor_dets", "wick_launch_count", "wick_launch_count_reset",
     "wick_last_error", "wick_version", "wick_profile_enable", "wick_profile_read", "wick_measure_fp64_peak",
 )
 
@@ -77,6 +77,8 @@ def load_library():
     lib.wick_terms_staged_schedule_check.argtypes = [vp, C.c_int, vp, vp, vp, vp]
     lib.wick_terms_free.argtypes = [vp]
     lib.wick_terms_free.restype = None
+    lib.wick_release_cached_buffers.restype = None
+    lib.wick_release_cached_buffers.argtypes = []
     for f in (lib.wick_contract_min_workspace_bytes, lib.wick_contract_workspace_bytes):
         f.argtypes = [vp, i32, i32, i32]
         f.restype = sz
@@ -273,6 +275,11 @@ def minor_dets(P, rows, cols, stream=None):
                                  _stream_ptr(stream))
     _check(rc, "wick_minor_dets")
     return out
+
+
+def release_cached_buffers() -> None:
+    """Free the device buffers contract_host keeps between calls (this thread)."""
+    _lib.wick_release_cached_buffers()
 
 
 def launch_count(reset: bool = False) -> int:

@@ -695,6 +695,57 @@ extern "C" int wick_contract(const void* U_dev, const void* D_dev, const wick_te
     return WICK_OK;
 }
 
+namespace {
+struct HostPathCache {
+    enum Slot { U0 = 0, U1, D0, D1, WS, C, S, N_SLOTS };
+    int device = -1;
+    void* buf[N_SLOTS] = {};
+    size_t cap[N_SLOTS] = {};
+    cudaStream_t sc = nullptr, sx = nullptr;
+    cudaEvent_t copied[2] = {nullptr, nullptr}, consumed[2] = {nullptr, nullptr};
+    void release() {
+        for (int k = 0; k < N_SLOTS; ++k) { if (buf[k]) cudaFree(buf[k]); buf[k] = nullptr; cap[k] = 0; }
+        for (int k = 0; k < 2; ++k) {
+            if (copied[k]) cudaEventDestroy(copied[k]);
+            if (consumed[k]) cudaEventDestroy(consumed[k]);
+            copied[k] = consumed[k] = nullptr;
+        }
+        if (sc) cudaStreamDestroy(sc);
+        if (sx) cudaStreamDestroy(sx);
+        sc = sx = nullptr;
+        device = -1;
+    }
+    cudaError_t prepare() {                                     // streams and events for the current device
+        int dev = -1;
+        cudaError_t e = cudaGetDevice(&dev);
+        if (e != cudaSuccess) return e;
+        if (dev != device) release();
+        device = dev;
+        if (!sc && (e = cudaStreamCreate(&sc)) != cudaSuccess) return e;
+        if (!sx && (e = cudaStreamCreate(&sx)) != cudaSuccess) return e;
+        for (int k = 0; k < 2; ++k) {
+            if (!copied[k] && (e = cudaEventCreateWithFlags(&copied[k], cudaEventDisableTiming)) != cudaSuccess) return e;
+            if (!consumed[k] && (e = cudaEventCreateWithFlags(&consumed[k], cudaEventDisableTiming)) != cudaSuccess) return e;
+        }
+        return cudaSuccess;
+    }
+    cudaError_t acquire(int slot, size_t bytes, void** out) {   // grow-only
+        if (cap[slot] < bytes) {
+            if (buf[slot]) { cudaFree(buf[slot]); buf[slot] = nullptr; cap[slot] = 0; }
+            const cudaError_t e = cudaMalloc(&buf[slot], bytes);
+            if (e != cudaSuccess) return e;
+            cap[slot] = bytes;
+        }
+        *out = buf[slot];
+        return cudaSuccess;
+    }
+    ~HostPathCache() {}                                         // process exit: the driver reclaims; no CUDA calls in static destructors
+};
+HostPathCache& host_path_cache() { static thread_local HostPathCache c; return c; }
+}  // namespace
+
+extern "C" void wick_release_cached_buffers(void) { host_path_cache().release(); }
+
 extern "C" int wick_contract_host(const void* U_host, const void* D_host, const wick_terms* t, const int32_t* momenta,
                                   int n_mom, int L, int T, void* C_out_host, void* sigma_out_host, unsigned flags) {
     if (!U_host || !D_host || !t || !C_out_host || (n_mom > 0 && !momenta) || L < 1 || T < 1 || n_mom < 0) {
@@ -708,28 +759,25 @@ extern "C" int wick_contract_host(const void* U_host, const void* D_host, const 
     Tb = std::min(Tb, T);
     const size_t ws_bytes = wick_contract_workspace_bytes(t, L, Tb, n_mom);
     if (!ws_bytes) { set_error("wick_contract_host: bad sizes"); return WICK_ERR_ARG; }
-    void *dU[2] = {nullptr, nullptr}, *dD[2] = {nullptr, nullptr}, *ws = nullptr, *dC = nullptr, *dS = nullptr;
-    cudaStream_t sc = nullptr, sx = nullptr;
-    cudaEvent_t copied[2] = {nullptr, nullptr}, consumed[2] = {nullptr, nullptr};
+    // device buffers, streams and events of the host path are kept per host thread between calls
+    // (wick_release_cached_buffers frees them): a cudaMalloc of the multi-GB workspace per call costs
+    // more than the contraction of a small lattice
+    HostPathCache& hc = host_path_cache();
     int rc = WICK_OK;
-    auto cleanup = [&]() {
-        for (int k = 0; k < 2; ++k) { cudaFree(dU[k]); cudaFree(dD[k]); if (copied[k]) cudaEventDestroy(copied[k]); if (consumed[k]) cudaEventDestroy(consumed[k]); }
-        cudaFree(ws); cudaFree(dC); cudaFree(dS);
-        if (sc) cudaStreamDestroy(sc);
-        if (sx) cudaStreamDestroy(sx);
-    };
+    auto cleanup = [&]() {};
 #define WICK_CUDA_H(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) { set_error(std::string(#call) + ": " + cudaGetErrorString(e_)); cleanup(); return WICK_ERR_CUDA; } } while (0)
-    WICK_CUDA_H(cudaStreamCreate(&sc));
-    WICK_CUDA_H(cudaStreamCreate(&sx));
+    WICK_CUDA_H(hc.prepare());
+    void *dU[2], *dD[2], *ws = nullptr, *dC = nullptr, *dS = nullptr;
+    cudaStream_t sc = hc.sc, sx = hc.sx;
+    cudaEvent_t* copied = hc.copied;
+    cudaEvent_t* consumed = hc.consumed;
     for (int k = 0; k < 2; ++k) {
-        WICK_CUDA_H(cudaMalloc(&dU[k], slice_bytes * Tb));
-        WICK_CUDA_H(cudaMalloc(&dD[k], slice_bytes * Tb));
-        WICK_CUDA_H(cudaEventCreateWithFlags(&copied[k], cudaEventDisableTiming));
-        WICK_CUDA_H(cudaEventCreateWithFlags(&consumed[k], cudaEventDisableTiming));
+        WICK_CUDA_H(hc.acquire(HostPathCache::U0 + k, slice_bytes * Tb, &dU[k]));
+        WICK_CUDA_H(hc.acquire(HostPathCache::D0 + k, slice_bytes * Tb, &dD[k]));
     }
-    WICK_CUDA_H(cudaMalloc(&ws, ws_bytes));
-    WICK_CUDA_H(cudaMalloc(&dC, std::max<size_t>(size_t(n_mom) * Tb * 16, 16)));
-    if (sigma_out_host) WICK_CUDA_H(cudaMalloc(&dS, size_t(V) * Tb * 16));
+    WICK_CUDA_H(hc.acquire(HostPathCache::WS, ws_bytes, &ws));
+    WICK_CUDA_H(hc.acquire(HostPathCache::C, std::max<size_t>(size_t(n_mom) * Tb * 16, 16), &dC));
+    if (sigma_out_host) WICK_CUDA_H(hc.acquire(HostPathCache::S, size_t(V) * Tb * 16, &dS));
     const unsigned char* Uh = static_cast<const unsigned char*>(U_host);
     const unsigned char* Dh = static_cast<const unsigned char*>(D_host);
     std::vector<double> Cblk(size_t(std::max(n_mom, 1)) * Tb * 2);
