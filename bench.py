@@ -51,7 +51,15 @@ def executed_flops_per_site(n: int, rows: np.ndarray, cols: np.ndarray, minor_ro
     nm = len(minor_row)
     if n <= 2 or nm == 0:
         return nm * flops_lu(n)
-    c = cols[minor_col]                                            # [nm][n] column tuples in minor order
+    c = cols[minor_col].astype(np.int64)                           # [nm][n] column tuples in minor order
+    if n >= 9:
+        # the library's processing order for large minors (contract.cu: build_minor_descs): column tuples that miss only
+        # small indices (< 6) are walked with descending columns, each group sorted by its processing order
+        descending = np.array([set(range(6, 12)) <= set(t) and len(t) < 12 for t in c.tolist()])
+        proc = np.where(descending[:, None], c[:, ::-1], c)
+        keys = [proc[:, k] for k in range(n - 1, -1, -1)] + [descending.astype(np.int64), minor_row.astype(np.int64)]
+        order = np.lexsort(keys)
+        c, minor_row = proc[order], minor_row[order]
     same_row = minor_row[1:] == minor_row[:-1]
     if n == 3:                                                     # cofactors of the last column per (rows, b0, b1)
         n_pair = 1 + int(np.count_nonzero(~(same_row & np.all(c[1:, :2] == c[:-1, :2], axis=1))))

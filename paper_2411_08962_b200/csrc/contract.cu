@@ -56,10 +56,57 @@ uint64_t nibbles_of_mask(uint16_t mask) {
     return w;
 }
 
-// minor descriptors for launch_minors (kernels.cu: struct Desc)
-void pack_minor_desc(int n, uint64_t rows, uint64_t cols, uint64_t* out) {
+// minor descriptors for launch_minors (kernels.cu: struct Desc); out_id / negate only exist for n >= 9
+void pack_minor_desc(int n, uint64_t rows, uint64_t cols, uint32_t out_id, bool negate, uint64_t* out) {
     if (minor_desc_words(n) == 1) out[0] = (rows & 0xffffffffull) | (cols << 32);
-    else { out[0] = rows; out[1] = cols; }
+    else {
+        out[0] = (rows & 0xffffffffffffull) | (uint64_t(out_id & 0xffffu) << 48);
+        out[1] = (cols & 0xffffffffffffull) | (uint64_t((out_id >> 16) & 0x7fffu) << 48) | (uint64_t(negate ? 1 : 0) << 63);
+    }
+}
+
+// nibble list reversed (n fields)
+uint64_t reverse_nibbles(uint64_t w, int n) {
+    uint64_t r = 0;
+    for (int k = 0; k < n; ++k) r |= ((w >> (4 * k)) & 15u) << (4 * (n - 1 - k));
+    return r;
+}
+
+// Descriptor list of one flavour in processing order.  n <= 8: minor order (row tuple by row tuple, column tuples
+// lexicographic: consecutive minors share leading columns).  n >= 9: within a row tuple, column tuples whose missing
+// indices are all small (< 6) are processed with DESCENDING columns, so that they share their leading (large) columns
+// the way the others share their small ones; each group is sorted by its processing order.  det with reversed columns
+// = (-1)^(n(n-1)/2) det, folded into the descriptor's sign.
+std::vector<uint64_t> build_minor_descs(const FlavourTables& ft) {
+    const int n = ft.n, words = minor_desc_words(n);
+    const size_t nm = ft.minor_row.size();
+    std::vector<uint64_t> desc(nm * size_t(words));
+    if (words == 1) {
+        for (size_t m = 0; m < nm; ++m)
+            pack_minor_desc(n, nibbles_of_mask(ft.rows[size_t(ft.minor_row[m])]), nibbles_of_mask(ft.cols[size_t(ft.minor_col[m])]), 0, false,
+                            desc.data() + m);
+        return desc;
+    }
+    struct Key { int32_t row; int group; uint64_t cols; uint32_t m; };
+    std::vector<Key> keys(nm);
+    const bool rev_negates = ((n * (n - 1) / 2) & 1) != 0;
+    for (size_t m = 0; m < nm; ++m) {
+        const uint16_t cmask = ft.cols[size_t(ft.minor_col[m])];
+        const bool descending = (uint16_t(~cmask) & 0x0fc0u) == 0 && cmask != 0x0fffu;   // nothing missing among 6..11, something among 0..5
+        const uint64_t asc = nibbles_of_mask(cmask);
+        keys[m] = Key{ft.minor_row[m], descending ? 1 : 0, descending ? reverse_nibbles(asc, n) : asc, uint32_t(m)};
+    }
+    // sort by (row tuple, group, columns in processing order read as a tuple: first column most significant)
+    auto tuple_key = [n](uint64_t w) { uint64_t k = 0; for (int i = 0; i < n; ++i) k = (k << 4) | ((w >> (4 * i)) & 15u); return k; };
+    std::stable_sort(keys.begin(), keys.end(), [&](const Key& a, const Key& b) {
+        if (a.row != b.row) return a.row < b.row;
+        if (a.group != b.group) return a.group < b.group;
+        return tuple_key(a.cols) < tuple_key(b.cols);
+    });
+    for (size_t k = 0; k < nm; ++k)
+        pack_minor_desc(n, nibbles_of_mask(ft.rows[size_t(keys[k].row)]), keys[k].cols, keys[k].m, keys[k].group == 1 && rev_negates,
+                        desc.data() + k * size_t(words));
+    return desc;
 }
 
 // Connected components of the bipartite graph (qu -- qd) of a factor list.  Physical sink lists are
@@ -175,11 +222,8 @@ int upload_tables(const wick_terms* t, cudaStream_t stream) {
     size_t o_desc[2];
     for (int f = 0; f < 2; ++f) {
         const FlavourTables& ft = t->f[f];
-        const int words = minor_desc_words(ft.n);
-        std::vector<uint64_t> desc(ft.minor_row.size() * size_t(words));
-        for (size_t m = 0; m < ft.minor_row.size(); ++m)
-            pack_minor_desc(ft.n, nibbles_of_mask(ft.rows[size_t(ft.minor_row[m])]), nibbles_of_mask(ft.cols[size_t(ft.minor_col[m])]),
-                            desc.data() + m * size_t(words));
+        if (ft.minor_row.size() >= (size_t(1) << 31)) { set_error("more than 2^31 unique minors"); return WICK_ERR_UNSUPPORTED; }
+        const std::vector<uint64_t> desc = build_minor_descs(ft);
         o_desc[f] = bb.add(desc.data(), desc.size() * 8);
     }
     size_t o_sp = 0, o_srd = 0, o_sc = 0, o_qp = 0, o_qcu = 0, o_qc = 0;
@@ -845,7 +889,7 @@ extern "C" int wick_minor_dets(const void* P_dev, int64_t n_sites, int n, const 
                 rw |= uint64_t(rows[(m0 + m) * n + i]) << (4 * i);
                 cw |= uint64_t(cols[(m0 + m) * n + i]) << (4 * i);
             }
-            pack_minor_desc(n, rw, cw, desc.data() + size_t(m) * size_t(words));
+            pack_minor_desc(n, rw, cw, uint32_t(m), false, desc.data() + size_t(m) * size_t(words));
         }
         WICK_CUDA_M(cudaMemcpyAsync(d_desc, desc.data(), size_t(nm) * size_t(words) * 8, cudaMemcpyHostToDevice, stream));
         double2* out = static_cast<double2*>(out_dev) + m0 * n_sites;

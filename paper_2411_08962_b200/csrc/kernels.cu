@@ -296,8 +296,12 @@ template <int N> struct MinorCfg {
 };
 
 // Minor descriptor (built on the host, contract.cu: pack_minor_desc): the row and column indices as
-// 4-bit fields, ascending.  n <= 8: one 64-bit word (rows in the low half, columns in the high half);
-// n >= 9: two 64-bit words (rows, columns).  One load per minor, no dependent second load.
+// 4-bit fields in PROCESSING order.  n <= 8: one 64-bit word (rows in the low half, columns in the high half),
+// ascending tuples, result stored at the descriptor's own position.  n >= 9: two 64-bit words
+//   w0 = rows (48 bits) | output minor id, low 16 bits;   w1 = columns (48 bits) | output id, high 15 bits | sign
+// where the columns may be listed descending (sign = parity of the reversal) so that tuples that differ in their
+// SMALL indices share leading columns too, and the descriptors are sorted for sharing, not by minor id.
+// One load per minor, no dependent second load.
 template <int N> struct Desc {
     static constexpr int kWords = (N <= 8) ? 1 : 2;
     unsigned long long w[kWords];
@@ -307,8 +311,14 @@ template <int N> struct Desc {
         else { const ulonglong2 v = __ldg(reinterpret_cast<const ulonglong2*>(tab) + m); d.w[0] = v.x; d.w[1] = v.y; }
         return d;
     }
-    __device__ __forceinline__ unsigned long long rows_bits() const { return kWords == 1 ? (w[0] & 0xffffffffull) : w[0]; }
-    __device__ __forceinline__ unsigned long long cols_bits() const { return kWords == 1 ? (w[0] >> 32) : w[kWords - 1]; }
+    __device__ __forceinline__ unsigned long long rows_bits() const { return kWords == 1 ? (w[0] & 0xffffffffull) : (w[0] & 0xffffffffffffull); }
+    __device__ __forceinline__ unsigned long long cols_bits() const { return kWords == 1 ? (w[0] >> 32) : (w[kWords - 1] & 0xffffffffffffull); }
+    // where the determinant goes (m = position of the descriptor) and whether it is negated
+    __device__ __forceinline__ int out_index(int m) const {
+        if constexpr (kWords == 1) return m;
+        else return int(w[0] >> 48) | (int((w[kWords - 1] >> 48) & 0x7fffull) << 16);
+    }
+    __device__ __forceinline__ bool negate() const { return kWords == 1 ? false : (w[kWords - 1] >> 63) != 0; }
     __device__ __forceinline__ uint32_t row(int i) const {
         if constexpr (kWords == 1) return (uint32_t(w[0]) >> (4 * i)) & 15u;
         else return uint32_t(w[0] >> (4 * i)) & 15u;
@@ -403,7 +413,7 @@ minors_kernel(const c128* __restrict__ P, int64_t st0, int64_t n_st_total, int S
             if (new_pair || (diff & kLead3) != 0) lu.third_column(tb, Ls, dc.col(K + 2) * kColStep);
             const c128 det = lu.finish(tb, Ls, dc.col(K + 3) * kColStep);
             prow = rws; pcol = dc.cols_bits();
-            if (valid) outp[int64_t(m) * S_b] = det;
+            if (valid) outp[int64_t(dc.out_index(m)) * S_b] = dc.negate() ? make_double2(-det.x, -det.y) : det;
         }
     }
 }

@@ -150,6 +150,25 @@ def test_shrunken_lattice_full_term_list(cfg, cuda_device):
         _check_C(Cf.cpu().numpy(), Cr, sabs.sum(axis=1))
 
 
+@pytest.mark.parametrize("n_u,n_d", [(9, 12), (10, 9), (11, 8), (7, 5)])
+def test_generic_lists_of_large_minors(n_u, n_d, cuda_device):
+    """Random term lists with 9..12-index tuples: the library walks such minors in its own order (column tuples that
+    miss only small indices are processed with descending columns and a parity sign, contract.cu: build_minor_descs);
+    the contraction must not depend on that."""
+    L, T, mom = 2, 2, [(0, 0, 0), (1, 0, 1)]
+    U, D = make_propagators_numpy(900 + n_u, L, T)
+    lst = make_random_term_list(77 + n_d, n_u, n_d, 300)
+    t = wk.build_terms_from_list(*lst)
+    Cg, sg = wk.contract(_dev(U, cuda_device), _dev(D, cuda_device), t, mom, L, T, want_sigma=True)
+    sg = sg.cpu().numpy()
+    sr, sabs = np.zeros((T, L ** 3), complex), np.zeros((T, L ** 3))
+    for tt in range(T):
+        for x in range(L ** 3):
+            sr[tt, x], sabs[tt, x] = wo.site_terms_value(U[tt, x], D[tt, x], *lst)
+    assert np.all(np.abs(sg - sr) <= REL_TOL * sabs), (np.abs(sg - sr) / sabs).max()
+    _check_C(Cg.cpu().numpy(), wo.reduce_sites(sr, mom, L), sabs.sum(axis=1))
+
+
 # ---------------------------------------------------------------------------------------------
 # BASELINE's full sizes: sampled sites + device reduction + structure
 # ---------------------------------------------------------------------------------------------
