@@ -43,34 +43,26 @@ def flops_lu(n: int) -> float:
         return 220.0
     return 8.0 * (n - 1) * n * (2 * n - 1) / 6 + 6.0 * n * (n - 1) / 2 + 15.0 * (n - 1) + 3.0 * (n * (n + 1) / 2 - 1)
 
-def executed_flops_per_site(n: int, rows: np.ndarray, cols: np.ndarray, minor_row: np.ndarray, minor_col: np.ndarray) -> float:
-    """Flops the minors kernel actually executes per site for one flavour: the pivoted-LU
-    state is kept across consecutive minors that share the row tuple and leading columns, so the K = n-4
-    pivot steps run once per (row tuple, first K columns), the 2x2 / 3x3 minors of the Schur complement
-    once per (.., first K+2 / K+3 columns), and only the last column once per minor."""
-    nm = len(minor_row)
+def executed_flops_per_site(n: int, row_in_order: np.ndarray, cols_in_order: np.ndarray) -> float:
+    """Flops the minors kernel actually executes per site for one flavour, from the order in which it
+    walks the minors (Terms.minor_order): the pivoted-LU state is kept across consecutive minors that share the row
+    tuple and leading columns, so the K = n-4 pivot steps run once per (row tuple, first K columns), the 2x2 / 3x3
+    minors of the Schur complement once per (.., first K+2 / K+3 columns), and only the last column once per minor."""
+    nm = len(row_in_order)
     if n <= 2 or nm == 0:
         return nm * flops_lu(n)
-    c = cols[minor_col].astype(np.int64)                           # [nm][n] column tuples in minor order
-    if n >= 9:
-        # the library's processing order for large minors (contract.cu: build_minor_descs): column tuples that miss only
-        # small indices (< 6) are walked with descending columns, each group sorted by its processing order
-        descending = np.array([set(range(6, 12)) <= set(t) and len(t) < 12 for t in c.tolist()])
-        proc = np.where(descending[:, None], c[:, ::-1], c)
-        keys = [proc[:, k] for k in range(n - 1, -1, -1)] + [descending.astype(np.int64), minor_row.astype(np.int64)]
-        order = np.lexsort(keys)
-        c, minor_row = proc[order], minor_row[order]
-    same_row = minor_row[1:] == minor_row[:-1]
+    c = cols_in_order.astype(np.int64)
+    same_row = row_in_order[1:] == row_in_order[:-1]
+
+    def same_lead(k):
+        return same_row & np.all(c[1:, :k] == c[:-1, :k], axis=1)
     if n == 3:                                                     # cofactors of the last column per (rows, b0, b1)
-        n_pair = 1 + int(np.count_nonzero(~(same_row & np.all(c[1:, :2] == c[:-1, :2], axis=1))))
-        return n_pair * 42.0 + nm * 22.0
+        return (1 + int(np.count_nonzero(~same_lead(2)))) * 42.0 + nm * 22.0
     K = n - 4
     f_col = 8.0 * sum(n - 1 - i for i in range(K))
     f_start = sum(8.0 * sum(n - 1 - i for i in range(J)) + (n - J) + 14.0 + 6.0 * (n - 1 - J) + (6.0 if J else 0.0)
                   for J in range(K))
     f_pair, f_third, f_finish = 2 * f_col + 84.0, f_col + 88.0, f_col + 36.0
-    def same_lead(k):
-        return same_row & np.all(c[1:, :k] == c[:-1, :k], axis=1)
     n_fresh = 1 + int(np.count_nonzero(~same_lead(K)))
     n_pair = 1 + int(np.count_nonzero(~same_lead(K + 2)))
     n_third = 1 + int(np.count_nonzero(~same_lead(K + 3)))
@@ -300,10 +292,9 @@ def main():
     ms_project = prof["project"][0] / args.steps
     n_minor_launches = (prof["minors_u"][1] + prof["minors_d"][1]) // args.steps
     achieved_tf = flop_minors / (ms_minors * 1e-3) / 1e12
-    tu_rows, tu_cols, td_rows, td_cols = terms.tuples()
-    mu_row, mu_col, md_row, md_col = terms.minors()
-    exec_site = (executed_flops_per_site(info.n_u, tu_rows, tu_cols, mu_row, mu_col),
-                 executed_flops_per_site(info.n_d, td_rows, td_cols, md_row, md_col))
+    mu_row, _, md_row, _ = terms.minors()
+    ou, od = terms.minor_order(0), terms.minor_order(1)
+    exec_site = (executed_flops_per_site(info.n_u, mu_row[ou[0]], ou[1]), executed_flops_per_site(info.n_d, md_row[od[0]], od[1]))
     executed_tf = st_per_step * (exec_site[0] + d_runs * exec_site[1]) / (ms_minors * 1e-3) / 1e12
     traffic = None
     try:

@@ -119,6 +119,12 @@ int  wick_terms_export_terms(const wick_terms* terms, int64_t first, int64_t cou
  * Returns WICK_ERR_UNSUPPORTED if !is_outer_product. */
 int  wick_terms_export_factors(const wick_terms* terms, int32_t* sink_ru, int32_t* sink_rd, double* sink_c_reim,
                                int32_t* src_cu, int32_t* src_cd, double* src_c_reim);
+/* The order in which the minors kernel walks one flavour's unique minors (flavour 0 = u, 1 = d) and the order in which
+ * it takes each minor's columns (consecutive minors share their row tuple and leading columns; for
+ * n >= 9 the column tuples are clustered by a common set of n-4 leading columns).  minor_id int32 [n_minors]: position ->
+ * unique-minor id; proc_cols uint8 [n_minors][n]; negate uint8 [n_minors]: 1 if that column order is an odd
+ * permutation of the ascending tuple (the kernel negates the result).  Any pointer may be NULL. */
+int  wick_terms_export_minor_order(const wick_terms* terms, int flavour, int32_t* minor_id, uint8_t* proc_cols, uint8_t* negate);
 /* Host-only self-check of the schedule of the staged factorised reduction (reduce_staged_kernel) for
  * n_bins CTA bins: every (u-row tuple, d-column tuple) pair of the factorised sum (PAPER.md Eq. A1-A5 regrouped) is
  * covered by exactly one batch, every batch fits the shared-memory capacities and every coefficient entry points

@@ -24,7 +24,7 @@ CONTRACT_COMPLEX_COEFFS = 4
 EXPORTED_SYMBOLS = (
     "wick_build_terms", "wick_build_terms_from_list", "wick_terms_get_info", "wick_terms_export_tuples",
     "wick_terms_export_minors", "wick_terms_export_terms", "wick_terms_export_factors",
-    "wick_terms_staged_schedule_check", "wick_terms_free",
+    "wick_terms_staged_schedule_check", "wick_terms_export_minor_order", "wick_terms_free",
     "wick_contract_min_workspace_bytes", "wick_contract_workspace_bytes", "wick_contract",
     "wick_contract_host", "wick_release_cached_buffers", "wick_minor_dets", "wick_launch_count", "wick_launch_count_reset",
     "wick_last_error", "wick_version", "wick_profile_enable", "wick_profile_read", "wick_measure_fp64_peak",
@@ -75,6 +75,7 @@ def load_library():
     lib.wick_terms_export_terms.argtypes = [vp, i64, i64, vp, vp, vp]
     lib.wick_terms_export_factors.argtypes = [vp, vp, vp, vp, vp, vp, vp]
     lib.wick_terms_staged_schedule_check.argtypes = [vp, C.c_int, vp, vp, vp, vp]
+    lib.wick_terms_export_minor_order.argtypes = [vp, C.c_int, vp, vp, vp]
     lib.wick_terms_free.argtypes = [vp]
     lib.wick_terms_free.restype = None
     lib.wick_release_cached_buffers.restype = None
@@ -150,6 +151,16 @@ class Terms:
         _check(_lib.wick_terms_export_factors(self._h, _np_ptr(sru), _np_ptr(srd), _np_ptr(sc),
                                               _np_ptr(qcu), _np_ptr(qcd), _np_ptr(qc)), "wick_terms_export_factors")
         return sru, srd, sc, qcu, qcd, qc
+
+    def minor_order(self, flavour: int):
+        """(minor_id [n_minors], proc_cols [n_minors][n], negate [n_minors]): the order in which the minors kernel walks this
+        flavour's unique minors and takes their columns (flavour 0 = u, 1 = d)."""
+        i = self.info
+        nm, n = (i.n_minors_u, i.n_u) if flavour == 0 else (i.n_minors_d, i.n_d)
+        mid, pc, neg = np.zeros(nm, np.int32), np.zeros((nm, n), np.uint8), np.zeros(nm, np.uint8)
+        _check(_lib.wick_terms_export_minor_order(self._h, flavour, _np_ptr(mid), _np_ptr(pc), _np_ptr(neg)),
+               "wick_terms_export_minor_order")
+        return mid, pc, neg
 
     def staged_schedule_check(self, n_bins: int):
         """Host-only self-check of the staged-reduction schedule; returns (batches, pairs covered, max MD block, max rows)."""

@@ -65,46 +65,79 @@ void pack_minor_desc(int n, uint64_t rows, uint64_t cols, uint32_t out_id, bool 
     }
 }
 
-// nibble list reversed (n fields)
-uint64_t reverse_nibbles(uint64_t w, int n) {
-    uint64_t r = 0;
-    for (int k = 0; k < n; ++k) r |= ((w >> (4 * k)) & 15u) << (4 * (n - 1 - k));
-    return r;
+// Processing order of one flavour's minors (what minors_kernel walks, position by position).
+struct MinorOrder {
+    std::vector<uint32_t> minor;      // position -> unique-minor id
+    std::vector<uint64_t> cols;       // position -> column indices as 4-bit fields in processing order
+    std::vector<uint8_t> negate;      // position -> the processing order is an odd permutation of the ascending tuple
+};
+
+// n <= 8: minor order (row tuple by row tuple, column tuples lexicographic: consecutive minors share leading columns).
+// n >= 9: the K = n-4 pivot steps dominate, so the column tuples are clustered by a shared set of K LEADING columns:
+// greedily take the K-subset contained in most of the remaining tuples, put it first (ascending) and the rest of each
+// tuple behind it (ascending); minors are sorted by (row tuple, cluster, rest).  The determinant with permuted columns
+// is the determinant times the parity of the permutation, kept as a sign bit of the descriptor.
+MinorOrder build_minor_order(const FlavourTables& ft) {
+    const int n = ft.n;
+    const size_t nm = ft.minor_row.size();
+    MinorOrder o;
+    o.minor.resize(nm); o.cols.resize(nm); o.negate.assign(nm, 0);
+    if (n <= 8) {
+        for (size_t m = 0; m < nm; ++m) { o.minor[m] = uint32_t(m); o.cols[m] = nibbles_of_mask(ft.cols[size_t(ft.minor_col[m])]); }
+        return o;
+    }
+    const int K = n - 4;
+    const size_t nc = ft.cols.size();
+    std::vector<int> cluster(nc, -1);
+    std::vector<uint64_t> proc(nc, 0);
+    std::vector<uint8_t> odd(nc, 0);
+    size_t left = nc;
+    for (int cl = 0; left > 0; ++cl) {
+        std::map<uint16_t, int> count;                                  // K-subset (mask) -> number of unassigned tuples containing it
+        for (size_t c = 0; c < nc; ++c) {
+            if (cluster[c] >= 0) continue;
+            const uint16_t full = ft.cols[c];
+            for (uint16_t sub = full;; sub = uint16_t((sub - 1) & full)) {   // all submasks of the tuple
+                if (__builtin_popcount(sub) == K) count[sub]++;
+                if (sub == 0) break;
+            }
+        }
+        uint16_t best = 0; int best_n = -1;
+        for (const auto& kv : count)                                    // most tuples; ties: the smallest mask value
+            if (kv.second > best_n) { best = kv.first; best_n = kv.second; }
+        for (size_t c = 0; c < nc; ++c) {
+            if (cluster[c] >= 0 || (ft.cols[c] & best) != best) continue;
+            cluster[c] = cl; --left;
+            const uint64_t lead = nibbles_of_mask(best), rest = nibbles_of_mask(uint16_t(ft.cols[c] & ~best));
+            proc[c] = lead | (rest << (4 * K));
+            int inv = 0;                                                // inversions of the processing order
+            for (int i = 0; i < n; ++i)
+                for (int j = i + 1; j < n; ++j) inv += ((proc[c] >> (4 * i)) & 15u) > ((proc[c] >> (4 * j)) & 15u);
+            odd[c] = uint8_t(inv & 1);
+        }
+    }
+    auto tuple_key = [n](uint64_t w) { uint64_t k = 0; for (int i = 0; i < n; ++i) k = (k << 4) | ((w >> (4 * i)) & 15u); return k; };
+    std::vector<uint32_t> idx(nm);
+    for (size_t m = 0; m < nm; ++m) idx[m] = uint32_t(m);
+    std::stable_sort(idx.begin(), idx.end(), [&](uint32_t a, uint32_t b) {
+        if (ft.minor_row[a] != ft.minor_row[b]) return ft.minor_row[a] < ft.minor_row[b];
+        const size_t ca = size_t(ft.minor_col[a]), cb = size_t(ft.minor_col[b]);
+        if (cluster[ca] != cluster[cb]) return cluster[ca] < cluster[cb];
+        return tuple_key(proc[ca]) < tuple_key(proc[cb]);
+    });
+    for (size_t k = 0; k < nm; ++k) {
+        const size_t c = size_t(ft.minor_col[idx[k]]);
+        o.minor[k] = idx[k]; o.cols[k] = proc[c]; o.negate[k] = odd[c];
+    }
+    return o;
 }
 
-// Descriptor list of one flavour in processing order.  n <= 8: minor order (row tuple by row tuple, column tuples
-// lexicographic: consecutive minors share leading columns).  n >= 9: within a row tuple, column tuples whose missing
-// indices are all small (< 6) are processed with DESCENDING columns, so that they share their leading (large) columns
-// the way the others share their small ones; each group is sorted by its processing order.  det with reversed columns
-// = (-1)^(n(n-1)/2) det, folded into the descriptor's sign.
 std::vector<uint64_t> build_minor_descs(const FlavourTables& ft) {
-    const int n = ft.n, words = minor_desc_words(n);
-    const size_t nm = ft.minor_row.size();
-    std::vector<uint64_t> desc(nm * size_t(words));
-    if (words == 1) {
-        for (size_t m = 0; m < nm; ++m)
-            pack_minor_desc(n, nibbles_of_mask(ft.rows[size_t(ft.minor_row[m])]), nibbles_of_mask(ft.cols[size_t(ft.minor_col[m])]), 0, false,
-                            desc.data() + m);
-        return desc;
-    }
-    struct Key { int32_t row; int group; uint64_t cols; uint32_t m; };
-    std::vector<Key> keys(nm);
-    const bool rev_negates = ((n * (n - 1) / 2) & 1) != 0;
-    for (size_t m = 0; m < nm; ++m) {
-        const uint16_t cmask = ft.cols[size_t(ft.minor_col[m])];
-        const bool descending = (uint16_t(~cmask) & 0x0fc0u) == 0 && cmask != 0x0fffu;   // nothing missing among 6..11, something among 0..5
-        const uint64_t asc = nibbles_of_mask(cmask);
-        keys[m] = Key{ft.minor_row[m], descending ? 1 : 0, descending ? reverse_nibbles(asc, n) : asc, uint32_t(m)};
-    }
-    // sort by (row tuple, group, columns in processing order read as a tuple: first column most significant)
-    auto tuple_key = [n](uint64_t w) { uint64_t k = 0; for (int i = 0; i < n; ++i) k = (k << 4) | ((w >> (4 * i)) & 15u); return k; };
-    std::stable_sort(keys.begin(), keys.end(), [&](const Key& a, const Key& b) {
-        if (a.row != b.row) return a.row < b.row;
-        if (a.group != b.group) return a.group < b.group;
-        return tuple_key(a.cols) < tuple_key(b.cols);
-    });
-    for (size_t k = 0; k < nm; ++k)
-        pack_minor_desc(n, nibbles_of_mask(ft.rows[size_t(keys[k].row)]), keys[k].cols, keys[k].m, keys[k].group == 1 && rev_negates,
+    const int words = minor_desc_words(ft.n);
+    const MinorOrder o = build_minor_order(ft);
+    std::vector<uint64_t> desc(o.minor.size() * size_t(words));
+    for (size_t k = 0; k < o.minor.size(); ++k)
+        pack_minor_desc(ft.n, nibbles_of_mask(ft.rows[size_t(ft.minor_row[o.minor[k]])]), o.cols[k], o.minor[k], o.negate[k] != 0,
                         desc.data() + k * size_t(words));
     return desc;
 }
@@ -578,6 +611,19 @@ extern "C" void wick_terms_release_device(DeviceTables* d) {
     if (d->flat_blob) cudaFree(d->flat_blob);
     for (auto& kv : d->staged) cudaFree(kv.second.blob);
     *d = DeviceTables();
+}
+
+extern "C" int wick_terms_export_minor_order(const wick_terms* t, int flavour, int32_t* minor_id, uint8_t* proc_cols, uint8_t* negate) {
+    if (!t || (flavour != 0 && flavour != 1)) { set_error("wick_terms_export_minor_order: bad argument"); return WICK_ERR_ARG; }
+    const FlavourTables& ft = t->f[flavour];
+    MinorOrder o;
+    try { o = build_minor_order(ft); } catch (const std::bad_alloc&) { set_error("out of host memory"); return WICK_ERR_NOMEM; }
+    for (size_t k = 0; k < o.minor.size(); ++k) {
+        if (minor_id) minor_id[k] = int32_t(o.minor[k]);
+        if (negate) negate[k] = o.negate[k];
+        if (proc_cols) for (int i = 0; i < ft.n; ++i) proc_cols[k * size_t(ft.n) + size_t(i)] = uint8_t((o.cols[k] >> (4 * i)) & 15u);
+    }
+    return WICK_OK;
 }
 
 extern "C" int wick_terms_staged_schedule_check(const wick_terms* t, int n_bins, int64_t* n_batches_out, int64_t* n_pairs_out,

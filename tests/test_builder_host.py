@@ -225,3 +225,31 @@ def test_staged_schedule_rejects_generic_lists():
     t = wk.build_terms_from_list(*make_random_term_list(c.seed, c.n_u, c.n_d, c.n_random_terms))
     with pytest.raises(wk.WickError):
         t.staged_schedule_check(4)
+
+
+# ---------------------------------------------------------------------------------------------
+# order in which the minors kernel walks the unique minors (host logic of contract.cu)
+# ---------------------------------------------------------------------------------------------
+
+def _perm_is_odd(p):
+    p = list(p)
+    return sum(1 for i in range(len(p)) for j in range(i + 1, len(p)) if p[i] > p[j]) % 2 == 1
+
+
+@pytest.mark.parametrize("cfg", ["cfg1", "cfg2", "cfg3", "cfg4", "cfg4b"])
+def test_minor_order_is_a_signed_permutation(cfg):
+    c = CONFIGS[cfg]
+    t = (wk.build_terms_from_list(*make_random_term_list(c.seed, c.n_u, c.n_d, c.n_random_terms)) if c.random_list
+         else wk.build_terms(c.nucleus))
+    rows_cols = t.tuples()
+    minors = t.minors()
+    for fl in (0, 1):
+        mid, pc, neg = t.minor_order(fl)
+        cols, mcol, mrow = rows_cols[2 * fl + 1], minors[2 * fl + 1], minors[2 * fl]
+        assert sorted(mid.tolist()) == list(range(len(mid)))                 # every unique minor exactly once
+        asc = cols[mcol[mid]]
+        assert np.array_equal(np.sort(pc, axis=1), asc)                      # same index set, some order
+        assert [bool(x) for x in neg] == [_perm_is_odd(p) for p in pc.tolist()]
+        assert np.all(np.diff(mrow[mid]) >= 0)                               # row tuple by row tuple
+        if pc.shape[1] <= 8:                                                 # small minors: minor order, ascending columns
+            assert np.array_equal(mid, np.arange(len(mid))) and not neg.any()
