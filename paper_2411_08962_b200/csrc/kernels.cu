@@ -630,6 +630,86 @@ __device__ __forceinline__ c128 staged_rows(const c128* MUs, const c128* MDl, c1
     return acc;
 }
 
+// Dense variant for pieces whose source block is (nearly) full, real coefficients: B[cu][cd] sits in shared memory as
+// a dense n_cu x n_cd matrix (row stride = n_cd rounded up to 2 doubles), and
+//   Q[cd] = sum_cu B[cu][cd] MU[ru, cu]
+// is accumulated straight from the row's registers: no per-entry record, offset or row-buffer traffic (a 15 x 15 block
+// has 225 entries: one broadcast LDS.128 feeds 4 DFMA here, against two loads and an address per 2 DFMA there).
+template <int NCU, int NCD>
+__device__ __forceinline__ c128 staged_rows_dense(const c128* MUs, const c128* MDl, int warp, int n_rows, int n_cu,
+                                                  const int* rowoff, const int* cuoff, const int* sinkp, const c128* sinkc,
+                                                  const double* Bd) {
+    constexpr int NCDP = (NCD + 1) & ~1;
+    c128 acc = make_double2(0.0, 0.0);
+    c128 X[NCU];
+#pragma unroll
+    for (int c = 0; c < NCU; ++c) X[c] = make_double2(0.0, 0.0);
+    int r = warp;
+    if (r < n_rows) {                                                    // first row: global -> registers
+        const c128* src = MUs + rowoff[r];
+#pragma unroll
+        for (int c = 0; c < NCU; ++c)
+            if (c < n_cu) X[c] = __ldg(src + cuoff[c]);
+    }
+    for (; r < n_rows; r += STG_W) {
+        c128 Q[NCDP];
+#pragma unroll
+        for (int c = 0; c < NCDP; ++c) Q[c] = make_double2(0.0, 0.0);
+#pragma unroll
+        for (int c = 0; c < NCU; ++c) {
+            if (c < n_cu) {
+                const c128 x = X[c];
+                const double2* bp = reinterpret_cast<const double2*>(Bd + c * NCDP);
+#pragma unroll
+                for (int h = 0; h < NCDP / 2; ++h) {
+                    const double2 b = bp[h];
+                    Q[2 * h].x = fma(b.x, x.x, Q[2 * h].x); Q[2 * h].y = fma(b.x, x.y, Q[2 * h].y);
+                    if (2 * h + 1 < NCD) { Q[2 * h + 1].x = fma(b.y, x.x, Q[2 * h + 1].x); Q[2 * h + 1].y = fma(b.y, x.y, Q[2 * h + 1].y); }
+                }
+            }
+        }
+        if (r + STG_W < n_rows) {                                        // next row: in flight during the rest of this row
+            const c128* src = MUs + rowoff[r + STG_W];
+#pragma unroll
+            for (int c = 0; c < NCU; ++c)
+                if (c < n_cu) X[c] = __ldg(src + cuoff[c]);
+        }
+        c128 P[NCD];
+#pragma unroll
+        for (int c = 0; c < NCD; ++c) P[c] = make_double2(0.0, 0.0);
+        const int i0 = sinkp[r], i1 = sinkp[r + 1];
+#pragma unroll 2
+        for (int i = i0; i < i1; ++i) {
+            const c128 a = sinkc[i];
+            const c128* md = MDl + __double2loint(a.y);
+#pragma unroll
+            for (int c = 0; c < NCD; ++c) {
+                const c128 v = md[c * GROUP];
+                P[c].x = fma(a.x, v.x, P[c].x); P[c].y = fma(a.x, v.y, P[c].y);
+            }
+        }
+#pragma unroll
+        for (int c = 0; c < NCD; ++c) acc = cfma(Q[c], P[c], acc);
+    }
+    return acc;
+}
+
+template <int NCU>
+__device__ __forceinline__ c128 staged_rows_dense_ncd(const c128* MUs, const c128* MDl, int warp, int n_rows, int n_cu, int n_cd,
+                                                      const int* rowoff, const int* cuoff, const int* sinkp, const c128* sinkc,
+                                                      const double* Bd) {
+#define WICK_STG_CALL(NCD) staged_rows_dense<NCU, NCD>(MUs, MDl, warp, n_rows, n_cu, rowoff, cuoff, sinkp, sinkc, Bd)
+    switch (n_cd) {
+        case 1: return WICK_STG_CALL(1);
+        case 2: return WICK_STG_CALL(2);
+        case 3: return WICK_STG_CALL(3);
+        case 4: return WICK_STG_CALL(4);
+        case 5: return WICK_STG_CALL(5);
+        default: return WICK_STG_CALL(6);
+    }
+#undef WICK_STG_CALL
+}
+
 template <int NCU, bool REAL>
 __device__ __forceinline__ c128 staged_rows_ncd(const c128* MUs, const c128* MDl, c128* row, int warp, int n_rows, int n_cu, int n_cd,
                                                 const int* rowoff, const int* cuoff, const int* sinkp, const c128* sinkc,
@@ -686,7 +766,7 @@ reduce_staged_kernel(const c128* __restrict__ MU, const c128* __restrict__ MD, i
             const c128 cf = __ldg(st.sink_c + sp0 + e);
             const int off = (__ldg(st.sink_rdpos + sp0 + e) - rd_a) * n_cd * GROUP;
             sinkc[e] = REAL ? make_double2(cf.x, __hiloint2double(0, off)) : cf;
-            sinko[e] = off;
+            if (!REAL) sinko[e] = off;
         }
         for (int r = threadIdx.x; r <= n_rows; r += STG_THREADS) {
             sinkp[r] = __ldg(st.sink_ptr + ru_a + r) - sp0;
@@ -697,7 +777,21 @@ reduce_staged_kernel(const c128* __restrict__ MU, const c128* __restrict__ MD, i
             const c128 cf = __ldg(st.src_c + q0 + e);
             const int off = (__ldg(st.src_cupos + q0 + e) - cu_a) * GROUP;
             srcc[e] = REAL ? make_double2(cf.x, __hiloint2double(0, off)) : cf;
-            srco[e] = off;
+            if (!REAL) srco[e] = off;
+        }
+        // (nearly) full source block with real coefficients: dense B[cu][cd] in the (then unused) offset buffer
+        const bool dense = REAL && n_cu > 4 && 2 * (q1 - q0) >= n_cu * n_cd;
+        if (dense) {
+            const int ncdp = (n_cd + 1) & ~1;
+            double* Bd = reinterpret_cast<double*>(sinko);
+            for (int e = threadIdx.x; e < n_cu * ncdp; e += STG_THREADS) {
+                const int cul = e / ncdp, cdi = e - cul * ncdp;
+                double v = 0.0;
+                if (cdi < n_cd)
+                    for (int j = __ldg(st.src_ptr + cd_a + cdi); j < __ldg(st.src_ptr + cd_a + cdi + 1); ++j)
+                        if (__ldg(st.src_cupos + j) - cu_a == cul) v += __ldg(st.src_c + j).x;
+                Bd[e] = v;
+            }
         }
         if (threadIdx.x <= n_cd) srcp[threadIdx.x] = __ldg(st.src_ptr + cd_a + threadIdx.x) - q0;
         if (threadIdx.x >= 32 && threadIdx.x < 32 + n_cu) cuoff[threadIdx.x - 32] = __ldg(st.cu_list + cu_a + threadIdx.x - 32) * S_b;
@@ -705,7 +799,11 @@ reduce_staged_kernel(const c128* __restrict__ MU, const c128* __restrict__ MD, i
         __syncthreads();
 #define WICK_STG_CALL(NCU) staged_rows_ncd<NCU, REAL>(MUs, MDl, row, warp, n_rows, n_cu, n_cd, rowoff, cuoff, sinkp, sinkc, sinko, srcp, srcc, srco)
         c128 v;
-        if (n_cu <= 2) v = WICK_STG_CALL(2);
+        if (dense) {
+            const double* Bd = reinterpret_cast<const double*>(sinko);
+            if (n_cu <= 8) v = staged_rows_dense_ncd<8>(MUs, MDl, warp, n_rows, n_cu, n_cd, rowoff, cuoff, sinkp, sinkc, Bd);
+            else v = staged_rows_dense_ncd<STG_ROW_CAP>(MUs, MDl, warp, n_rows, n_cu, n_cd, rowoff, cuoff, sinkp, sinkc, Bd);
+        } else if (n_cu <= 2) v = WICK_STG_CALL(2);
         else if (n_cu <= 4) v = WICK_STG_CALL(4);
         else if (n_cu <= 8) v = WICK_STG_CALL(8);
         else v = WICK_STG_CALL(STG_ROW_CAP);
