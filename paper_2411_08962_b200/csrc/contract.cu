@@ -326,14 +326,19 @@ int upload_tables(const wick_terms* t, cudaStream_t stream) {
 
 struct StagedHost {
     bool ok = false;                                              // false: a block exceeds the staging capacities
+    bool real = false;                                            // all factor coefficients real: dense-B kernel, larger MD block
     std::vector<int32_t> sink_ptr, sink_rdpos, src_ptr, src_cupos, ru_list, rd_list, cu_list, cd_list, bin_ptr;
     std::vector<double> sink_c, src_c;
     std::vector<StagedBatch> batches;
 };
 
 // Host part of the staged schedule (no CUDA call): also what wick_terms_staged_schedule_check verifies.
-StagedHost build_staged_host(const wick_terms* t, int n_bins) {
+StagedHost build_staged_host(const wick_terms* t, int n_bins, bool force_complex) {
     StagedHost h;
+    h.real = !force_complex;
+    for (const FactorTerm& f : t->sink) if (f.c.imag() != 0.0) h.real = false;
+    for (const FactorTerm& f : t->source) if (f.c.imag() != 0.0) h.real = false;
+    const int md_cap = stg_md_cap(h.real);
     const int nru = int(t->f[0].rows.size()), nrd = int(t->f[1].rows.size());
     const int ncu = int(t->f[0].cols.size()), ncd = int(t->f[1].cols.size());
     const Components cs = factor_components(nru, nrd, t->sink);
@@ -365,7 +370,7 @@ StagedHost build_staged_host(const wick_terms* t, int n_bins) {
     int max_rd = 1, max_cu = 1;
     for (int k = 0; k < cs.n; ++k) max_rd = std::max(max_rd, rd_ptr[size_t(k) + 1] - rd_ptr[size_t(k)]);
     for (int k = 0; k < cq.n; ++k) max_cu = std::max(max_cu, cu_ptr[size_t(k) + 1] - cu_ptr[size_t(k)]);
-    if (max_rd > STG_MD_CAP || max_cu > STG_ROW_CAP || cs.n == 0 || cq.n == 0) return h;
+    if (max_rd > md_cap || max_cu > STG_ROW_CAP || cs.n == 0 || cq.n == 0) return h;
 
     // coefficient lists regrouped by list position, so that a batch's entries are contiguous:
     // sink entries by position of ru in ru_list, source entries by position of cd in cd_list
@@ -404,7 +409,7 @@ StagedHost build_staged_host(const wick_terms* t, int n_bins) {
     // sink block; neighbouring small blocks share a piece (their union is just a block-diagonal source block)
     struct Piece { int ca, cb, cuA, cuB; };
     std::vector<Piece> pieces;
-    const int piece_max = std::max(1, std::min(STG_NCD_CAP, STG_MD_CAP / max_rd));
+    const int piece_max = std::max(1, std::min(STG_NCD_CAP, md_cap / max_rd));
     for (int kp = 0; kp < cq.n;) {
         const int cdA = cd_ptr[size_t(kp)], cdB = cd_ptr[size_t(kp) + 1];
         const int cuA = cu_ptr[size_t(kp)];
@@ -438,7 +443,7 @@ StagedHost build_staged_host(const wick_terms* t, int n_bins) {
                     const int n_rd2 = n_rd + rd_ptr[size_t(kb) + 1] - rd_ptr[size_t(kb)];
                     const int rows2 = ru_ptr[size_t(kb) + 1] - ru_ptr[size_t(ka)];
                     const int ent2 = sink_ptr[size_t(ru_ptr[size_t(kb) + 1])] - sink_ptr[size_t(ru_ptr[size_t(ka)])];
-                    if (kb > ka && (n_rd2 * n_cd > STG_MD_CAP || rows2 > STG_ROWS_CAP || ent2 > STG_SINK_CAP)) break;
+                    if (kb > ka && (n_rd2 * n_cd > md_cap || rows2 > STG_ROWS_CAP || ent2 > STG_SINK_CAP)) break;
                     n_rd = n_rd2;
                     ++kb;
                 }
@@ -483,7 +488,7 @@ StagedHost build_staged_host(const wick_terms* t, int n_bins) {
 // batches are assigned to n_bins CTAs by longest-processing-time, each bin keeps a fixed order.
 // Returns 1 and fills `out` when the list is eligible, 0 when a block is too large (caller falls back
 // to reduce_outer_kernel), negative on error.
-int ensure_staged(const wick_terms* t, int n_bins, cudaStream_t stream, StagedTables* out) {
+int ensure_staged(const wick_terms* t, int n_bins, bool force_complex, cudaStream_t stream, StagedTables* out) {
     std::lock_guard<std::mutex> lock(t->mu);
     DeviceTables& d = t->dev;
     if (d.staged_state < 0) return 0;
@@ -491,18 +496,17 @@ int ensure_staged(const wick_terms* t, int n_bins, cudaStream_t stream, StagedTa
     const int ncu = int(t->f[0].cols.size()), ncd = int(t->f[1].cols.size());
     auto fill = [&](const StagedDev& sd) {
         out->n_cols_u = ncu; out->n_cols_d = ncd; out->n_bins = sd.n_bins;
-        out->real_coeffs = true;
-        for (const FactorTerm& f : t->sink) if (f.c.imag() != 0.0) out->real_coeffs = false;
-        for (const FactorTerm& f : t->source) if (f.c.imag() != 0.0) out->real_coeffs = false;
+        out->real_coeffs = sd.real;
         out->sink_ptr = sd.sink_ptr; out->sink_rdpos = sd.sink_rdpos; out->sink_c = reinterpret_cast<const double2*>(sd.sink_c);
         out->src_ptr = sd.src_ptr; out->src_cupos = sd.src_cupos; out->src_c = reinterpret_cast<const double2*>(sd.src_c);
         out->ru_list = sd.ru_list; out->rd_list = sd.rd_list; out->cu_list = sd.cu_list; out->cd_list = sd.cd_list;
         out->bin_ptr = sd.bin_ptr; out->batches = static_cast<const StagedBatch*>(sd.batches);
     };
-    auto hit = d.staged.find(n_bins);
+    const int key = 2 * n_bins + (force_complex ? 1 : 0);          // schedules differ: the real-coefficient kernel stages larger MD blocks
+    auto hit = d.staged.find(key);
     if (hit != d.staged.end()) { fill(hit->second); return 1; }
 
-    const StagedHost h = build_staged_host(t, n_bins);
+    const StagedHost h = build_staged_host(t, n_bins, force_complex);
     if (!h.ok) { d.staged_state = -1; return 0; }
     d.staged_state = 1;
     const std::vector<int32_t>&sink_rdpos = h.sink_rdpos, &src_cupos = h.src_cupos, &sink_ptr = h.sink_ptr, &src_ptr = h.src_ptr;
@@ -523,14 +527,14 @@ int ensure_staged(const wick_terms* t, int n_bins, cudaStream_t stream, StagedTa
     if (e != cudaSuccess) { cudaFree(blob); set_error(std::string("staged schedule upload: ") + cudaGetErrorString(e)); return WICK_ERR_CUDA; }
     unsigned char* b = static_cast<unsigned char*>(blob);
     StagedDev sd;
-    sd.blob = blob; sd.n_bins = n_bins;
+    sd.blob = blob; sd.n_bins = n_bins; sd.real = h.real;
     sd.sink_rdpos = reinterpret_cast<const int32_t*>(b + o_srp); sd.src_cupos = reinterpret_cast<const int32_t*>(b + o_scp);
     sd.sink_ptr = reinterpret_cast<const int32_t*>(b + o_sp); sd.src_ptr = reinterpret_cast<const int32_t*>(b + o_qp);
     sd.sink_c = reinterpret_cast<const double*>(b + o_sc); sd.src_c = reinterpret_cast<const double*>(b + o_qc);
     sd.ru_list = reinterpret_cast<const int32_t*>(b + o_ru); sd.rd_list = reinterpret_cast<const int32_t*>(b + o_rd);
     sd.cu_list = reinterpret_cast<const int32_t*>(b + o_cu); sd.cd_list = reinterpret_cast<const int32_t*>(b + o_cd);
     sd.bin_ptr = reinterpret_cast<const int32_t*>(b + o_bp); sd.batches = b + o_ba;
-    d.staged[n_bins] = sd;
+    d.staged[key] = sd;
     fill(sd);
     return 1;
 }
@@ -631,7 +635,7 @@ extern "C" int wick_terms_staged_schedule_check(const wick_terms* t, int n_bins,
     if (!t || n_bins < 1) { set_error("wick_terms_staged_schedule_check: bad argument"); return WICK_ERR_ARG; }
     if (!t->outer) { set_error("not an outer-product term list"); return WICK_ERR_UNSUPPORTED; }
     StagedHost h;
-    try { h = build_staged_host(t, n_bins); } catch (const std::bad_alloc&) { set_error("out of host memory"); return WICK_ERR_NOMEM; }
+    try { h = build_staged_host(t, n_bins, false); } catch (const std::bad_alloc&) { set_error("out of host memory"); return WICK_ERR_NOMEM; }
     if (!h.ok) { set_error("a block of the factor lists exceeds the staging capacities (the unstaged kernel is used)"); return WICK_ERR_UNSUPPORTED; }
     const size_t nru = t->f[0].rows.size(), ncd = t->f[1].cols.size();
     std::vector<uint8_t> covered(nru * ncd, 0);
@@ -642,7 +646,7 @@ extern "C" int wick_terms_staged_schedule_check(const wick_terms* t, int n_bins,
     for (const StagedBatch& b : h.batches) {
         const int n_cd = b.cd_b - b.cd_a, n_cu = b.cu_b - b.cu_a, n_rd = b.rd_b - b.rd_a, rows = b.ru_b - b.ru_a;
         if (n_cd < 1 || n_cd > STG_NCD_CAP || n_cu < 1 || n_cu > STG_ROW_CAP || rows < 1 || rows > STG_ROWS_CAP ||
-            int64_t(n_rd) * n_cd > STG_MD_CAP) return fail("a batch exceeds a capacity");
+            int64_t(n_rd) * n_cd > stg_md_cap(h.real)) return fail("a batch exceeds a capacity");
         if (h.sink_ptr[size_t(b.ru_b)] - h.sink_ptr[size_t(b.ru_a)] > STG_SINK_CAP ||
             h.src_ptr[size_t(b.cd_b)] - h.src_ptr[size_t(b.cd_a)] > STG_SRC_CAP) return fail("a batch exceeds an entry buffer");
         max_md = std::max<int64_t>(max_md, int64_t(n_rd) * n_cd);
@@ -741,10 +745,9 @@ extern "C" int wick_contract(const void* U_dev, const void* D_dev, const wick_te
         std::max(nmu, nmd) * int64_t(S_b) < (int64_t(1) << 31)) {   // the staged kernel keeps 32-bit element offsets
         const int groups_full = int(std::min<int64_t>(S_b, (p.n_st + GROUP - 1) / GROUP * GROUP) / GROUP);
         const int n_bins = std::max(1, std::min(MAX_CHUNKS, 148 * STG_CTAS_PER_SM / std::max(1, groups_full)));
-        rc = ensure_staged(t, n_bins, stream, &stg);
+        rc = ensure_staged(t, n_bins, (flags & WICK_CONTRACT_COMPLEX_COEFFS) != 0, stream, &stg);
         if (rc < 0) return rc;
         have_staged = (rc == 1);
-        if (flags & WICK_CONTRACT_COMPLEX_COEFFS) stg.real_coeffs = false;
     }
     for (int64_t st0 = 0; st0 < p.n_st; st0 += S_b) {
         const int64_t n_valid = std::min<int64_t>(S_b, p.n_st - st0);

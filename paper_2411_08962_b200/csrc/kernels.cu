@@ -564,6 +564,14 @@ constexpr size_t STG_OFF_SINKP = STG_OFF_SRCO + size_t(STG_SRC_CAP) * 4;        
 constexpr size_t STG_OFF_ROWOFF = STG_OFF_SINKP + size_t(STG_ROWS_CAP + 2) * 4;             // int[STG_ROWS_CAP] MU row offsets
 constexpr size_t STG_OFF_SRCP = STG_OFF_ROWOFF + size_t(STG_ROWS_CAP + 2) * 4;              // int[16] per-cd entry ranges, int[16] u column offsets
 constexpr size_t STG_SMEM = STG_OFF_SRCP + 32 * 4;
+// real coefficients: {MD block, sink records, dense B, per-row entry ranges, MU row offsets, u column offsets}
+constexpr size_t STG_R_SINKC = size_t(STG_MD_CAP_REAL) * GROUP * 16;
+constexpr size_t STG_R_BD = STG_R_SINKC + size_t(STG_SINK_CAP) * 16;                        // double[STG_ROW_CAP][STG_NCD_CAP]
+constexpr size_t STG_R_SINKP = STG_R_BD + size_t(STG_ROW_CAP) * STG_NCD_CAP * 8 + 64;
+constexpr size_t STG_R_ROWOFF = STG_R_SINKP + size_t(STG_ROWS_CAP + 2) * 4;
+constexpr size_t STG_R_CUOFF = STG_R_ROWOFF + size_t(STG_ROWS_CAP + 2) * 4;
+constexpr size_t STG_SMEM_REAL = STG_R_CUOFF + 16 * 4;
+constexpr size_t stg_smem(bool real) { return real ? STG_SMEM_REAL : STG_SMEM; }
 
 // All u-row tuples of a batch that belong to this warp.  NCU = compile-time bound on the u columns of the
 // piece (loads / stores of the row are unrolled and predicated), NCD = its number of d columns (exact).
@@ -705,7 +713,9 @@ __device__ __forceinline__ c128 staged_rows_dense_ncd(const c128* MUs, const c12
         case 3: return WICK_STG_CALL(3);
         case 4: return WICK_STG_CALL(4);
         case 5: return WICK_STG_CALL(5);
-        default: return WICK_STG_CALL(6);
+        case 6: return WICK_STG_CALL(6);
+        case 7: return WICK_STG_CALL(7);
+        default: return WICK_STG_CALL(8);
     }
 #undef WICK_STG_CALL
 }
@@ -715,14 +725,16 @@ __device__ __forceinline__ c128 staged_rows_ncd(const c128* MUs, const c128* MDl
                                                 const int* rowoff, const int* cuoff, const int* sinkp, const c128* sinkc,
                                                 const int* sinko, const int* srcp, const c128* srcc, const int* srco) {
 #define WICK_STG_CALL(NCD) staged_rows<NCU, NCD, REAL>(MUs, MDl, row, warp, n_rows, n_cu, rowoff, cuoff, sinkp, sinkc, sinko, srcp, srcc, srco)
-    static_assert(STG_NCD_CAP == 6, "one case per d-column count");
+    static_assert(STG_NCD_CAP == 8, "one case per d-column count");
     switch (n_cd) {
         case 1: return WICK_STG_CALL(1);
         case 2: return WICK_STG_CALL(2);
         case 3: return WICK_STG_CALL(3);
         case 4: return WICK_STG_CALL(4);
         case 5: return WICK_STG_CALL(5);
-        default: return WICK_STG_CALL(6);
+        case 6: return WICK_STG_CALL(6);
+        case 7: return WICK_STG_CALL(7);
+        default: return WICK_STG_CALL(8);
     }
 #undef WICK_STG_CALL
 }
@@ -733,16 +745,18 @@ reduce_staged_kernel(const c128* __restrict__ MU, const c128* __restrict__ MD, i
                      c128* __restrict__ partial) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     c128* MDs = reinterpret_cast<c128*>(smem_raw);                       // [element][lane]
-    c128* sinkc = reinterpret_cast<c128*>(smem_raw + STG_OFF_SINKC);
-    c128* srcc = reinterpret_cast<c128*>(smem_raw + STG_OFF_SRCC);
+    // REAL: {MD block, sink records, dense B, entry ranges, row offsets, column offsets}; general: the map above
+    c128* sinkc = reinterpret_cast<c128*>(smem_raw + (REAL ? STG_R_SINKC : STG_OFF_SINKC));
+    c128* srcc = reinterpret_cast<c128*>(smem_raw + STG_OFF_SRCC);        // general coefficients only
     int* sinko = reinterpret_cast<int*>(smem_raw + STG_OFF_SINKO);
     int* srco = reinterpret_cast<int*>(smem_raw + STG_OFF_SRCO);
-    int* sinkp = reinterpret_cast<int*>(smem_raw + STG_OFF_SINKP);        // [0..rows]: sink entry ranges
-    int* rowoff = reinterpret_cast<int*>(smem_raw + STG_OFF_ROWOFF);      // [rows]: element offset of MU[ru, 0]
-    int* srcp = reinterpret_cast<int*>(smem_raw + STG_OFF_SRCP);          // [0..n_cd]: source entry ranges
-    int* cuoff = srcp + 16;                                               // [n_cu]: element offset of u column tuple
+    double* Bd = reinterpret_cast<double*>(smem_raw + STG_R_BD);          // real coefficients only
+    int* sinkp = reinterpret_cast<int*>(smem_raw + (REAL ? STG_R_SINKP : STG_OFF_SINKP));      // [0..rows]: sink entry ranges
+    int* rowoff = reinterpret_cast<int*>(smem_raw + (REAL ? STG_R_ROWOFF : STG_OFF_ROWOFF));   // [rows]: element offset of MU[ru, 0]
+    int* srcp = reinterpret_cast<int*>(smem_raw + STG_OFF_SRCP);          // [0..n_cd]: source entry ranges (general only)
+    int* cuoff = REAL ? reinterpret_cast<int*>(smem_raw + STG_R_CUOFF) : srcp + 16;            // [n_cu]: element offset of u column tuple
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    c128* row = reinterpret_cast<c128*>(smem_raw + STG_OFF_ROWS) + warp * STG_ROW_CAP * GROUP + lane;
+    c128* row = reinterpret_cast<c128*>(smem_raw + STG_OFF_ROWS) + warp * STG_ROW_CAP * GROUP + lane;   // general only
     const c128* MDl = MDs + lane;
     const int64_t s = int64_t(blockIdx.x) * GROUP + lane;
     const c128* MUs = MU + s;
@@ -772,18 +786,9 @@ reduce_staged_kernel(const c128* __restrict__ MU, const c128* __restrict__ MD, i
             sinkp[r] = __ldg(st.sink_ptr + ru_a + r) - sp0;
             if (r < n_rows) rowoff[r] = __ldg(st.ru_list + ru_a + r) * st.n_cols_u * S_b;
         }
-        const int q0 = __ldg(st.src_ptr + cd_a), q1 = __ldg(st.src_ptr + cd_a + n_cd);
-        for (int e = threadIdx.x; e < q1 - q0; e += STG_THREADS) {
-            const c128 cf = __ldg(st.src_c + q0 + e);
-            const int off = (__ldg(st.src_cupos + q0 + e) - cu_a) * GROUP;
-            srcc[e] = REAL ? make_double2(cf.x, __hiloint2double(0, off)) : cf;
-            if (!REAL) srco[e] = off;
-        }
-        // (nearly) full source block with real coefficients: dense B[cu][cd] in the (then unused) offset buffer
-        const bool dense = REAL && n_cu > 4 && 2 * (q1 - q0) >= n_cu * n_cd;
-        if (dense) {
+        if constexpr (REAL) {
+            // dense B[cu][cd] of the piece (row stride = n_cd rounded up to 2 doubles; zeros where there is no source term)
             const int ncdp = (n_cd + 1) & ~1;
-            double* Bd = reinterpret_cast<double*>(sinko);
             for (int e = threadIdx.x; e < n_cu * ncdp; e += STG_THREADS) {
                 const int cul = e / ncdp, cdi = e - cul * ncdp;
                 double v = 0.0;
@@ -792,16 +797,24 @@ reduce_staged_kernel(const c128* __restrict__ MU, const c128* __restrict__ MD, i
                         if (__ldg(st.src_cupos + j) - cu_a == cul) v += __ldg(st.src_c + j).x;
                 Bd[e] = v;
             }
+            if (threadIdx.x < n_cu) cuoff[threadIdx.x] = __ldg(st.cu_list + cu_a + threadIdx.x) * S_b;
+        } else {
+            const int q0 = __ldg(st.src_ptr + cd_a), q1 = __ldg(st.src_ptr + cd_a + n_cd);
+            for (int e = threadIdx.x; e < q1 - q0; e += STG_THREADS) {
+                srcc[e] = __ldg(st.src_c + q0 + e);
+                srco[e] = (__ldg(st.src_cupos + q0 + e) - cu_a) * GROUP;
+            }
+            if (threadIdx.x <= n_cd) srcp[threadIdx.x] = __ldg(st.src_ptr + cd_a + threadIdx.x) - q0;
+            if (threadIdx.x >= 32 && threadIdx.x < 32 + n_cu) cuoff[threadIdx.x - 32] = __ldg(st.cu_list + cu_a + threadIdx.x - 32) * S_b;
         }
-        if (threadIdx.x <= n_cd) srcp[threadIdx.x] = __ldg(st.src_ptr + cd_a + threadIdx.x) - q0;
-        if (threadIdx.x >= 32 && threadIdx.x < 32 + n_cu) cuoff[threadIdx.x - 32] = __ldg(st.cu_list + cu_a + threadIdx.x - 32) * S_b;
         cp_async_wait_all();
         __syncthreads();
-#define WICK_STG_CALL(NCU) staged_rows_ncd<NCU, REAL>(MUs, MDl, row, warp, n_rows, n_cu, n_cd, rowoff, cuoff, sinkp, sinkc, sinko, srcp, srcc, srco)
+#define WICK_STG_CALL(NCU) staged_rows_ncd<NCU, false>(MUs, MDl, row, warp, n_rows, n_cu, n_cd, rowoff, cuoff, sinkp, sinkc, sinko, srcp, srcc, srco)
         c128 v;
-        if (dense) {
-            const double* Bd = reinterpret_cast<const double*>(sinko);
-            if (n_cu <= 8) v = staged_rows_dense_ncd<8>(MUs, MDl, warp, n_rows, n_cu, n_cd, rowoff, cuoff, sinkp, sinkc, Bd);
+        if constexpr (REAL) {
+            if (n_cu <= 2) v = staged_rows_dense_ncd<2>(MUs, MDl, warp, n_rows, n_cu, n_cd, rowoff, cuoff, sinkp, sinkc, Bd);
+            else if (n_cu <= 4) v = staged_rows_dense_ncd<4>(MUs, MDl, warp, n_rows, n_cu, n_cd, rowoff, cuoff, sinkp, sinkc, Bd);
+            else if (n_cu <= 8) v = staged_rows_dense_ncd<8>(MUs, MDl, warp, n_rows, n_cu, n_cd, rowoff, cuoff, sinkp, sinkc, Bd);
             else v = staged_rows_dense_ncd<STG_ROW_CAP>(MUs, MDl, warp, n_rows, n_cu, n_cd, rowoff, cuoff, sinkp, sinkc, Bd);
         } else if (n_cu <= 2) v = WICK_STG_CALL(2);
         else if (n_cu <= 4) v = WICK_STG_CALL(4);
@@ -826,7 +839,7 @@ cudaError_t launch_reduce_staged(const double2* MU, const double2* MD, int n_gro
                                  double2* partial, int* n_chunks_out, cudaStream_t stream) {
     dim3 grid(n_groups, st.n_bins);
     ProfScope prof(PROF_REDUCE, stream);
-    if (st.real_coeffs) reduce_staged_kernel<true><<<grid, STG_THREADS, STG_SMEM, stream>>>(MU, MD, S_b, st, partial);
+    if (st.real_coeffs) reduce_staged_kernel<true><<<grid, STG_THREADS, STG_SMEM_REAL, stream>>>(MU, MD, S_b, st, partial);
     else reduce_staged_kernel<false><<<grid, STG_THREADS, STG_SMEM, stream>>>(MU, MD, S_b, st, partial);
     ++g_launches;
     *n_chunks_out = st.n_bins;
@@ -979,7 +992,7 @@ template <int N> static cudaError_t set_smem_attr() {
 
 cudaError_t configure_kernels() {
     cudaError_t e;
-    if ((e = cudaFuncSetAttribute(reduce_staged_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(STG_SMEM))) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(reduce_staged_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(STG_SMEM_REAL))) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(reduce_staged_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(STG_SMEM))) != cudaSuccess) return e;
 #define WICK_ATTR(N) if ((e = set_smem_attr<N>()) != cudaSuccess) return e;
     WICK_ATTR(0) WICK_ATTR(1) WICK_ATTR(2) WICK_ATTR(3) WICK_ATTR(4) WICK_ATTR(5) WICK_ATTR(6)

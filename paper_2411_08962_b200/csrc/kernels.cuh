@@ -49,12 +49,14 @@ cudaError_t launch_reduce_outer(const double2* MU, const double2* MD, int n_grou
 // block-grouped tuple lists ru_list / rd_list / cu_list / cd_list.
 constexpr int STG_THREADS = 192;          // 6 warps, two CTAs per SM (one loads while the other computes)
 constexpr int STG_CTAS_PER_SM = 2;
-constexpr int STG_MD_CAP = 96;            // MD elements (512 B each) of a batch
+constexpr int STG_MD_CAP = 96;            // MD elements (512 B each) of a batch, general complex coefficients
+constexpr int STG_MD_CAP_REAL = 184;      // ... real coefficients: no MU row buffers, the space goes to the MD block
 constexpr int STG_ROW_CAP = 15;           // MU elements of one (u-row tuple, source block) row
-constexpr int STG_NCD_CAP = 6;            // d columns of a batch piece (one template instance per count)
+constexpr int STG_NCD_CAP = 8;            // d columns of a batch piece (one template instance per count)
 constexpr int STG_SINK_CAP = 512;         // sink entries of a batch's u-row tuples
 constexpr int STG_SRC_CAP = 256;          // source entries of a batch piece's d columns
-constexpr int STG_ROWS_CAP = STG_MD_CAP;  // u-row tuples of a batch
+constexpr int STG_ROWS_CAP = STG_MD_CAP_REAL;  // u-row tuples of a batch
+constexpr int stg_md_cap(bool real) { return real ? STG_MD_CAP_REAL : STG_MD_CAP; }
 struct StagedBatch { int32_t cd_a, cd_b, cu_a, cu_b, rd_a, rd_b, ru_a, ru_b; };
 struct StagedTables {
     int n_cols_u, n_cols_d, n_bins;

@@ -29,6 +29,7 @@ struct FactorTerm { int32_t qu, qd; cplx c; };
 struct StagedDev {
     void* blob = nullptr;
     int n_bins = 0;
+    bool real = false;                          // schedule built for the real-coefficient kernel
     const int32_t *sink_ptr = nullptr, *sink_rdpos = nullptr, *src_ptr = nullptr, *src_cupos = nullptr;   // CSR by list position
     const double *sink_c = nullptr, *src_c = nullptr;
     const int32_t *ru_list = nullptr, *rd_list = nullptr, *cu_list = nullptr, *cd_list = nullptr;
@@ -59,7 +60,7 @@ struct DeviceTables {
     const int32_t* red_items = nullptr;         // [n_items][2]  (sink component, source component)
     int n_red_bins = 0;
     int staged_state = 0;                       // 0 = not checked, 1 = eligible, -1 = blocks too large for the staged kernel
-    std::map<int, StagedDev> staged;            // by number of CTA bins
+    std::map<int, StagedDev> staged;            // by 2 * number of CTA bins + (general-coefficient schedule ? 1 : 0)
     // flat list (uploaded only when the flat path runs)
     void* flat_blob = nullptr;
     const int32_t* t_uid = nullptr;

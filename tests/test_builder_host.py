@@ -217,7 +217,7 @@ def test_staged_schedule_covers_every_pair_once(cfg, n_bins):
     i = t.info
     batches, pairs, max_md, max_rows = t.staged_schedule_check(n_bins)   # raises if a pair is missed / doubled / out of range
     assert pairs == i.n_rows_u * i.n_cols_d
-    assert 1 <= batches and 1 <= max_md <= 96 and 1 <= max_rows <= 96
+    assert 1 <= batches and 1 <= max_md <= 184 and 1 <= max_rows <= 184
 
 
 def test_staged_schedule_rejects_generic_lists():
