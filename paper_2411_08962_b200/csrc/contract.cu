@@ -752,9 +752,9 @@ extern "C" int wick_contract(const void* U_dev, const void* D_dev, const wick_te
     for (int64_t st0 = 0; st0 < p.n_st; st0 += S_b) {
         const int64_t n_valid = std::min<int64_t>(S_b, p.n_st - st0);
         const int n_groups = int((n_valid + GROUP - 1) / GROUP);
-        WICK_CUDA(launch_minors(t->n_u, U, st0, p.n_st, n_groups, S_b, d.minor_desc[0], nmu, MU, PROF_MINORS_U, stream));
+        WICK_CUDA(launch_minors(t->n_u, U, st0, p.n_st, n_groups, S_b, d.minor_desc[0], nmu, true, MU, PROF_MINORS_U, stream));
         if (!shared_minors)
-            WICK_CUDA(launch_minors(t->n_d, D, st0, p.n_st, n_groups, S_b, d.minor_desc[1], nmd, MD, PROF_MINORS_D, stream));
+            WICK_CUDA(launch_minors(t->n_d, D, st0, p.n_st, n_groups, S_b, d.minor_desc[1], nmd, true, MD, PROF_MINORS_D, stream));
         int n_chunks = 1;
         if (t->n_terms == 0) {
             WICK_CUDA(cudaMemsetAsync(sigma + st0, 0, size_t(n_valid) * 16, stream));
@@ -944,12 +944,12 @@ extern "C" int wick_minor_dets(const void* P_dev, int64_t n_sites, int n, const 
         double2* out = static_cast<double2*>(out_dev) + m0 * n_sites;
         if (direct) {
             WICK_CUDA_M(launch_minors(n, static_cast<const double2*>(P_dev), 0, n_sites, int(n_sites / GROUP), int(S_b),
-                                      d_desc, nm, out, PROF_MINORS_U, stream));
+                                      d_desc, nm, false, out, PROF_MINORS_U, stream));
         } else {
             for (int64_t s0 = 0; s0 < n_sites; s0 += S_b) {
                 const int64_t nv = std::min(S_b, n_sites - s0);
                 WICK_CUDA_M(launch_minors(n, static_cast<const double2*>(P_dev), s0, n_sites, int((nv + GROUP - 1) / GROUP), int(S_b),
-                                          d_desc, nm, static_cast<double2*>(d_tmp), PROF_MINORS_U, stream));
+                                          d_desc, nm, false, static_cast<double2*>(d_tmp), PROF_MINORS_U, stream));
                 WICK_CUDA_M(cudaMemcpy2DAsync(out + s0, size_t(n_sites) * 16, d_tmp, size_t(S_b) * 16, size_t(nv) * 16, size_t(nm),
                                               cudaMemcpyDeviceToDevice, stream));
             }

@@ -255,35 +255,44 @@ struct LuState {
         for (int r = 0; r < 4; ++r) t[r] = make_double2(cr[K + r], ci[K + r]);
     }
     // level 1: columns K, K+1 of the minor -> s = 2x2 minors of Schur columns 0, 1 over the row pairs
-    __device__ __forceinline__ void first_pair(const unsigned char* tb, const c128* Ls, uint32_t cba, uint32_t cbb) {
-        c128 t0[4], t1[4];
-        schur_column(tb, Ls, cba, t0);
-        schur_column(tb, Ls, cbb, t1);
+    __device__ __forceinline__ void pair_from(const c128 (&t0)[4], const c128 (&t1)[4]) {
         int k = 0;
 #pragma unroll
         for (int a = 0; a < 4; ++a)
 #pragma unroll
             for (int b = a + 1; b < 4; ++b) s[k++] = det2(t0[a], t1[a], t0[b], t1[b]);
     }
+    __device__ __forceinline__ void first_pair(const unsigned char* tb, const c128* Ls, uint32_t cba, uint32_t cbb) {
+        c128 t0[4], t1[4];
+        schur_column(tb, Ls, cba, t0);
+        schur_column(tb, Ls, cbb, t1);
+        pair_from(t0, t1);
+    }
     // level 2: column K+2 -> signed 3x3 minors of Schur columns 0..2: c3[r] = (-1)^(r+3) det(rows != r),
     // each expanded along its last column in the 2x2 minors s
-    __device__ __forceinline__ void third_column(const unsigned char* tb, const c128* Ls, uint32_t cbj) {
-        c128 t[4];
-        schur_column(tb, Ls, cbj, t);
+    __device__ __forceinline__ void third_from(const c128 (&t)[4]) {
         const c128 m0 = cfma(t[3], s[3], cfnma(t[2], s[4], cmul(t[1], s[5])));   // rows 1,2,3
         const c128 m1 = cfma(t[3], s[1], cfnma(t[2], s[2], cmul(t[0], s[5])));   // rows 0,2,3
         const c128 m2 = cfma(t[3], s[0], cfnma(t[1], s[2], cmul(t[0], s[4])));   // rows 0,1,3
         const c128 m3 = cfma(t[2], s[0], cfnma(t[1], s[1], cmul(t[0], s[3])));   // rows 0,1,2
         c3[0] = make_double2(-m0.x, -m0.y); c3[1] = m1; c3[2] = make_double2(-m2.x, -m2.y); c3[3] = m3;
     }
-    // level 3: last column -> det = detp * sum_r S[r][3] c3[r]  (Laplace expansion of the 4x4 Schur
-    // complement along its last column); two independent partial sums keep the dependency chain short
-    __device__ __forceinline__ c128 finish(const unsigned char* tb, const c128* Ls, uint32_t cbj) const {
+    __device__ __forceinline__ void third_column(const unsigned char* tb, const c128* Ls, uint32_t cbj) {
         c128 t[4];
         schur_column(tb, Ls, cbj, t);
+        third_from(t);
+    }
+    // level 3: last column -> det = detp * sum_r S[r][3] c3[r]  (Laplace expansion of the 4x4 Schur
+    // complement along its last column); two independent partial sums keep the dependency chain short
+    __device__ __forceinline__ c128 finish_from(const c128 (&t)[4]) const {
         const c128 e0 = cfma(t[1], c3[1], cmul(t[0], c3[0]));
         const c128 e1 = cfma(t[3], c3[3], cmul(t[2], c3[2]));
         return cmul(detp, cadd(e0, e1));
+    }
+    __device__ __forceinline__ c128 finish(const unsigned char* tb, const c128* Ls, uint32_t cbj) const {
+        c128 t[4];
+        schur_column(tb, Ls, cbj, t);
+        return finish_from(t);
     }
 };
 
@@ -418,9 +427,95 @@ minors_kernel(const c128* __restrict__ P, int64_t st0, int64_t n_st_total, int S
     }
 }
 
+// ---------------------------------------------------------------------------------------------
+// a4, 6x6 minors with a per-thread cache of Schur columns.  After the two pivot steps of a (row tuple, b0, b1) instance
+// the Schur column of column index b is the same for every minor of the instance, whatever position b takes in it; the
+// trie of minors_kernel re-evaluates it once per level (1143 columns per He-4 row tuple for ~100 distinct ones).  Here
+// the columns b = 3..11 of the instance are computed once (9 x 4 complex = 576 B per thread in shared memory, entry e at
+// Sc[e * NT + thread]: conflict free) and the levels read them; b = 2 (only possible as b2 of the instance (0,1)) is kept
+// in registers.  One 256-thread CTA per SM (147 KB cache + 74 KB tile).
+// ---------------------------------------------------------------------------------------------
+constexpr int M6C_THREADS = 256;
+constexpr size_t M6C_SMEM = size_t(TILE_BYTES) + size_t(9 * 4) * 16 * M6C_THREADS;
+
+__global__ void __launch_bounds__(M6C_THREADS, 1)
+minors6_cached_kernel(const c128* __restrict__ P, int64_t st0, int64_t n_st_total, int S_b,
+                      const unsigned long long* __restrict__ desc, int n_minors, int chunk, c128* __restrict__ out) {
+    constexpr int N = 6, K = 2, NT = M6C_THREADS;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    c128* tile = reinterpret_cast<c128*>(smem_raw);
+    c128* Sc = tile + TILE_ELEMS + threadIdx.x;                          // this thread's cache: entry e at Sc[e * NT]
+    const int g = blockIdx.x;
+    const int64_t st_first = st0 + int64_t(g) * GROUP;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int m_begin = blockIdx.y * chunk;
+    const int m_end = min(n_minors, m_begin + chunk);
+    int m = m_begin + warp * (chunk / (NT / 32));
+    const int m_stop = min(m_end, m + chunk / (NT / 32));
+    Desc<N> dn;
+    if (m < m_stop) dn = Desc<N>::load(desc, m);
+    stage_tile(tile, P, st_first, n_st_total, NT);
+    __syncthreads();
+    const unsigned char* tb = reinterpret_cast<const unsigned char*>(tile + lane);
+    const bool valid = st_first + lane < n_st_total;
+    c128* outp = out + int64_t(g) * GROUP + lane;
+    constexpr uint32_t kRowStep = 12 * GROUP * 16, kColStep = GROUP * 16;
+    LuState<N, 0, NT> lu;
+    c128 col2[4];                                                        // Schur column of column index 2 (instance (0,1) only)
+#pragma unroll
+    for (int r = 0; r < 4; ++r) col2[r] = make_double2(0.0, 0.0);
+    unsigned long long prow = ~0ull, pcol = 0;
+    auto cached = [&](uint32_t b, c128 (&t)[4]) {
+#pragma unroll
+        for (int r = 0; r < 4; ++r) t[r] = Sc[((b - 3) * 4 + r) * NT];
+    };
+    for (; m < m_stop; ++m) {
+        const Desc<N> dc = dn;
+        if (m + 1 < m_stop) dn = Desc<N>::load(desc, m + 1);
+        const unsigned long long rws = dc.rows_bits(), diff = dc.cols_bits() ^ pcol;
+        const bool fresh = (rws != prow) || (diff & 0xffull) != 0;
+        if (fresh) {
+            uint32_t rb[N], cb[N];
+#pragma unroll
+            for (int i = 0; i < N; ++i) { rb[i] = dc.row(i) * kRowStep; cb[i] = dc.col(i) * kColStep; }
+            lu.start(tb, nullptr, rb, cb);
+            const uint32_t b1 = dc.col(1);
+            if (b1 < 2) lu.schur_column(tb, nullptr, 2 * kColStep, col2);
+#pragma unroll 1
+            for (uint32_t b = (b1 + 1 > 3 ? b1 + 1 : 3); b < 12; ++b) {
+                c128 t[4];
+                lu.schur_column(tb, nullptr, b * kColStep, t);
+#pragma unroll
+                for (int r = 0; r < 4; ++r) Sc[((b - 3) * 4 + r) * NT] = t[r];
+            }
+        }
+        const bool new_pair = fresh || (diff & 0xffffull) != 0;
+        if (new_pair) {
+            c128 t0[4], t1[4];
+            const uint32_t b2 = dc.col(2);
+            if (b2 == 2) {
+#pragma unroll
+                for (int r = 0; r < 4; ++r) t0[r] = col2[r];
+            } else cached(b2, t0);
+            cached(dc.col(3), t1);
+            lu.pair_from(t0, t1);
+        }
+        if (new_pair || (diff & 0xfffffull) != 0) {
+            c128 t[4];
+            cached(dc.col(4), t);
+            lu.third_from(t);
+        }
+        c128 t[4];
+        cached(dc.col(5), t);
+        const c128 det = lu.finish_from(t);
+        prow = rws; pcol = dc.cols_bits();
+        if (valid) outp[int64_t(m) * S_b] = det;
+    }
+}
+
 template <int N>
 static cudaError_t launch_minors_n(const c128* P, int64_t st0, int64_t n_st_total, int n_groups, int S_b,
-                                   const void* desc, int64_t n_minors, c128* out, int prof_cls, cudaStream_t stream) {
+                                   const void* desc, int64_t n_minors, bool ascending, c128* out, int prof_cls, cudaStream_t stream) {
     constexpr int NT = MinorCfg<N>::kThreads;
     constexpr int warps = NT / 32;
     // enough CTAs for ~4 waves on 148 SMs, but at least 2 minors per warp per CTA
@@ -434,8 +529,12 @@ static cudaError_t launch_minors_n(const c128* P, int64_t st0, int64_t n_st_tota
     chunks = int((n_minors + chunk - 1) / chunk);
     dim3 grid(n_groups, chunks);
     ProfScope prof(prof_cls, stream);
-    minors_kernel<N><<<grid, NT, MinorCfg<N>::kSmem, stream>>>(P, st0, n_st_total, S_b,
-                                                             static_cast<const unsigned long long*>(desc), int(n_minors), chunk, out);
+    if (N == 6 && ascending)                                   // the cache slots assume ascending column tuples (library tables)
+        minors6_cached_kernel<<<grid, M6C_THREADS, M6C_SMEM, stream>>>(P, st0, n_st_total, S_b,
+                                                                       static_cast<const unsigned long long*>(desc), int(n_minors), chunk, out);
+    else
+        minors_kernel<N><<<grid, NT, MinorCfg<N>::kSmem, stream>>>(P, st0, n_st_total, S_b,
+                                                                 static_cast<const unsigned long long*>(desc), int(n_minors), chunk, out);
     ++g_launches;
     return cudaGetLastError();
 }
@@ -443,9 +542,9 @@ static cudaError_t launch_minors_n(const c128* P, int64_t st0, int64_t n_st_tota
 int minor_desc_words(int n) { return n <= 8 ? 1 : 2; }
 
 cudaError_t launch_minors(int n, const double2* P, int64_t st0, int64_t n_st_total, int n_groups, int S_b,
-                          const void* desc, int64_t n_minors, double2* out, int prof_cls, cudaStream_t stream) {
+                          const void* desc, int64_t n_minors, bool ascending, double2* out, int prof_cls, cudaStream_t stream) {
     if (n_minors == 0 || n_groups == 0) return cudaSuccess;
-#define WICK_CASE(N) case N: return launch_minors_n<N>(P, st0, n_st_total, n_groups, S_b, desc, n_minors, out, prof_cls, stream);
+#define WICK_CASE(N) case N: return launch_minors_n<N>(P, st0, n_st_total, n_groups, S_b, desc, n_minors, ascending, out, prof_cls, stream);
     switch (n) {
         WICK_CASE(0) WICK_CASE(1) WICK_CASE(2) WICK_CASE(3) WICK_CASE(4) WICK_CASE(5) WICK_CASE(6)
         WICK_CASE(7) WICK_CASE(8) WICK_CASE(9) WICK_CASE(10) WICK_CASE(11) WICK_CASE(12)
@@ -992,6 +1091,7 @@ template <int N> static cudaError_t set_smem_attr() {
 
 cudaError_t configure_kernels() {
     cudaError_t e;
+    if ((e = cudaFuncSetAttribute(minors6_cached_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, int(M6C_SMEM))) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(reduce_staged_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(STG_SMEM_REAL))) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(reduce_staged_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(STG_SMEM))) != cudaSuccess) return e;
 #define WICK_ATTR(N) if ((e = set_smem_attr<N>()) != cudaSuccess) return e;

@@ -26,10 +26,11 @@ cudaError_t profile_read(double ms[PROF_CLASSES], int64_t count[PROF_CLASSES]);
 cudaError_t measure_fp64_peak(double* tflops, cudaStream_t stream);
 
 // launchers (kernels.cu); all enqueue on `stream` and return the cudaGetLastError() code
-// `desc`: one descriptor per minor, minor_desc_words(n) 64-bit words each (kernels.cu: struct Desc)
+// `desc`: one descriptor per minor, minor_desc_words(n) 64-bit words each (kernels.cu: struct Desc);
+// `ascending`: every column tuple is ascending (the library's own tables), which the cached 6x6 kernel relies on
 int minor_desc_words(int n);
 cudaError_t launch_minors(int n, const double2* P, int64_t st0, int64_t n_st_total, int n_groups, int S_b,
-                          const void* desc, int64_t n_minors, double2* out, int prof_cls, cudaStream_t stream);
+                          const void* desc, int64_t n_minors, bool ascending, double2* out, int prof_cls, cudaStream_t stream);
 cudaError_t launch_reduce_flat(const double2* MU, const double2* MD, int n_groups, int S_b,
                                const int32_t* uid, const int32_t* did, const double2* w, int64_t n_terms,
                                double2* partial, int* n_chunks_out, int max_chunks, cudaStream_t stream);
