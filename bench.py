@@ -63,6 +63,15 @@ def executed_flops_per_site(n: int, row_in_order: np.ndarray, cols_in_order: np.
     f_start = sum(8.0 * sum(n - 1 - i for i in range(J)) + (n - J) + 14.0 + 6.0 * (n - 1 - J) + (6.0 if J else 0.0)
                   for J in range(K))
     f_pair, f_third, f_finish = 2 * f_col + 84.0, f_col + 88.0, f_col + 36.0
+    if n == 6:
+        # minors6_cached_kernel: every Schur column of a (row tuple, b0, b1) instance is computed once, right after the two
+        # pivot steps (column indices max(b1 + 1, 3) .. 11, plus index 2 for b1 < 2); the levels only combine cached columns
+        first = np.concatenate(([True], ~same_lead(K)))
+        b1 = c[first, 1]
+        n_cols = int(np.sum(12 - np.maximum(b1 + 1, 3) + (b1 < 2)))
+        n_pair = 1 + int(np.count_nonzero(~same_lead(K + 2)))
+        n_third = 1 + int(np.count_nonzero(~same_lead(K + 3)))
+        return int(first.sum()) * f_start + n_cols * f_col + n_pair * 84.0 + n_third * 88.0 + nm * 36.0
     n_fresh = 1 + int(np.count_nonzero(~same_lead(K)))
     n_pair = 1 + int(np.count_nonzero(~same_lead(K + 2)))
     n_third = 1 + int(np.count_nonzero(~same_lead(K + 3)))
@@ -303,7 +312,8 @@ def main():
     except Exception:
         pass
     roofline = {
-        "bound": "alu", "kernel": f"minors_kernel<{info.n_u}>/<{info.n_d}> (a4, LU with partial pivoting)",
+        "bound": "alu", "kernel": " / ".join("minors6_cached_kernel" if n == 6 else f"minors_kernel<{n}>" for n in (info.n_u, info.n_d))
+                                  + " (a4, LU with partial pivoting)",
         "achieved": achieved_tf, "peak": FP64_PEAK_DERIVED_TFLOPS, "unit": "TFLOP/s",
         "frac": achieved_tf / FP64_PEAK_DERIVED_TFLOPS,
         "peak_source": "derived: 148 SMs x 64 FP64 lanes x 2 flop x 1.965 GHz (MEASURED_PEAKS.json has no FP64 entry)",
