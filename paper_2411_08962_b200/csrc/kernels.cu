@@ -513,6 +513,91 @@ minors6_cached_kernel(const c128* __restrict__ P, int64_t st0, int64_t n_st_tota
     }
 }
 
+// ---------------------------------------------------------------------------------------------
+// a4, 10x10 minors with the same per-thread cache of Schur columns: after the 6 pivot steps of a (row tuple, leading
+// columns) instance only 6 column indices remain, and every minor of the instance takes 4 of them.  The 6 Schur columns
+// (156 DFMA each) are computed once per instance (6 x 4 complex = 384 B per thread) and the levels combine them.
+// Column tuples come in the library's clustered order (build_minor_descs), so the slot of a column index is its rank
+// among the non-leading indices, kept as a nibble map.  One 256-thread CTA per SM as before (registers).
+// ---------------------------------------------------------------------------------------------
+constexpr size_t M10C_SMEM = size_t(TILE_BYTES) + size_t(6 * 4) * 16 * 256;
+
+__global__ void __launch_bounds__(256, 1)
+minors10_cached_kernel(const c128* __restrict__ P, int64_t st0, int64_t n_st_total, int S_b,
+                       const unsigned long long* __restrict__ desc, int n_minors, int chunk, c128* __restrict__ out) {
+    constexpr int N = 10, K = 6, NT = 256;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    c128* tile = reinterpret_cast<c128*>(smem_raw);
+    c128* Sc = tile + TILE_ELEMS + threadIdx.x;                          // this thread's cache: entry e at Sc[e * NT]
+    const int g = blockIdx.x;
+    const int64_t st_first = st0 + int64_t(g) * GROUP;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int m_begin = blockIdx.y * chunk;
+    const int m_end = min(n_minors, m_begin + chunk);
+    int m = m_begin + warp * (chunk / (NT / 32));
+    const int m_stop = min(m_end, m + chunk / (NT / 32));
+    Desc<N> dn;
+    if (m < m_stop) dn = Desc<N>::load(desc, m);
+    stage_tile(tile, P, st_first, n_st_total, NT);
+    __syncthreads();
+    const unsigned char* tb = reinterpret_cast<const unsigned char*>(tile + lane);
+    const bool valid = st_first + lane < n_st_total;
+    c128* outp = out + int64_t(g) * GROUP + lane;
+    constexpr uint32_t kRowStep = 12 * GROUP * 16, kColStep = GROUP * 16;
+    constexpr unsigned long long kLead = (1ull << (4 * K)) - 1, kLeadPair = (1ull << (4 * (K + 2))) - 1,
+                                 kLead3 = (1ull << (4 * (K + 3))) - 1;
+    LuState<N, 0, NT> lu;
+    unsigned long long smap = 0;                                         // column index -> cache slot (4 bits each)
+    unsigned long long prow = ~0ull, pcol = 0;
+    auto cached = [&](uint32_t b, c128 (&t)[4]) {
+        const uint32_t slot = uint32_t(smap >> (4 * b)) & 15u;
+#pragma unroll
+        for (int r = 0; r < 4; ++r) t[r] = Sc[(slot * 4 + r) * NT];
+    };
+    for (; m < m_stop; ++m) {
+        const Desc<N> dc = dn;
+        if (m + 1 < m_stop) dn = Desc<N>::load(desc, m + 1);
+        const unsigned long long rws = dc.rows_bits(), diff = dc.cols_bits() ^ pcol;
+        const bool fresh = (rws != prow) || (diff & kLead) != 0;
+        if (fresh) {
+            uint32_t rb[N], cb[N];
+            uint32_t lead = 0;
+#pragma unroll
+            for (int i = 0; i < N; ++i) { rb[i] = dc.row(i) * kRowStep; cb[i] = dc.col(i) * kColStep; if (i < K) lead |= 1u << dc.col(i); }
+            lu.start(tb, nullptr, rb, cb);
+            smap = 0;
+            uint32_t slot = 0;
+#pragma unroll 1
+            for (uint32_t b = 0; b < 12; ++b) {
+                if (lead & (1u << b)) continue;
+                c128 t[4];
+                lu.schur_column(tb, nullptr, b * kColStep, t);
+#pragma unroll
+                for (int r = 0; r < 4; ++r) Sc[(slot * 4 + r) * NT] = t[r];
+                smap |= (unsigned long long)slot << (4 * b);
+                ++slot;
+            }
+        }
+        const bool new_pair = fresh || (diff & kLeadPair) != 0;
+        if (new_pair) {
+            c128 t0[4], t1[4];
+            cached(dc.col(K), t0);
+            cached(dc.col(K + 1), t1);
+            lu.pair_from(t0, t1);
+        }
+        if (new_pair || (diff & kLead3) != 0) {
+            c128 t[4];
+            cached(dc.col(K + 2), t);
+            lu.third_from(t);
+        }
+        c128 t[4];
+        cached(dc.col(K + 3), t);
+        const c128 det = lu.finish_from(t);
+        prow = rws; pcol = dc.cols_bits();
+        if (valid) outp[int64_t(dc.out_index(m)) * S_b] = dc.negate() ? make_double2(-det.x, -det.y) : det;
+    }
+}
+
 template <int N>
 static cudaError_t launch_minors_n(const c128* P, int64_t st0, int64_t n_st_total, int n_groups, int S_b,
                                    const void* desc, int64_t n_minors, bool ascending, c128* out, int prof_cls, cudaStream_t stream) {
@@ -529,6 +614,12 @@ static cudaError_t launch_minors_n(const c128* P, int64_t st0, int64_t n_st_tota
     chunks = int((n_minors + chunk - 1) / chunk);
     dim3 grid(n_groups, chunks);
     ProfScope prof(prof_cls, stream);
+    if (N == 10 && ascending) {                                // library tables (no repeated index); slots = ranks among the non-leading indices
+        minors10_cached_kernel<<<grid, 256, M10C_SMEM, stream>>>(P, st0, n_st_total, S_b,
+                                                                 static_cast<const unsigned long long*>(desc), int(n_minors), chunk, out);
+        ++g_launches;
+        return cudaGetLastError();
+    }
     if (N == 6 && ascending)                                   // the cache slots assume ascending column tuples (library tables)
         minors6_cached_kernel<<<grid, M6C_THREADS, M6C_SMEM, stream>>>(P, st0, n_st_total, S_b,
                                                                        static_cast<const unsigned long long*>(desc), int(n_minors), chunk, out);
@@ -1091,6 +1182,7 @@ template <int N> static cudaError_t set_smem_attr() {
 
 cudaError_t configure_kernels() {
     cudaError_t e;
+    if ((e = cudaFuncSetAttribute(minors10_cached_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, int(M10C_SMEM))) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(minors6_cached_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, int(M6C_SMEM))) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(reduce_staged_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(STG_SMEM_REAL))) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(reduce_staged_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(STG_SMEM))) != cudaSuccess) return e;

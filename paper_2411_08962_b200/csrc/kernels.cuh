@@ -27,7 +27,7 @@ cudaError_t measure_fp64_peak(double* tflops, cudaStream_t stream);
 
 // launchers (kernels.cu); all enqueue on `stream` and return the cudaGetLastError() code
 // `desc`: one descriptor per minor, minor_desc_words(n) 64-bit words each (kernels.cu: struct Desc);
-// `ascending`: every column tuple is ascending (the library's own tables), which the cached 6x6 kernel relies on
+// `ascending`: the descriptors come from the library's own tables (distinct indices, 6x6 tuples ascending), which the cached kernels rely on
 int minor_desc_words(int n);
 cudaError_t launch_minors(int n, const double2* P, int64_t st0, int64_t n_st_total, int n_groups, int S_b,
                           const void* desc, int64_t n_minors, bool ascending, double2* out, int prof_cls, cudaStream_t stream);
