@@ -72,8 +72,8 @@ def executed_flops_per_site(n: int, row_in_order: np.ndarray, cols_in_order: np.
         n_pair = 1 + int(np.count_nonzero(~same_lead(K + 2)))
         n_third = 1 + int(np.count_nonzero(~same_lead(K + 3)))
         return int(first.sum()) * f_start + n_cols * f_col + n_pair * 84.0 + n_third * 88.0 + nm * 36.0
-    if n == 10:
-        # minors10_cached_kernel: the 6 Schur columns of a (row tuple, leading columns) instance are computed once
+    if n in (10, 11):
+        # minors_large_cached_kernel: the 12 - K Schur columns of a (row tuple, leading columns) instance are computed once
         n_inst = 1 + int(np.count_nonzero(~same_lead(K)))
         n_pair = 1 + int(np.count_nonzero(~same_lead(K + 2)))
         n_third = 1 + int(np.count_nonzero(~same_lead(K + 3)))
@@ -318,7 +318,7 @@ def main():
     except Exception:
         pass
     roofline = {
-        "bound": "alu", "kernel": " / ".join({6: "minors6_cached_kernel", 10: "minors10_cached_kernel"}.get(n, f"minors_kernel<{n}>") for n in (info.n_u, info.n_d))
+        "bound": "alu", "kernel": " / ".join({6: "minors6_cached_kernel", 10: "minors_large_cached_kernel<10>", 11: "minors_large_cached_kernel<11>"}.get(n, f"minors_kernel<{n}>") for n in (info.n_u, info.n_d))
                                   + " (a4, LU with partial pivoting)",
         "achieved": achieved_tf, "peak": FP64_PEAK_DERIVED_TFLOPS, "unit": "TFLOP/s",
         "frac": achieved_tf / FP64_PEAK_DERIVED_TFLOPS,

@@ -514,21 +514,25 @@ minors6_cached_kernel(const c128* __restrict__ P, int64_t st0, int64_t n_st_tota
 }
 
 // ---------------------------------------------------------------------------------------------
-// a4, 10x10 minors with the same per-thread cache of Schur columns: after the 6 pivot steps of a (row tuple, leading
+// a4, 10x10 (and 11x11) minors with the same per-thread cache of Schur columns: after the 6 pivot steps of a (row tuple, leading
 // columns) instance only 6 column indices remain, and every minor of the instance takes 4 of them.  The 6 Schur columns
 // (156 DFMA each) are computed once per instance (6 x 4 complex = 384 B per thread) and the levels combine them.
 // Column tuples come in the library's clustered order (build_minor_descs), so the slot of a column index is its rank
 // among the non-leading indices, kept as a nibble map.  One 256-thread CTA per SM as before (registers).
 // ---------------------------------------------------------------------------------------------
-constexpr size_t M10C_SMEM = size_t(TILE_BYTES) + size_t(6 * 4) * 16 * 256;
+// n = 11 works the same way with 5 remaining columns; its first multiplier column lives in shared memory (R = 1).
+template <int N, int R> constexpr size_t mlc_smem() { return size_t(TILE_BYTES) + size_t(lcol_base<N>(R) + (12 - (N - 4)) * 4) * 16 * 256; }
 
+template <int N, int R>
 __global__ void __launch_bounds__(256, 1)
-minors10_cached_kernel(const c128* __restrict__ P, int64_t st0, int64_t n_st_total, int S_b,
-                       const unsigned long long* __restrict__ desc, int n_minors, int chunk, c128* __restrict__ out) {
-    constexpr int N = 10, K = 6, NT = 256;
+minors_large_cached_kernel(const c128* __restrict__ P, int64_t st0, int64_t n_st_total, int S_b,
+                           const unsigned long long* __restrict__ desc, int n_minors, int chunk, c128* __restrict__ out) {
+    static_assert(N == 10 || N == 11, "slot map and shared-memory budget are laid out for these sizes");
+    constexpr int K = N - 4, NT = 256;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     c128* tile = reinterpret_cast<c128*>(smem_raw);
-    c128* Sc = tile + TILE_ELEMS + threadIdx.x;                          // this thread's cache: entry e at Sc[e * NT]
+    c128* Ls = tile + TILE_ELEMS + threadIdx.x;                          // multipliers of the first R columns
+    c128* Sc = Ls + lcol_base<N>(R) * NT;                                // this thread's cache: entry e at Sc[e * NT]
     const int g = blockIdx.x;
     const int64_t st_first = st0 + int64_t(g) * GROUP;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -546,7 +550,7 @@ minors10_cached_kernel(const c128* __restrict__ P, int64_t st0, int64_t n_st_tot
     constexpr uint32_t kRowStep = 12 * GROUP * 16, kColStep = GROUP * 16;
     constexpr unsigned long long kLead = (1ull << (4 * K)) - 1, kLeadPair = (1ull << (4 * (K + 2))) - 1,
                                  kLead3 = (1ull << (4 * (K + 3))) - 1;
-    LuState<N, 0, NT> lu;
+    LuState<N, R, NT> lu;
     unsigned long long smap = 0;                                         // column index -> cache slot (4 bits each)
     unsigned long long prow = ~0ull, pcol = 0;
     auto cached = [&](uint32_t b, c128 (&t)[4]) {
@@ -564,14 +568,14 @@ minors10_cached_kernel(const c128* __restrict__ P, int64_t st0, int64_t n_st_tot
             uint32_t lead = 0;
 #pragma unroll
             for (int i = 0; i < N; ++i) { rb[i] = dc.row(i) * kRowStep; cb[i] = dc.col(i) * kColStep; if (i < K) lead |= 1u << dc.col(i); }
-            lu.start(tb, nullptr, rb, cb);
+            lu.start(tb, Ls, rb, cb);
             smap = 0;
             uint32_t slot = 0;
 #pragma unroll 1
             for (uint32_t b = 0; b < 12; ++b) {
                 if (lead & (1u << b)) continue;
                 c128 t[4];
-                lu.schur_column(tb, nullptr, b * kColStep, t);
+                lu.schur_column(tb, Ls, b * kColStep, t);
 #pragma unroll
                 for (int r = 0; r < 4; ++r) Sc[(slot * 4 + r) * NT] = t[r];
                 smap |= (unsigned long long)slot << (4 * b);
@@ -614,11 +618,14 @@ static cudaError_t launch_minors_n(const c128* P, int64_t st0, int64_t n_st_tota
     chunks = int((n_minors + chunk - 1) / chunk);
     dim3 grid(n_groups, chunks);
     ProfScope prof(prof_cls, stream);
-    if (N == 10 && ascending) {                                // library tables (no repeated index); slots = ranks among the non-leading indices
-        minors10_cached_kernel<<<grid, 256, M10C_SMEM, stream>>>(P, st0, n_st_total, S_b,
-                                                                 static_cast<const unsigned long long*>(desc), int(n_minors), chunk, out);
-        ++g_launches;
-        return cudaGetLastError();
+    if constexpr (N == 10 || N == 11) {
+        if (ascending) {                                       // library tables (no repeated index); slots = ranks among the non-leading indices
+            constexpr int R = (N == 10) ? 0 : 1;
+            minors_large_cached_kernel<N, R><<<grid, 256, mlc_smem<N, R>(), stream>>>(P, st0, n_st_total, S_b,
+                                                                                      static_cast<const unsigned long long*>(desc), int(n_minors), chunk, out);
+            ++g_launches;
+            return cudaGetLastError();
+        }
     }
     if (N == 6 && ascending)                                   // the cache slots assume ascending column tuples (library tables)
         minors6_cached_kernel<<<grid, M6C_THREADS, M6C_SMEM, stream>>>(P, st0, n_st_total, S_b,
@@ -1182,7 +1189,8 @@ template <int N> static cudaError_t set_smem_attr() {
 
 cudaError_t configure_kernels() {
     cudaError_t e;
-    if ((e = cudaFuncSetAttribute(minors10_cached_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, int(M10C_SMEM))) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(minors_large_cached_kernel<10, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(mlc_smem<10, 0>()))) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(minors_large_cached_kernel<11, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(mlc_smem<11, 1>()))) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(minors6_cached_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, int(M6C_SMEM))) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(reduce_staged_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(STG_SMEM_REAL))) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(reduce_staged_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(STG_SMEM))) != cudaSuccess) return e;
