@@ -313,7 +313,7 @@ def main():
     executed_tf = st_per_step * (exec_site[0] + d_runs * exec_site[1]) / (ms_minors * 1e-3) / 1e12
     traffic = None
     try:
-        with open(os.path.join(ROOT, "profiles", "roofline_traffic.json")) as f:
+        with open(os.path.join(ROOT, "profiles", "r01_roofline_traffic.json.txt")) as f:
             traffic = json.load(f).get(cfg.name, {}).get("minors_dram_bytes_per_launch")
     except Exception:
         pass
