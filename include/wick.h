@@ -48,6 +48,7 @@ extern "C" {
 /* wick_contract flags */
 #define WICK_CONTRACT_FORCE_FLAT 1u  /* use the flat (uid, did, w) term list even if a factorised form exists */
 #define WICK_CONTRACT_COMPLEX_COEFFS 4u /* staged reduction: do not use the cheaper entries for all-real factor coefficients */
+#define WICK_CONTRACT_NO_REG_MINORS 8u /* 6x6 grid tables: use the shared-memory Schur-column cache kernel instead of the register-resident one */
 #define WICK_CONTRACT_NO_STAGED  2u  /* factorised lists: walk the block items from L1/L2 instead of staging them in shared memory */
 
 #define WICK_NUCLEON_PROTON  0

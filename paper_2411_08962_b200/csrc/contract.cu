@@ -539,6 +539,138 @@ int ensure_staged(const wick_terms* t, int n_bins, bool force_complex, cudaStrea
     return 1;
 }
 
+// ---- register-resident minors kernel: host schedule (minors_reg.cu) -----------------------------
+// Grid tables only (minor (r, c) = r * n_cols + c, column tuples sorted lexicographically).  Column tuples are
+// grouped by their K = n-4 leading columns (an "instance"); the candidate columns of an instance are the indices
+// that occur behind the leading ones, and every column tuple of the instance is a 4-subset of candidate
+// positions.  Because the tuples are sorted, the minors of an instance are contiguous in a row tuple's list and
+// appear in the rank order of their 4-subsets.
+struct RegHost {
+    bool ok = false;
+    int n = 0;
+    std::vector<RegJob> jobs;
+    std::vector<uint32_t> prog;                                     // trie programs of the jobs (kernels.cuh: RegTables::prog)
+    std::vector<double> cost;                                       // per job, in flops (LPT weights)
+    std::vector<uint32_t> rows;                                     // row tuples as 4-bit fields
+};
+
+RegHost build_reg_host(const FlavourTables& ft, bool grid) {
+    RegHost h;
+    h.n = ft.n;
+    const int n = ft.n, K = n - 4;
+    if (!grid || n < 5 || ft.cols.empty() || ft.rows.empty() || ft.rows.size() >= (size_t(1) << 24)) return h;
+    const size_t nc = ft.cols.size();
+    if (ft.minor_row.size() != ft.rows.size() * nc) return h;
+    const uint64_t lead_bits = (uint64_t(1) << (4 * K)) - 1;
+    int max_cand = 0;
+    for (size_t c0 = 0; c0 < nc;) {
+        const uint64_t lead = nibbles_of_mask(ft.cols[c0]) & lead_bits;
+        uint16_t lead_mask = 0;
+        for (int i = 0; i < K; ++i) lead_mask |= uint16_t(1u << ((lead >> (4 * i)) & 15u));
+        size_t c1 = c0;
+        uint16_t cand_mask = 0;
+        while (c1 < nc && (nibbles_of_mask(ft.cols[c1]) & lead_bits) == lead) { cand_mask |= uint16_t(ft.cols[c1] & ~lead_mask); ++c1; }
+        RegJob j;
+        std::memset(&j, 0, sizeof(j));
+        j.lead = lead;
+        j.cand = nibbles_of_mask(cand_mask);
+        j.ncand = uint32_t(__builtin_popcount(cand_mask));
+        max_cand = std::max(max_cand, int(j.ncand));
+        if (int(j.ncand) > REG_NC_MAX) return h;
+        j.out_base = uint32_t(c0);
+        j.prog_begin = uint32_t(h.prog.size());
+        int pos_of[12];
+        { int k = 0; for (int b = 0; b < 12; ++b) pos_of[b] = (cand_mask & (1u << b)) ? k++ : -1; }
+        // the tuples are sorted, so consecutive tuples with equal (i2, i3) form a pair node and with equal (i2, i3, i4) a third node
+        int n_pairs = 0, n_thirds = 0;
+        size_t pair_word = 0;
+        int p2 = -1, p3 = -1, p4 = -1;
+        for (size_t c = c0; c < c1; ++c) {
+            const uint64_t w = nibbles_of_mask(ft.cols[c]) >> (4 * K);
+            int x[4];
+            for (int i = 0; i < 4; ++i) x[i] = pos_of[(w >> (4 * i)) & 15u];
+            if (x[0] != p2 || x[1] != p3) {
+                pair_word = h.prog.size();
+                h.prog.push_back(uint32_t(x[0]) | (uint32_t(x[1]) << 4));
+                p2 = x[0]; p3 = x[1]; p4 = -1; ++n_pairs;
+            }
+            if (x[2] != p4) {
+                h.prog.push_back(uint32_t(x[2]));
+                h.prog[pair_word] += 1u << 8;
+                p4 = x[2]; ++n_thirds;
+            }
+            h.prog.back() |= 1u << (4 + x[3]);
+        }
+        j.prog_end = uint32_t(h.prog.size());
+        h.jobs.push_back(j);
+        // pivot steps + one Schur column per candidate + the trie levels (flops) + per-node overhead
+        h.cost.push_back(150.0 * K + 8.0 * K * (2 * n - K - 1) / 2 * j.ncand + 110.0 * n_pairs + 120.0 * n_thirds + 36.0 * double(c1 - c0) + 200.0);
+        c0 = c1;
+    }
+    if (h.jobs.size() > 256 || !minors_reg_supported(n, max_cand)) { h.jobs.clear(); return h; }
+    h.prog.push_back(0);                                            // the kernel reads one word ahead
+    h.rows.resize(ft.rows.size());
+    for (size_t r = 0; r < ft.rows.size(); ++r) h.rows[r] = uint32_t(nibbles_of_mask(ft.rows[r]));
+    h.ok = true;
+    return h;
+}
+
+// Returns 1 and fills `out` when flavour f's minors can go through the register-resident kernel, 0 when not.
+int ensure_reg(const wick_terms* t, int f, int n_bins, cudaStream_t stream, RegTables* out) {
+    std::lock_guard<std::mutex> lock(t->mu);
+    DeviceTables& d = t->dev;
+    if (d.reg_state[f] < 0) return 0;
+    auto fill = [&](const RegDev& rd) {
+        out->n_cols = int(t->f[f].cols.size()); out->n_bins = rd.n_bins;
+        out->jobs = static_cast<const RegJob*>(rd.jobs); out->prog = static_cast<const uint32_t*>(rd.prog); out->row_nibbles = static_cast<const uint32_t*>(rd.rows);
+        out->bin_ptr = static_cast<const uint32_t*>(rd.bin_ptr); out->bin_jobs = static_cast<const uint32_t*>(rd.bin_jobs);
+    };
+    auto hit = d.reg[f].find(n_bins);
+    if (hit != d.reg[f].end()) { fill(hit->second); return 1; }
+    const RegHost h = build_reg_host(t->f[f], t->outer);
+    if (!h.ok) { d.reg_state[f] = -1; return 0; }
+    d.reg_state[f] = 1;
+    // longest-processing-time assignment of (row tuple, job) pairs to the warp bins; fixed order
+    const size_t nr = h.rows.size(), nq = h.jobs.size();
+    std::vector<uint32_t> order(nq);
+    for (size_t q = 0; q < nq; ++q) order[q] = uint32_t(q);
+    std::stable_sort(order.begin(), order.end(), [&](uint32_t a, uint32_t b) { return h.cost[a] > h.cost[b]; });
+    std::vector<std::vector<uint32_t>> bins(static_cast<size_t>(n_bins));
+    std::vector<std::pair<double, int>> heap;
+    for (int b = 0; b < n_bins; ++b) heap.push_back({0.0, b});
+    auto cmp = [](const std::pair<double, int>& a, const std::pair<double, int>& b) { return a > b; };
+    std::make_heap(heap.begin(), heap.end(), cmp);
+    for (uint32_t q : order)
+        for (size_t r = 0; r < nr; ++r) {
+            std::pop_heap(heap.begin(), heap.end(), cmp);
+            bins[size_t(heap.back().second)].push_back((uint32_t(r) << 8) | q);
+            heap.back().first += h.cost[q];
+            std::push_heap(heap.begin(), heap.end(), cmp);
+        }
+    std::vector<uint32_t> bin_ptr(size_t(n_bins) + 1, 0), bin_jobs;
+    bin_jobs.reserve(nr * nq);
+    for (int b = 0; b < n_bins; ++b) {
+        bin_jobs.insert(bin_jobs.end(), bins[size_t(b)].begin(), bins[size_t(b)].end());
+        bin_ptr[size_t(b) + 1] = uint32_t(bin_jobs.size());
+    }
+    BlobBuilder bb;
+    const size_t o_j = bb.add(h.jobs.data(), h.jobs.size() * sizeof(RegJob)), o_r = bb.add(h.rows.data(), h.rows.size() * 4);
+    const size_t o_p = bb.add(h.prog.data(), h.prog.size() * 4);
+    const size_t o_bp = bb.add(bin_ptr.data(), bin_ptr.size() * 4), o_bj = bb.add(bin_jobs.data(), bin_jobs.size() * 4);
+    void* blob = nullptr;
+    WICK_CUDA(cudaMalloc(&blob, std::max<size_t>(bb.host.size(), 256)));
+    cudaError_t e = cudaMemcpyAsync(blob, bb.host.data(), bb.host.size(), cudaMemcpyHostToDevice, stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(stream);
+    if (e != cudaSuccess) { cudaFree(blob); set_error(std::string("minor job schedule upload: ") + cudaGetErrorString(e)); return WICK_ERR_CUDA; }
+    unsigned char* b = static_cast<unsigned char*>(blob);
+    RegDev rd;
+    rd.blob = blob; rd.n_bins = n_bins;
+    rd.jobs = b + o_j; rd.prog = b + o_p; rd.rows = b + o_r; rd.bin_ptr = b + o_bp; rd.bin_jobs = b + o_bj;
+    d.reg[f][n_bins] = rd;
+    fill(rd);
+    return 1;
+}
+
 int upload_flat(const wick_terms* t, cudaStream_t stream) {
     try { t->ensure_flat(); } catch (const std::bad_alloc&) { set_error("flat term list: out of host memory"); return WICK_ERR_NOMEM; }
     std::lock_guard<std::mutex> lock(t->mu);
@@ -614,6 +746,7 @@ extern "C" void wick_terms_release_device(DeviceTables* d) {
     if (d->blob) cudaFree(d->blob);
     if (d->flat_blob) cudaFree(d->flat_blob);
     for (auto& kv : d->staged) cudaFree(kv.second.blob);
+    for (int f = 0; f < 2; ++f) for (auto& kv : d->reg[f]) cudaFree(kv.second.blob);
     *d = DeviceTables();
 }
 
@@ -749,12 +882,23 @@ extern "C" int wick_contract(const void* U_dev, const void* D_dev, const wick_te
         if (rc < 0) return rc;
         have_staged = (rc == 1);
     }
+    const bool try_reg = t->outer && !(flags & WICK_CONTRACT_NO_REG_MINORS);
     for (int64_t st0 = 0; st0 < p.n_st; st0 += S_b) {
         const int64_t n_valid = std::min<int64_t>(S_b, p.n_st - st0);
         const int n_groups = int((n_valid + GROUP - 1) / GROUP);
-        WICK_CUDA(launch_minors(t->n_u, U, st0, p.n_st, n_groups, S_b, d.minor_desc[0], nmu, true, MU, PROF_MINORS_U, stream));
-        if (!shared_minors)
-            WICK_CUDA(launch_minors(t->n_d, D, st0, p.n_st, n_groups, S_b, d.minor_desc[1], nmd, true, MD, PROF_MINORS_D, stream));
+        // grid tables of 6x6 minors: register-resident instance kernel, one wave of CTAs (8 warp bins each)
+        const int reg_bins = std::max(1, (148 + n_groups - 1) / n_groups) * (REG_THREADS / 32);
+        for (int f = 0; f < (shared_minors ? 1 : 2); ++f) {
+            const int n = f == 0 ? t->n_u : t->n_d;
+            const double2* Pf = f == 0 ? U : D;
+            double2* Mf = f == 0 ? MU : MD;
+            RegTables rt;
+            rc = try_reg ? ensure_reg(t, f, reg_bins, stream, &rt) : 0;
+            if (rc < 0) return rc;
+            if (rc == 1) WICK_CUDA(launch_minors_reg(n, Pf, st0, p.n_st, n_groups, S_b, rt, Mf, f == 0 ? PROF_MINORS_U : PROF_MINORS_D, stream));
+            else WICK_CUDA(launch_minors(n, Pf, st0, p.n_st, n_groups, S_b, d.minor_desc[f], f == 0 ? nmu : nmd, true, Mf,
+                                         f == 0 ? PROF_MINORS_U : PROF_MINORS_D, stream));
+        }
         int n_chunks = 1;
         if (t->n_terms == 0) {
             WICK_CUDA(cudaMemsetAsync(sigma + st0, 0, size_t(n_valid) * 16, stream));

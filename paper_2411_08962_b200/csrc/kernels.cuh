@@ -31,6 +31,31 @@ cudaError_t measure_fp64_peak(double* tflops, cudaStream_t stream);
 int minor_desc_words(int n);
 cudaError_t launch_minors(int n, const double2* P, int64_t st0, int64_t n_st_total, int n_groups, int S_b,
                           const void* desc, int64_t n_minors, bool ascending, double2* out, int prof_cls, cudaStream_t stream);
+// Instance kernel for grid tables (minors_reg.cu).  An instance-job q is the same for every row tuple: K = n-4 leading
+// columns, up to REG_NC_MAX candidate columns behind them, and the trie of the instance's column tuples over candidate
+// POSITIONS as a word program.  The minors of a job are stored in trie order from column position out_base of the row
+// tuple's list.
+constexpr int REG_THREADS = 256;
+constexpr int REG_NC_MAX = 10;
+struct RegJob {
+    unsigned long long lead, cand;        // column indices as 4-bit fields: leading (K), candidates (ncand)
+    uint32_t ncand, prog_begin, prog_end, out_base;   // the job's words in RegTables::prog; first column position of its minors
+};
+static_assert(sizeof(RegJob) == 32, "RegJob is read with 16-byte loads");
+struct RegTables {
+    int n_cols, n_bins;                   // column tuples per row tuple; warps of work per site group (multiple of 8)
+    const RegJob* jobs;                   // [n_jobs <= 256]
+    const uint32_t* prog;                 // pair words i2 | i3 << 4 | n_third << 8, each followed by its third words i4 | mask(i5) << 4
+    const uint32_t* row_nibbles;          // [n_rows] row indices as 4-bit fields
+    const uint32_t* bin_ptr;              // [n_bins + 1]
+    const uint32_t* bin_jobs;             // (row tuple << 8) | job, grouped by bin
+};
+cudaError_t launch_minors_reg(int n, const double2* P, int64_t st0, int64_t n_st_total, int n_groups, int S_b,
+                              const RegTables& rt, double2* out, int prof_cls, cudaStream_t stream);
+cudaError_t launch_minors_reg_impl(int n, const double2* P, int64_t st0, int64_t n_st_total, int n_groups, int S_b,
+                                   const RegTables& rt, double2* out, cudaStream_t stream);   // minors_reg.cu
+bool minors_reg_supported(int n, int max_candidates);
+cudaError_t configure_reg_kernels();
 cudaError_t launch_reduce_flat(const double2* MU, const double2* MD, int n_groups, int S_b,
                                const int32_t* uid, const int32_t* did, const double2* w, int64_t n_terms,
                                double2* partial, int* n_chunks_out, int max_chunks, cudaStream_t stream);

@@ -1,0 +1,170 @@
+// a4 for "grid" minor tables (every row tuple x every column tuple, i.e. outer-product term lists), N = 5, 6:
+// register-resident instance kernel.
+//
+// A job = (row tuple, instance) where an instance is a set of K = N-4 leading columns shared by many column
+// tuples.  After the K pivot steps of the instance (left-looking LU with partial pivoting, lu_device.cuh) every
+// minor of the instance is  detp * det4(S[:, b_K], S[:, b_K+1], S[:, b_K+2], S[:, b_K+3])  with S the 4-row Schur
+// complement; its columns are needed for the NC <= 10 (11) "candidate" column indices that occur behind the
+// leading ones.  The thread computes all candidate Schur columns ONCE into registers (4 complex each) and then
+// walks the trie of 4-subsets of candidate POSITIONS with fully unrolled code, so every register index is
+// static: 2x2 minors of (i2, i3), signed 3x3 minors of (i2, i3, i4), Laplace sum with i5.  Which pairs, triples
+// and quadruples exist is a bit mask per instance (built on the host from the column tuples; warp uniform, so
+// every test is a uniform branch).  No per-thread shared-memory cache: shared memory holds the propagator tile
+// only, and levels 1-3 touch no memory but the result store.
+//
+// PAPER.md:203 ("analytic up to 4x4, LU above") and R.2 (:226, nothing is evaluated twice) one level below the
+// unique-minor table: every minor is still the pivoted LU of its own matrix, identical leading work is shared.
+#include "kernels.cuh"
+#include "lu_device.cuh"
+
+namespace wick {
+
+namespace {
+
+template <int NC>
+struct Trie {
+    c128 T[NC][4];                    // Schur columns of the candidate positions (registers: the static last level)
+    c128 s[6];                        // 2x2 minors of (detp * T[i2], T[i3]) over the row pairs 01 02 03 12 13 23
+    c128 c3[4];                       // signed 3x3 minors of (.., T[i4])
+    c128* o;                          // where the next minor goes (this lane)
+    size_t step;                      // S_b
+    bool valid;
+};
+
+// signed 3x3 minors of (.., t): c3[r] = (-1)^(r+3) det(rows != r), expanded along the last column in the 2x2 minors s
+__device__ __forceinline__ void third_from(const c128 (&s)[6], const c128 (&t)[4], c128 (&c3)[4]) {
+    const c128 m0 = cfma(t[3], s[3], cfnma(t[2], s[4], cmul(t[1], s[5])));   // rows 1,2,3
+    const c128 m1 = cfma(t[3], s[1], cfnma(t[2], s[2], cmul(t[0], s[5])));   // rows 0,2,3
+    const c128 m2 = cfma(t[3], s[0], cfnma(t[1], s[2], cmul(t[0], s[4])));   // rows 0,1,3
+    const c128 m3 = cfma(t[2], s[0], cfnma(t[1], s[1], cmul(t[0], s[3])));   // rows 0,1,2
+    c3[0] = make_double2(-m0.x, -m0.y); c3[1] = m1; c3[2] = make_double2(-m2.x, -m2.y); c3[3] = m3;
+}
+
+// last level, static in the candidate position: det = sum_r T[I5][r] c3[r]
+template <int NC, int I5>
+__device__ __forceinline__ void finish_all(Trie<NC>& c, uint32_t mask5) {
+    if constexpr (I5 < NC) {
+        if ((mask5 >> I5) & 1u) {
+            const c128 e0 = cfma(c.T[I5][1], c.c3[1], cmul(c.T[I5][0], c.c3[0]));
+            const c128 e1 = cfma(c.T[I5][3], c.c3[3], cmul(c.T[I5][2], c.c3[2]));
+            if (c.valid) *c.o = cadd(e0, e1);
+            c.o += c.step;
+        }
+        finish_all<NC, I5 + 1>(c, mask5);
+    }
+}
+
+template <int N, int NC, int J>
+__device__ __forceinline__ void schur_columns(const LuState<N, 0, REG_THREADS>& lu, const unsigned char* tb, unsigned long long cand,
+                                              int ncand, Trie<NC>& c, c128* Sc) {
+    if constexpr (J < NC) {
+        if (J < ncand) {
+            lu.schur_column(tb, nullptr, (uint32_t(cand >> (4 * J)) & 15u) * uint32_t(GROUP * 16), c.T[J]);
+            if constexpr (J < NC - 1) {                               // the last position can only be a last column
+#pragma unroll
+                for (int r = 0; r < 4; ++r) Sc[(J * 4 + r) * REG_THREADS] = c.T[J][r];
+            }
+        }
+        schur_columns<N, NC, J + 1>(lu, tb, cand, ncand, c, Sc);
+    }
+}
+
+__device__ __forceinline__ void cached_column(const c128* Sc, uint32_t pos, c128 (&t)[4]) {
+#pragma unroll
+    for (int r = 0; r < 4; ++r) t[r] = Sc[(pos * 4 + r) * REG_THREADS];
+}
+
+}  // namespace
+
+template <int NC> constexpr size_t reg_smem() { return size_t(TILE_BYTES) + size_t(NC - 1) * 4 * 16 * REG_THREADS; }
+
+template <int N, int NC>
+__global__ void __launch_bounds__(REG_THREADS, 1)
+minors_reg_kernel(const c128* __restrict__ P, int64_t st0, int64_t n_st_total, int S_b, RegTables rt, c128* __restrict__ out) {
+    constexpr int K = N - 4;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    c128* tile = reinterpret_cast<c128*>(smem_raw);
+    c128* Sc = tile + TILE_ELEMS + threadIdx.x;                       // this thread's copy of the Schur columns: entry e at Sc[e * NT]
+    const int g = blockIdx.x;
+    const int64_t st_first = st0 + int64_t(g) * GROUP;
+    const int lane = threadIdx.x & 31;
+    const int warp = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0);        // tells the compiler that everything derived from it is warp uniform
+    stage_tile(tile, P, st_first, n_st_total, REG_THREADS);
+    __syncthreads();
+    const unsigned char* tb = reinterpret_cast<const unsigned char*>(tile + lane);
+    constexpr uint32_t kRowStep = 12 * GROUP * 16, kColStep = GROUP * 16;
+    const int bin = blockIdx.y * (REG_THREADS / 32) + warp;
+    const int j0 = __ldg(rt.bin_ptr + bin), j1 = __ldg(rt.bin_ptr + bin + 1);
+    Trie<NC> c;
+    c.valid = st_first + lane < n_st_total;
+    c.step = size_t(S_b);
+    c128* outp = out + int64_t(g) * GROUP + lane;
+    for (int j = j0; j < j1; ++j) {
+        const uint32_t jr = __ldg(rt.bin_jobs + j);
+        const RegJob* job = rt.jobs + (jr & 255u);
+        const uint32_t r = jr >> 8;
+        const uint32_t rows = __ldg(rt.row_nibbles + r);
+        const ulonglong2 h0 = __ldg(reinterpret_cast<const ulonglong2*>(job));            // lead, cand
+        const uint4 h1 = __ldg(reinterpret_cast<const uint4*>(job) + 1);                  // ncand, prog_begin, prog_end, out_base
+        c128 detp;
+        {
+            LuState<N, 0, REG_THREADS> lu;
+            uint32_t rb[N], cb[N];
+#pragma unroll
+            for (int i = 0; i < N; ++i) { rb[i] = ((rows >> (4 * i)) & 15u) * kRowStep; cb[i] = (i < K) ? (uint32_t(h0.x >> (4 * i)) & 15u) * kColStep : 0u; }
+            lu.start(tb, nullptr, rb, cb);
+            schur_columns<N, NC, 0>(lu, tb, h0.y, int(h1.x), c, Sc);
+            detp = lu.detp;
+        }
+        c.o = outp + (size_t(r) * size_t(rt.n_cols) + size_t(h1.w)) * size_t(S_b);
+        // the instance's trie: pair words {i2, i3, number of third words}, each followed by its third words {i4, mask of i5}
+        const uint32_t* pw = rt.prog + h1.y;
+        const uint32_t* const pend = rt.prog + h1.z;
+        while (pw < pend) {
+            const uint32_t w = __ldg(pw++);
+            const uint32_t n3 = w >> 8;
+            {
+                c128 a[4], b[4];
+                cached_column(Sc, w & 15u, a);
+                cached_column(Sc, (w >> 4) & 15u, b);
+#pragma unroll
+                for (int q = 0; q < 4; ++q) a[q] = cmul(detp, a[q]);
+                int k = 0;
+#pragma unroll
+                for (int x = 0; x < 4; ++x)
+#pragma unroll
+                    for (int y = x + 1; y < 4; ++y) c.s[k++] = det2(a[x], b[x], a[y], b[y]);
+            }
+            uint32_t w3 = __ldg(pw);
+            c128 t[4];
+            cached_column(Sc, w3 & 15u, t);
+            for (uint32_t q = 0; q < n3; ++q) {
+                third_from(c.s, t, c.c3);
+                const uint32_t mask5 = w3 >> 4;
+                ++pw;
+                if (q + 1 < n3) {                                     // next third column: in flight during this node's last level
+                    w3 = __ldg(pw);
+                    cached_column(Sc, w3 & 15u, t);
+                }
+                finish_all<NC, 3>(c, mask5);
+            }
+        }
+    }
+}
+
+cudaError_t launch_minors_reg_impl(int n, const double2* P, int64_t st0, int64_t n_st_total, int n_groups, int S_b,
+                                   const RegTables& rt, double2* out, cudaStream_t stream) {
+    if (n_groups == 0 || rt.n_bins == 0) return cudaSuccess;
+    dim3 grid(n_groups, rt.n_bins / (REG_THREADS / 32));
+    if (n == 6) minors_reg_kernel<6, 10><<<grid, REG_THREADS, reg_smem<10>(), stream>>>(P, st0, n_st_total, S_b, rt, out);
+    else return cudaErrorInvalidValue;
+    return cudaGetLastError();
+}
+
+bool minors_reg_supported(int n, int max_candidates) { return n == 6 && max_candidates <= 10; }
+
+cudaError_t configure_reg_kernels() {
+    return cudaFuncSetAttribute(minors_reg_kernel<6, 10>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(reg_smem<10>()));
+}
+
+}  // namespace wick

@@ -37,6 +37,13 @@ struct StagedDev {
     const void* batches = nullptr;
 };
 
+// Job schedule of the register-resident minors kernel for one flavour and bin count (contract.cu: ensure_reg)
+struct RegDev {
+    void* blob = nullptr;
+    int n_bins = 0;
+    const void *jobs = nullptr, *prog = nullptr, *rows = nullptr, *bin_ptr = nullptr, *bin_jobs = nullptr;
+};
+
 // Device-resident copies, created by the first device call that needs them (contract.cu).
 struct DeviceTables {
     int device = -1;
@@ -61,6 +68,8 @@ struct DeviceTables {
     int n_red_bins = 0;
     int staged_state = 0;                       // 0 = not checked, 1 = eligible, -1 = blocks too large for the staged kernel
     std::map<int, StagedDev> staged;            // by 2 * number of CTA bins + (general-coefficient schedule ? 1 : 0)
+    int reg_state[2] = {0, 0};                  // per flavour: 0 = not checked, 1 = register-resident minors kernel usable, -1 = not
+    std::map<int, RegDev> reg[2];               // by number of warp bins per site group
     // flat list (uploaded only when the flat path runs)
     void* flat_blob = nullptr;
     const int32_t* t_uid = nullptr;
