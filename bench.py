@@ -5,10 +5,13 @@
 
 A "step" is one pass of the whole hot path (steps a3-a6 of DESIGN.md: propagator staging, unique minor
 determinants, weighted products, momentum projection) over one batch of synthetic input: the FULL term
-list of the workload on `timeslices_per_step` full timeslices of its lattice.  Default workload: cfg3
-(Helium-4, L = 32, 2716 x 2716 terms, 858,050 unique 6x6 minors per site), the configuration
-BASELINE.json's target is quoted on.  Metric: correlator timeslices/s (whole job); the same run also
-reports unique minor dets/s and the FP64 roofline fraction of the dominant kernel.
+list of the workload on `timeslices_per_step` (default 4, contiguous) full timeslices of its lattice per GPU.
+Default workload: cfg3 (Helium-4, L = 32, 2716 x 2716 terms, 858,050 unique 6x6 minors per site), the
+configuration BASELINE.json's target is quoted on.  Metric: correlator timeslices/s (whole job).  The timed loop
+runs with the library's per-launch events OFF; the kernel classes are timed in a separate pass.  The same JSON
+line carries the rooflines of the minors kernels (FP64 ALU: flops the kernels EXECUTE / time / the DFMA rate
+measured in this run) and of the reduction (HBM), and a "workloads" object with the Lithium-7-sized
+configurations (cfg4, cfg4b), measured the same way in this run.
 
 Prints ONE JSON line (rank 0).  `--impl reference` times the CPU oracle (oracle/, as it stands) on a
 bounded sample of the same workload instead.
@@ -43,7 +46,7 @@ def flops_lu(n: int) -> float:
         return 220.0
     return 8.0 * (n - 1) * n * (2 * n - 1) / 6 + 6.0 * n * (n - 1) / 2 + 15.0 * (n - 1) + 3.0 * (n * (n + 1) / 2 - 1)
 
-def executed_flops_per_site(n: int, row_in_order: np.ndarray, cols_in_order: np.ndarray) -> float:
+def executed_flops_per_site(n: int, row_in_order: np.ndarray, cols_in_order: np.ndarray, grid_cols=None) -> float:
     """Flops the minors kernel actually executes per site for one flavour, from the order in which it
     walks the minors (Terms.minor_order): the pivoted-LU state is kept across consecutive minors that share the row
     tuple and leading columns, so the K = n-4 pivot steps run once per (row tuple, first K columns), the 2x2 / 3x3
@@ -59,6 +62,22 @@ def executed_flops_per_site(n: int, row_in_order: np.ndarray, cols_in_order: np.
     if n == 3:                                                     # cofactors of the last column per (rows, b0, b1)
         return (1 + int(np.count_nonzero(~same_lead(2)))) * 42.0 + nm * 22.0
     K = n - 4
+    if grid_cols is not None:
+        # minors_reg_kernel (grid tables, n = 6): per (row tuple, K leading columns) instance the pivot steps and one Schur
+        # column per candidate column index; per (i2, i3) pair node 4 complex multiplications by the pivot product and six
+        # 2x2 minors; per (i2, i3, i4) node four signed 3x3 minors; per minor a 4-term Laplace sum
+        f_col_ = 8.0 * sum(n - 1 - i for i in range(K))
+        f_start_ = sum(8.0 * sum(n - 1 - i for i in range(J)) + (n - J) + 14.0 + 6.0 * (n - 1 - J) + (6.0 if J else 0.0)
+                       for J in range(K))
+        cc = [tuple(int(x) for x in t) for t in grid_cols]
+        inst, pairs, thirds = {}, set(), set()
+        for t in cc:
+            inst.setdefault(t[:K], set()).update(t[K:])
+            pairs.add(t[:K + 2])
+            thirds.add(t[:K + 3])
+        per_row = (len(inst) * f_start_ + sum(len(v) for v in inst.values()) * f_col_ + len(pairs) * (84.0 + 24.0)
+                   + len(thirds) * 88.0 + len(cc) * 30.0)
+        return per_row * (nm // len(cc))
     f_col = 8.0 * sum(n - 1 - i for i in range(K))
     f_start = sum(8.0 * sum(n - 1 - i for i in range(J)) + (n - J) + 14.0 + 6.0 * (n - 1 - J) + (6.0 if J else 0.0)
                   for J in range(K))
@@ -136,21 +155,78 @@ def workload_terms(wk, cfg):
     return wk.build_terms(cfg.nucleus)
 
 
-def oracle_seconds_per_site(cfg, n_sites: int):
-    """Time the oracle (MERGED mode = the paper's method A, two fresh determinants per term) on
-    n_sites sites of the workload.  Returns (seconds per site, threads used)."""
+def _oracle_site_runner(cfg, method: str):
+    """Closure that evaluates one site of the workload with the oracle.  method 'A' = two fresh determinants per term
+    (the paper's vanilla method: the oracle proper); 'B' = every distinct minor once per site, then the
+    term sum (the paper's improved method: what its SERIAL C / OPENMP C rows run)."""
     from oracle import wick_oracle as wo
     U, D = make_propagators_numpy(cfg.seed, cfg.L, cfg.T, t0=0, nt=1)
     if cfg.random_list:
         lst = make_random_term_list(cfg.seed, cfg.n_u, cfg.n_d, cfg.n_random_terms)
-        run = lambda s: wo.site_terms_value(U[0, s], D[0, s], *lst)
-    else:
-        sink = wo.merged_terms(cfg.nucleus)
-        run = lambda s: wo.site_value_outer(U[0, s], D[0, s], sink)
+        return lambda s: wo.site_terms_value(U[0, s], D[0, s], *lst)
+    sink = wo.merged_terms(cfg.nucleus)
+    if method == "B":
+        return lambda s: wo.site_value_method_b(U[0, s], D[0, s], sink)
+    return lambda s: wo.site_value_outer(U[0, s], D[0, s], sink)
+
+
+def _oracle_worker(args):
+    name, method, sites = args
+    os.environ["OMP_NUM_THREADS"] = "1"
+    run = _oracle_site_runner(CONFIGS[name], method)
+    t0 = time.perf_counter()
+    for s in sites:
+        run(s)
+    return time.perf_counter() - t0
+
+
+def oracle_seconds_per_site(cfg, n_sites: int, method: str = "A"):
+    """Time the oracle on n_sites sites of the workload, one core.  Returns (seconds per site, threads used)."""
+    run = _oracle_site_runner(cfg, method)
     t0 = time.perf_counter()
     for s in range(n_sites):
         run(s)
     return (time.perf_counter() - t0) / n_sites, 1          # numpy elementwise code: one thread
+
+
+def oracle_sites_per_second_all_cores(cfg, key: str, sites_per_worker: int, method: str = "A"):
+    """The same oracle code on every host core: one process per core, each evaluating its own sites (sites are
+    independent, Eq. A5).  Returns (sites per second of the whole pool, processes used)."""
+    import multiprocessing as mp
+    cores = len(os.sched_getaffinity(0))
+    jobs = [(key, method, list(range(w * sites_per_worker, (w + 1) * sites_per_worker))) for w in range(cores)]
+    with mp.get_context("spawn").Pool(cores) as pool:
+        t0 = time.perf_counter()
+        busy = pool.map(_oracle_worker, jobs)
+        wall = time.perf_counter() - t0
+    # the pool start-up (interpreter + numpy import + term expansion per process) is not oracle work: use the slowest worker
+    return cores * sites_per_worker / max(max(busy), 1e-9), cores, wall
+
+
+def cpu_baseline_rows(cfg, key: str, sites_a: int, all_cores: bool):
+    """cpu_baseline of the bench line: the oracle as it stands (method A) on one core, plus the same
+    on all host cores and the plain method-B CPU row, each on a bounded sample scaled by L^3 sites per timeslice."""
+    sps, cores = oracle_seconds_per_site(cfg, sites_a)
+    out = {"value": 1.0 / (sps * cfg.volume), "unit": "timeslices/s", "cores": cores, "kind": "oracle",
+           "sample": f"{sites_a} site(s) of {cfg.name} (full term list), {sps:.3g} s per site, scaled by L^3 = {cfg.volume} sites per timeslice",
+           "host_cores_available": len(os.sched_getaffinity(0))}
+    if not cfg.random_list:
+        n_b = max(sites_a, 2)
+        sps_b, _ = oracle_seconds_per_site(cfg, n_b, "B")
+        out["method_b_one_core"] = {"value": 1.0 / (sps_b * cfg.volume), "unit": "timeslices/s", "cores": 1, "kind": "oracle (method B: unique minors once per site, PAPER.md:294)",
+                                    "sample": f"{n_b} sites, {sps_b:.3g} s per site"}
+    if all_cores:
+        try:
+            rate, n_proc, wall = oracle_sites_per_second_all_cores(cfg, key, 1, "A")
+            out["all_cores"] = {"value": rate / cfg.volume, "unit": "timeslices/s", "cores": n_proc, "kind": "oracle",
+                                "sample": f"1 site per process, {n_proc} processes, slowest worker as the time (pool wall {wall:.1f} s)"}
+            if not cfg.random_list:
+                rate_b, n_proc, wall = oracle_sites_per_second_all_cores(cfg, key, 2, "B")
+                out["method_b_all_cores"] = {"value": rate_b / cfg.volume, "unit": "timeslices/s", "cores": n_proc,
+                                             "kind": "oracle (method B)", "sample": f"2 sites per process, {n_proc} processes"}
+        except Exception as exc:                                   # a missing /dev/shm or fork limit must not kill the bench line
+            out["all_cores"] = {"unavailable": repr(exc)}
+    return out
 
 
 def run_reference(args, cfg):
@@ -182,6 +258,168 @@ def run_reference(args, cfg):
     print(json.dumps(line))
 
 
+def kernel_source_hash() -> str:
+    """sha256 over the CUDA sources: keys the committed ncu traffic figures to the kernels they were measured on."""
+    import hashlib
+    h = hashlib.sha256()
+    csrc = os.path.join(ROOT, "paper_2411_08962_b200", "csrc")
+    for name in sorted(os.listdir(csrc)):
+        if name.endswith((".cu", ".cuh", ".h", ".cpp")):
+            with open(os.path.join(csrc, name), "rb") as f:
+                h.update(name.encode() + b"\0" + f.read())
+    return h.hexdigest()[:16]
+
+
+def read_traffic(cfg_name: str):
+    """DRAM bytes per launch from the committed `ncu --set full` capture (profiles/r02_roofline_traffic.json.txt), only
+    if that capture was taken on the kernel sources of this tree; otherwise null with the reason."""
+    path = os.path.join(ROOT, "profiles", "r02_roofline_traffic.json.txt")
+    try:
+        with open(path) as f:
+            rec = json.load(f)
+    except Exception:
+        return None, "no committed capture (profiles/r02_roofline_traffic.json.txt)"
+    here = kernel_source_hash()
+    if rec.get("kernel_source_hash") != here:
+        return None, f"stale: capture taken on kernel sources {rec.get('kernel_source_hash')}, this tree is {here}"
+    return rec.get("workloads", {}).get(cfg_name), f"profiles/r02_roofline_traffic.json.txt ({rec.get('command', 'ncu --set full')})"
+
+
+def minors_kernel_names(info, outer: bool):
+    def one(n):
+        if n == 6 and outer:
+            return "minors_reg_kernel<6,10>"
+        return {6: "minors6_cached_kernel", 10: "minors_large_cached_kernel<10>", 11: "minors_large_cached_kernel<11>"}.get(n, f"minors_kernel<{n}>")
+    return " / ".join(one(n) for n in (info.n_u, info.n_d))
+
+
+def reduce_executed_flops_per_site(terms, info) -> float:
+    """Flops the weighted-product kernel executes per site.  Factorised lists (reduce_staged_kernel): Q = B . MU row
+    (2 DFMA per real coefficient and (u row tuple, source entry)), P likewise over the sink entries, one complex FMA per
+    (u row tuple, d column tuple).  Flat lists: two complex multiplications and one addition per term."""
+    if not info.is_outer_product:
+        return float(info.n_terms) * FLOPS_PER_TERM
+    sru, srd, sc, qcu, qcd, qc = terms.factors()
+    real = bool(np.all(sc.imag == 0) and np.all(qc.imag == 0))
+    per_entry = 4.0 if real else 8.0
+    return per_entry * (info.n_source * info.n_rows_u + info.n_sink * info.n_cols_d) + 8.0 * info.n_rows_u * info.n_cols_d
+
+
+def class_times(wk, torch, step, n_prof):
+    """Per-class device time per step (CUDA events around every launch of a class, on the launching stream)."""
+    wk.profile_enable(True)
+    for _ in range(n_prof):
+        step()
+    torch.cuda.synchronize()
+    prof = wk.profile_read()
+    wk.profile_enable(False)
+    return {k: (v[0] / n_prof, v[1] // n_prof) for k, v in prof.items()}
+
+
+def rooflines(wk, cfg, terms, info, prof, ms_step, Tb, fp64_probe, hbm_gbs, d_runs):
+    """roofline blocks of one workload: the minors kernels (FP64 ALU) and the weighted-product kernel (HBM)."""
+    st_per_step = Tb * cfg.volume
+    ms_minors = prof["minors_u"][0] + prof["minors_d"][0]
+    ms_reduce, ms_project = prof["reduce"][0], prof["project"][0]
+    n_minor_launches = prof["minors_u"][1] + prof["minors_d"][1]
+    ur, uc, dr, dc = terms.tuples()
+    mu_row, _, md_row, _ = terms.minors()
+    ou, od = terms.minor_order(0), terms.minor_order(1)
+    outer = bool(info.is_outer_product)
+    exec_site = (executed_flops_per_site(info.n_u, mu_row[ou[0]], ou[1], uc if (outer and info.n_u == 6) else None),
+                 executed_flops_per_site(info.n_d, md_row[od[0]], od[1], dc if (outer and info.n_d == 6) else None))
+    exec_flop = st_per_step * (exec_site[0] + d_runs * exec_site[1])
+    alg_flop = st_per_step * (info.n_minors_u * flops_lu(info.n_u) + d_runs * info.n_minors_d * flops_lu(info.n_d))
+    executed_tf = exec_flop / (ms_minors * 1e-3) / 1e12 if ms_minors > 0 else 0.0
+    peak = fp64_probe if fp64_probe else FP64_PEAK_DERIVED_TFLOPS
+    traffic, traffic_src = read_traffic(cfg.name)
+    minors = {
+        "bound": "alu", "kernel": minors_kernel_names(info, outer) + " (a4, LU with partial pivoting)",
+        "achieved": executed_tf, "peak": peak, "unit": "TFLOP/s", "frac": executed_tf / peak,
+        "achieved_is": "flops the kernels execute (pivot steps and Schur columns shared by minors with equal row tuple and "
+                       "leading columns, DESIGN.md 6b), counted on the host from the tables, / CUDA-event time of the minors launches",
+        "peak_source": "register-only DFMA stream measured in this run (wick_measure_fp64_peak); MEASURED_PEAKS.json has no FP64 entry",
+        "peak_spec_arithmetic": FP64_PEAK_DERIVED_TFLOPS, "frac_of_spec_arithmetic": executed_tf / FP64_PEAK_DERIVED_TFLOPS,
+        "executed_flops_per_minor": {"u": exec_site[0] / max(info.n_minors_u, 1), "d": exec_site[1] / max(info.n_minors_d, 1)},
+        "algorithmic_equivalent": {"tflops": alg_flop / (ms_minors * 1e-3) / 1e12 if ms_minors > 0 else None,
+                                   "flops_per_minor": {"u": flops_lu(info.n_u), "d": flops_lu(info.n_d)},
+                                   "note": "one full LU per unique minor (SURVEY 8d convention); not a roofline fraction"},
+        "traffic": (traffic or {}).get("minors_dram_bytes_per_launch"), "traffic_source": traffic_src,
+        "launches_per_step": int(n_minor_launches), "avg_launch_ms": ms_minors / max(n_minor_launches, 1),
+        "kernel_share_of_step": ms_minors / ms_step,
+        "per_flavour_ms_per_step": {"u": prof["minors_u"][0], "d": prof["minors_d"][0]},
+    }
+    red_flop = st_per_step * reduce_executed_flops_per_site(terms, info)
+    red_bytes = st_per_step * 16.0 * (info.n_minors_u + info.n_minors_d * d_runs + 1)   # every minor read once + sigma
+    reduce = {
+        "bound": "hbm", "kernel": "reduce_staged_kernel (a5)" if outer else "reduce_flat_kernel (a5)",
+        "achieved": red_bytes / (ms_reduce * 1e-3) / 1e9 if ms_reduce > 0 else None, "peak": hbm_gbs, "unit": "GB/s",
+        "frac": (red_bytes / (ms_reduce * 1e-3) / 1e9 / hbm_gbs) if (ms_reduce > 0 and hbm_gbs) else None,
+        "achieved_is": "16 B x unique minors x site-times (each minor read once) / CUDA-event time of the reduction launches",
+        "peak_source": "MEASURED_PEAKS.json hbm_gbs" if hbm_gbs else "unavailable",
+        "executed_tflops": red_flop / (ms_reduce * 1e-3) / 1e12 if ms_reduce > 0 else None,
+        "executed_frac_of_fp64_peak": (red_flop / (ms_reduce * 1e-3) / 1e12 / peak) if ms_reduce > 0 else None,
+        "traffic": (traffic or {}).get("reduce_dram_bytes_per_launch"), "traffic_source": traffic_src,
+        "launches_per_step": int(prof["reduce"][1]), "avg_launch_ms": ms_reduce / max(prof["reduce"][1], 1),
+        "kernel_share_of_step": ms_reduce / ms_step,
+    }
+    dram_step = (traffic or {}).get("dram_bytes_per_timeslice")
+    return minors, reduce, {"project_ms_per_step": ms_project,
+                            "dram_bytes_per_timeslice": dram_step,
+                            "dram_over_algorithmic": (dram_step / (4608.0 * cfg.volume)) if dram_step else None,
+                            "algorithmic_bytes_per_timeslice": 4608.0 * cfg.volume}
+
+
+def bench_workload(wk, torch, cfg, key, Tb, steps, warmup, dev, fp64_probe, hbm_gbs, isospin=False, sampler=None):
+    """One workload on this rank's GPU, device-resident inputs: timeslices/s, rooflines, launches.  Single-GPU path."""
+    from wick_inputs import make_propagators_torch
+    terms = workload_terms(wk, cfg)
+    info = terms.info
+    n_mom = len(cfg.momenta)
+    Tb = min(Tb, cfg.T)
+    U, D = make_propagators_torch(cfg.seed, cfg.L, cfg.T, dev, t0=0, nt=Tb)
+    if isospin:
+        D = U
+    ws = torch.empty(wk.contract_workspace_bytes(terms, cfg.L, Tb, n_mom), dtype=torch.uint8, device=dev)
+    Cout = torch.empty((n_mom, Tb), dtype=torch.complex128, device=dev)
+
+    def step():
+        wk.contract(U, D, terms, cfg.momenta, cfg.L, Tb, workspace=ws, out=Cout)
+
+    for _ in range(max(warmup, 3)):
+        step()
+    torch.cuda.synchronize()
+    if sampler is not None:
+        sampler.start()
+    wk.launch_count(reset=True)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(steps):
+        step()
+    e1.record()
+    torch.cuda.synchronize()
+    ms_step = e0.elapsed_time(e1) / steps
+    launches = wk.launch_count(reset=True)
+    clocks = sampler.stop() if sampler is not None else None
+    prof = class_times(wk, torch, step, max(1, min(3, steps)))
+    wk.launch_count(reset=True)
+    d_runs = 1.0 if prof["minors_d"][1] > 0 else 0.0
+    minors, reduce, extra = rooflines(wk, cfg, terms, info, prof, ms_step, Tb, fp64_probe, hbm_gbs, d_runs)
+    st = Tb * cfg.volume
+    rec = {
+        "workload": cfg.name, "value": Tb / (ms_step * 1e-3), "unit": "timeslices/s", "ms_per_step": ms_step, "steps": steps,
+        "timeslices_per_step": Tb, "L": cfg.L, "n_u": info.n_u, "n_d": info.n_d, "n_terms": int(info.n_terms),
+        "unique_minors_per_site": int(info.n_minors_u + info.n_minors_d),
+        "minor_dets_per_s": st * (info.n_minors_u + info.n_minors_d) / (ms_step * 1e-3),
+        "minor_dets_per_s_kernel_only": st * (info.n_minors_u + d_runs * info.n_minors_d) / ((prof["minors_u"][0] + prof["minors_d"][0]) * 1e-3),
+        "roofline": minors, "roofline_reduce": reduce, "gpu_launches": int(launches),
+        "propagator_read_gbs": st * 4608 / (ms_step * 1e-3) / 1e9, **extra,
+    }
+    if clocks is not None:
+        rec["clocks"] = clocks
+    return rec, terms, (U, D, Cout)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -189,11 +427,15 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="cfg3", choices=sorted(CONFIGS))
-    ap.add_argument("--timeslices-per-step", type=int, default=1)
+    ap.add_argument("--timeslices-per-step", type=int, default=4, help="contiguous timeslices per step and GPU (SURVEY 8(d): >= 4)")
     ap.add_argument("--ref-sites", type=int, default=1, help="oracle sites per step for --impl reference")
-    ap.add_argument("--cpu-baseline-sites", type=int, default=2)
+    ap.add_argument("--cpu-baseline-sites", type=int, default=1)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-cpu-all-cores", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--side-workloads", default="cfg4,cfg4b", help="comma list measured in the same run and reported under "
+                    "'workloads' (north_star names Li-7 next to He-4); '' to skip")
+    ap.add_argument("--side-steps", type=int, default=400)
     ap.add_argument("--isospin", action="store_true",
                     help="side measurement, not the headline: one propagator for both flavours (the paper's m_u = m_d, "
                          "PAPER.md:518); flavours with equal unique-minor tables then share one evaluation")
@@ -206,6 +448,7 @@ def main():
     import torch
     import torch.distributed as dist
     import paper_2411_08962_b200 as wk
+    from paper_2411_08962_b200 import sharding
     from wick_inputs import make_propagators_torch
 
     rank = int(os.environ.get("RANK", "0"))
@@ -223,32 +466,42 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
-    Tb = min(args.timeslices_per_step, cfg.T)
+    def max_over_ranks(x: float) -> float:
+        if world == 1:
+            return x
+        tt = torch.tensor([x], dtype=torch.float64, device=dev)
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        return float(tt.item())
+
+    hbm_gbs = read_measured_peaks().get("hbm_gbs")
+    Tb = min(args.timeslices_per_step, max(cfg.T // world, 1))
+    T_job = Tb * world                                        # weak scaling: Tb timeslices per GPU
     terms = workload_terms(wk, cfg)
     info = terms.info
     n_mom = len(cfg.momenta)
-    # weak scaling: every rank owns its own block of Tb timeslices (shard by timeslice, no exchange)
-    t0_slice = (rank * Tb) % max(cfg.T - Tb + 1, 1)
-    U, D = make_propagators_torch(cfg.seed, cfg.L, cfg.T, dev, t0=t0_slice, nt=Tb)
-    if args.isospin:
-        D = U
-    ws = torch.empty(wk.contract_workspace_bytes(terms, cfg.L, Tb, n_mom), dtype=torch.uint8, device=dev)
-    Cout = torch.empty((n_mom, Tb), dtype=torch.complex128, device=dev)
+    # rank r owns the timeslices t = r (mod world) of the job's T_job timeslices (sharding.timeslices_of_rank);
+    # no collective on the data path, one gather of C[p][t] at the end of every step
+    mine = sharding.timeslices_of_rank(T_job, rank, world)
+    parts = [make_propagators_torch(cfg.seed, cfg.L, cfg.T, dev, t0=t, nt=1) for t in mine]
+    U = torch.cat([p[0] for p in parts]).contiguous()
+    D = U if args.isospin else torch.cat([p[1] for p in parts]).contiguous()
+    del parts
+    ws = torch.empty(wk.contract_workspace_bytes(terms, cfg.L, len(mine), n_mom), dtype=torch.uint8, device=dev)
+    result = {}
 
     def step():
-        wk.contract(U, D, terms, cfg.momenta, cfg.L, Tb, workspace=ws, out=Cout)
+        result["C"] = sharding.contract_sharded(U, D, terms, cfg.momenta, cfg.L, T_job, workspace=ws)
 
     for _ in range(max(args.warmup, 3)):
         step()
     barrier()
     fp64_probe = wk.measure_fp64_peak()
 
-    # ---- timed region: K steps, device time via CUDA events on the launching stream ----
+    # ---- timed region: K steps, profiling events off, device time via CUDA events on the launching stream ----
     sampler = ClockSampler(local_rank)
     if rank == 0:
         sampler.start()
     wk.launch_count(reset=True)
-    wk.profile_enable(True)
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
     e0.record()
@@ -256,114 +509,100 @@ def main():
         step()
     e1.record()
     barrier()
-    ms_total = e0.elapsed_time(e1)
+    ms_step = max_over_ranks(e0.elapsed_time(e1)) / args.steps
     launches = wk.launch_count(reset=True)
-    prof = wk.profile_read()
-    wk.profile_enable(False)
     clocks = sampler.stop() if rank == 0 else None
-    if world > 1:
-        tt = torch.tensor([ms_total], dtype=torch.float64, device=dev)
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        ms_total = float(tt.item())
-    ms_step = ms_total / args.steps
-    value = world * Tb / (ms_step * 1e-3)
+    value = T_job / (ms_step * 1e-3)
+    C_dev = result["C"]
+
+    # multi-GPU self-check: rank 0 recomputes a timeslice another rank owns and compares the gathered row bitwise
+    shard_check = None
+    if world > 1 and rank == 0:
+        t_other = 1
+        Uo, Do = make_propagators_torch(cfg.seed, cfg.L, cfg.T, dev, t0=t_other, nt=1)
+        Co = wk.contract(Uo, Uo if args.isospin else Do, terms, cfg.momenta, cfg.L, 1)
+        shard_check = bool(torch.equal(Co[:, 0], C_dev[:, t_other]))
+        if not shard_check:
+            raise RuntimeError("gathered C[p][t] differs from the single-rank result")
+
+    # ---- separate pass: per-class kernel times (events around every launch) ----
+    def local_step():
+        wk.contract(U, D, terms, cfg.momenta, cfg.L, len(mine), workspace=ws)
+    prof = class_times(wk, torch, local_step, max(1, min(3, args.steps)))
+    wk.launch_count(reset=True)
 
     # ---- e2e: the same step through the host-buffer C-ABI call (H2D + D2H inside the timed region) ----
     e2e = None
     if not args.no_e2e:
         Uh = torch.empty(U.shape, dtype=U.dtype, pin_memory=True)
-        Dh = torch.empty(D.shape, dtype=D.dtype, pin_memory=True)
         Uh.copy_(U)
-        Dh.copy_(D)
-        wk.contract_host(Uh, Dh, terms, cfg.momenta, cfg.L, Tb)          # warm-up
+        if args.isospin:
+            Dh = Uh
+        else:
+            Dh = torch.empty(D.shape, dtype=D.dtype, pin_memory=True)
+            Dh.copy_(D)
+        wk.contract_host(Uh, Dh, terms, cfg.momenta, cfg.L, len(mine))          # warm-up
         barrier()
         t_a = time.perf_counter()
         for _ in range(args.steps):
-            C_host = wk.contract_host(Uh, Dh, terms, cfg.momenta, cfg.L, Tb)   # synchronises before returning
+            C_host = wk.contract_host(Uh, Dh, terms, cfg.momenta, cfg.L, len(mine))   # synchronises before returning
         barrier()
-        e2e_ms = (time.perf_counter() - t_a) * 1e3 / args.steps
-        if world > 1:
-            tt = torch.tensor([e2e_ms], dtype=torch.float64, device=dev)
-            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-            e2e_ms = float(tt.item())
-        if not np.allclose(C_host, Cout.cpu().numpy(), rtol=1e-12, atol=0):
+        e2e_ms = max_over_ranks((time.perf_counter() - t_a) * 1e3 / args.steps)
+        if not np.array_equal(C_host, C_dev[:, mine].cpu().numpy()):
             raise RuntimeError("host-buffer call disagrees with the device-buffer call")
-        e2e = {"value": world * Tb / (e2e_ms * 1e-3), "unit": "timeslices/s",
-               "h2d_bytes_per_step": int(2 * Uh.numel() * 16), "d2h_bytes_per_step": int(C_host.size * 16),
-               "ms_per_step": e2e_ms}
+        e2e = {"value": T_job / (e2e_ms * 1e-3), "unit": "timeslices/s",
+               "h2d_bytes_per_step": int((1 if args.isospin else 2) * Uh.numel() * 16), "d2h_bytes_per_step": int(C_host.size * 16),
+               "ms_per_step": e2e_ms, "timeslices_per_call": len(mine),
+               "note": "wick_contract_host: timeslice blocks of <= 256 MB per flavour, H2D of block b+1 overlapped with the kernels of block b"}
+        del Uh, Dh
 
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
         return
 
-    # ---- roofline of the dominant kernel (a4: minors_kernel<n_u>, minors_kernel<n_d>) ----
-    st_per_step = Tb * cfg.volume
+    d_runs = 1.0 if prof["minors_d"][1] > 0 else 0.0
+    ms_step_local = ms_step
+    minors, reduce, extra = rooflines(wk, cfg, terms, info, prof, ms_step_local, len(mine), fp64_probe, hbm_gbs, d_runs)
+    st_per_step = len(mine) * cfg.volume
     minors_per_st = info.n_minors_u + info.n_minors_d
-    d_runs = 1.0 if prof["minors_d"][1] > 0 else 0.0           # isospin: the d minors may be served by the u table
-    flop_minors = st_per_step * (info.n_minors_u * flops_lu(info.n_u) + d_runs * info.n_minors_d * flops_lu(info.n_d))
-    ms_minors = (prof["minors_u"][0] + prof["minors_d"][0]) / args.steps
-    ms_reduce = prof["reduce"][0] / args.steps
-    ms_project = prof["project"][0] / args.steps
-    n_minor_launches = (prof["minors_u"][1] + prof["minors_d"][1]) // args.steps
-    achieved_tf = flop_minors / (ms_minors * 1e-3) / 1e12
-    mu_row, _, md_row, _ = terms.minors()
-    ou, od = terms.minor_order(0), terms.minor_order(1)
-    exec_site = (executed_flops_per_site(info.n_u, mu_row[ou[0]], ou[1]), executed_flops_per_site(info.n_d, md_row[od[0]], od[1]))
-    executed_tf = st_per_step * (exec_site[0] + d_runs * exec_site[1]) / (ms_minors * 1e-3) / 1e12
-    traffic = None
-    try:
-        with open(os.path.join(ROOT, "profiles", "r01_roofline_traffic.json.txt")) as f:
-            traffic = json.load(f).get(cfg.name, {}).get("minors_dram_bytes_per_launch")
-    except Exception:
-        pass
-    roofline = {
-        "bound": "alu", "kernel": " / ".join({6: "minors6_cached_kernel", 10: "minors_large_cached_kernel<10>", 11: "minors_large_cached_kernel<11>"}.get(n, f"minors_kernel<{n}>") for n in (info.n_u, info.n_d))
-                                  + " (a4, LU with partial pivoting)",
-        "achieved": achieved_tf, "peak": FP64_PEAK_DERIVED_TFLOPS, "unit": "TFLOP/s",
-        "frac": achieved_tf / FP64_PEAK_DERIVED_TFLOPS,
-        "peak_source": "derived: 148 SMs x 64 FP64 lanes x 2 flop x 1.965 GHz (MEASURED_PEAKS.json has no FP64 entry)",
-        "executed": {"tflops": executed_tf, "frac": executed_tf / FP64_PEAK_DERIVED_TFLOPS,
-                     "flops_per_minor": {"u": exec_site[0] / max(info.n_minors_u, 1), "d": exec_site[1] / max(info.n_minors_d, 1)},
-                     "note": "flops the kernel issues: LU state shared by minors with equal row tuple and leading columns "
-                             "(DESIGN.md 6b); `achieved`/`frac` count one full LU per unique minor (SURVEY 8d) and can exceed 1"},
-        "peak_measured_dfma_probe": fp64_probe, "frac_of_dfma_probe": achieved_tf / fp64_probe if fp64_probe else None,
-        "traffic": traffic, "launches_per_step": int(n_minor_launches),
-        "avg_launch_ms": ms_minors / max(n_minor_launches, 1),
-        "algorithmic_flops_per_minor": {"u": flops_lu(info.n_u), "d": flops_lu(info.n_d)},
-        "kernel_share_of_step": ms_minors / ms_step,
-        "reduce": {"ms_per_step": ms_reduce, "tflops": st_per_step * info.n_terms * FLOPS_PER_TERM / (ms_reduce * 1e-3) / 1e12
-                   if ms_reduce > 0 else None, "share_of_step": ms_reduce / ms_step},
-        "project_ms_per_step": ms_project,
-        "per_flavour": {
-            q: {"n": n, "ms_per_step": prof[k][0] / args.steps,
-                "frac": (st_per_step * nm * flops_lu(n) / (prof[k][0] / args.steps * 1e-3) / 1e12 / FP64_PEAK_DERIVED_TFLOPS)
-                if prof[k][0] > 0 else None}
-            for q, k, n, nm in (("u", "minors_u", info.n_u, info.n_minors_u), ("d", "minors_d", info.n_d, info.n_minors_d))},
-        "whole_step_tflops": (flop_minors + st_per_step * info.n_terms * FLOPS_PER_TERM) / (ms_step * 1e-3) / 1e12,
-    }
+
+    # ---- side workloads (north_star: He-4 AND Li-7), rank 0's GPU, same run ----
+    del U, D, ws
+    torch.cuda.empty_cache()
+    workloads = {}
+    if world == 1:
+        for key in [k for k in args.side_workloads.split(",") if k]:
+            side_sampler = ClockSampler(local_rank)
+            rec, _, _ = bench_workload(wk, torch, CONFIGS[key], key, args.timeslices_per_step, args.side_steps, args.warmup, dev,
+                                       fp64_probe, hbm_gbs, sampler=side_sampler)
+            if not args.no_cpu_baseline:
+                rec["cpu_baseline"] = cpu_baseline_rows(CONFIGS[key], key, 4, False)
+            workloads[CONFIGS[key].name] = rec
+            torch.cuda.empty_cache()
 
     cpu_baseline = None
     if not args.no_cpu_baseline:
-        sps, cores = oracle_seconds_per_site(cfg, args.cpu_baseline_sites)
-        cpu_baseline = {"value": 1.0 / (sps * cfg.volume), "unit": "timeslices/s", "cores": cores, "kind": "oracle",
-                        "sample": f"{args.cpu_baseline_sites} sites of {cfg.name} (full term list), {sps:.2f} s per site, "
-                                  f"scaled by L^3 = {cfg.volume} sites per timeslice",
-                        "host_cores_available": len(os.sched_getaffinity(0))}
+        cpu_baseline = cpu_baseline_rows(cfg, args.workload, args.cpu_baseline_sites, not args.no_cpu_all_cores)
 
     line = {
         "metric": "correlator_timeslices_per_s", "value": value, "unit": "timeslices/s",
         "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms_step,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64 (complex128)", "data": "synthetic",
-        "config": {"workload": cfg.name, "L": cfg.L, "T": cfg.T, "timeslices_per_step": Tb, "n_u": info.n_u, "n_d": info.n_d,
+        "config": {"workload": cfg.name, "L": cfg.L, "T": cfg.T, "timeslices_per_step": T_job, "timeslices_per_gpu": len(mine),
+                   "n_u": info.n_u, "n_d": info.n_d,
                    "isospin_u_equals_d": bool(args.isospin), "n_terms": int(info.n_terms), "unique_minors_per_site": int(minors_per_st), "n_momenta": n_mom,
-                   "l2_policy": "inputs_larger_than_l2" if 2 * U.numel() * 16 > 126e6 else "working_set_larger_than_l2",
-                   "parallelism": f"timeslice shards x{world}, no collective on the data path"},
+                   "l2_policy": "inputs_larger_than_l2 (and every site batch streams ~1.7 GB of minors through the 126 MB L2)",
+                   "parallelism": f"timeslice shards t = r mod {world} (sharding.contract_sharded), no collective on the data path, one gather of C per step",
+                   "profiling_events_in_timed_loop": False},
+        "ms_per_timeslice": ms_step / len(mine),
         "minor_dets_per_s": world * st_per_step * minors_per_st / (ms_step * 1e-3),
-        "minor_dets_per_s_kernel_only": st_per_step * (info.n_minors_u + d_runs * info.n_minors_d) / (ms_minors * 1e-3),
-        "roofline": roofline, "cpu_baseline": cpu_baseline, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
-        "hbm_peak_gbs_measured": read_measured_peaks().get("hbm_gbs"),
-        "propagator_read_gbs": st_per_step * 4608 / (ms_step * 1e-3) / 1e9,
+        "minor_dets_per_s_kernel_only": st_per_step * (info.n_minors_u + d_runs * info.n_minors_d) / ((prof["minors_u"][0] + prof["minors_d"][0]) * 1e-3),
+        "roofline": minors, "roofline_reduce": reduce, **extra,
+        "cpu_baseline": cpu_baseline, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
+        "hbm_peak_gbs_measured": hbm_gbs, "fp64_peak_tflops_measured": fp64_probe,
+        "propagator_read_gbs": world * st_per_step * 4608 / (ms_step * 1e-3) / 1e9,
+        "workloads": workloads, "sharded_result_bitwise_equal": shard_check,
     }
     print(json.dumps(line))
     if world > 1:

@@ -43,8 +43,13 @@ extern "C" {
 
 /* wick_build_terms* flags */
 #define WICK_BUILD_IDENTITY_TEST 1u  /* run the randomised identity test (Sec. III B PAPER.md:234-246, App. C) */
-#define WICK_BUILD_ISOSPIN       2u  /* the caller promises U == D (m_u = m_d): the identity   */
-                                     /* test then evaluates both flavours on the SAME random matrix          */
+#define WICK_BUILD_ISOSPIN       2u  /* the caller promises U == D (m_u = m_d).  Alone (nucleus  */
+                                     /* specs): sink terms related by the u <-> d swap are folded (factor 2),  */
+                                     /* the list stays an outer product and runs through the factorised        */
+                                     /* reduction with about half the products.  With IDENTITY_TEST: the test  */
+                                     /* evaluates both flavours on the SAME random matrix and merges the swap  */
+                                     /* classes of the flat list.  A handle changed by either can only be      */
+                                     /* contracted with U_dev == D_dev (WICK_ERR_ARG otherwise).               */
 /* wick_contract flags */
 #define WICK_CONTRACT_FORCE_FLAT 1u  /* use the flat (uid, did, w) term list even if a factorised form exists */
 #define WICK_CONTRACT_COMPLEX_COEFFS 4u /* staged reduction: do not use the cheaper entries for all-real factor coefficients */
@@ -179,6 +184,13 @@ int wick_contract_host(const void* U_host, const void* D_host, const wick_terms*
  * out_dev: device complex128 [n_minors][n_sites].  n = 0..12 (n = 0 gives 1).  Synchronises. */
 int wick_minor_dets(const void* P_dev, int64_t n_sites, int n, const uint8_t* rows, const uint8_t* cols,
                     int64_t n_minors, void* out_dev, void* cuda_stream);
+
+/* Step a4 for one flavour (0 = u, 1 = d) of a handle's unique-minor table, through exactly the kernels wick_contract
+ * launches for it (the register-resident / cached kernels for the library's own tables; `flags` as for wick_contract).
+ * P_dev: device complex128 [n_sites][12][12]; out_dev: device complex128 [n_minors][S] with S = n_sites rounded up to a
+ * multiple of 32 (columns >= n_sites are not written).  Enqueues on cuda_stream, does not synchronise. */
+int wick_terms_minor_table(const void* P_dev, int64_t n_sites, const wick_terms* terms, int flavour, unsigned flags,
+                           void* out_dev, void* cuda_stream);
 
 /* Measurement helpers (bench.py).  wick_profile_enable(1) makes every kernel launch of this thread's
  * device calls record CUDA events on its stream; wick_profile_read synchronises them, returns the

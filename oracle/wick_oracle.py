@@ -301,6 +301,34 @@ def site_value_outer(U: np.ndarray, D: np.ndarray, sink, source=None):
     return complex(_sum_ld(np.array(parts))), float(sum(absparts))
 
 
+def site_value_method_b(U: np.ndarray, D: np.ndarray, sink, source=None):
+    """The paper's "improved" method B (PAPER.md:294; what its SERIAL C / OPENMP C rows run, :432): every DISTINCT
+    (row tuple, column tuple) minor of a flavour is evaluated once per site (the minimal sets zeta_u, zeta_d of
+    Eq. A1), then sigma = sum_ij c_i conj(c_j) MU[a_u(i), b_u(j)] MD[a_d(i), b_d(j)].
+    Same result as site_value_outer (method A) up to rounding; used as a timed CPU baseline row and pinned against
+    method A in tests/test_oracle_pins.py.  Returns (sigma, S_abs)."""
+    source = sink if source is None else source
+    out = []
+    for f in (0, 1):
+        rows = sorted({t[f] for t in sink})
+        cols = sorted({t[f] for t in source})
+        P = U if f == 0 else D
+        r = np.array(rows, dtype=np.intp).reshape(len(rows), -1)
+        c = np.array(cols, dtype=np.intp).reshape(len(cols), -1)
+        M = det_elim(P[r[:, None, :, None], c[None, :, None, :]]) if r.shape[1] else np.ones((len(rows), len(cols)), complex)
+        out.append((M, {t: k for k, t in enumerate(rows)}, {t: k for k, t in enumerate(cols)}))
+    (MU, ru, cu), (MD, rd, cd) = out
+    ju = np.array([cu[t[0]] for t in source], dtype=np.intp)
+    jd = np.array([cd[t[1]] for t in source], dtype=np.intp)
+    cq = np.conj(np.array([t[2] for t in source], dtype=np.complex128))
+    parts, absparts = [], []
+    for (au, ad, ci) in sink:
+        v = (ci * cq) * MU[ru[au], ju] * MD[rd[ad], jd]
+        parts.append(_sum_ld(v))
+        absparts.append(float(np.sum(np.abs(v))))
+    return complex(_sum_ld(np.array(parts))), float(sum(absparts))
+
+
 def momentum_phases(L: int, momenta: Sequence[Tuple[int, int, int]]) -> np.ndarray:
     """e^{+2 pi i (n.x)/L} for every site s = x + L*(y + L*z); shape [n_mom][L^3].  (n.x) is reduced
     mod L in integers first so the phase is exact at multiples of L/4."""

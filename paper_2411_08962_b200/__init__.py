@@ -3,5 +3,5 @@ library libwick_b200.so (include/wick.h).  See DESIGN.md."""
 from .binding import (  # noqa: F401
     BUILD_IDENTITY_TEST, BUILD_ISOSPIN, CONTRACT_FORCE_FLAT, CONTRACT_NO_STAGED, CONTRACT_COMPLEX_COEFFS, CONTRACT_NO_REG_MINORS, EXPORTED_SYMBOLS, Terms, WickError,
     build_terms, build_terms_from_list, contract, contract_host, contract_workspace_bytes,
-    launch_count, library_path, load_library, measure_fp64_peak, minor_dets, profile_enable, profile_read, release_cached_buffers,
+    launch_count, library_path, load_library, measure_fp64_peak, minor_dets, minor_table, profile_enable, profile_read, release_cached_buffers,
 )

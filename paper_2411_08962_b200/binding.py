@@ -27,7 +27,7 @@ EXPORTED_SYMBOLS = (
     "wick_terms_export_minors", "wick_terms_export_terms", "wick_terms_export_factors",
     "wick_terms_staged_schedule_check", "wick_terms_export_minor_order", "wick_terms_free",
     "wick_contract_min_workspace_bytes", "wick_contract_workspace_bytes", "wick_contract",
-    "wick_contract_host", "wick_release_cached_buffers", "wick_minor_dets", "wick_launch_count", "wick_launch_count_reset",
+    "wick_contract_host", "wick_release_cached_buffers", "wick_minor_dets", "wick_terms_minor_table", "wick_launch_count", "wick_launch_count_reset",
     "wick_last_error", "wick_version", "wick_profile_enable", "wick_profile_read", "wick_measure_fp64_peak",
 )
 
@@ -87,6 +87,7 @@ def load_library():
     lib.wick_contract.argtypes = [vp, vp, vp, vp, i32, i32, i32, vp, vp, vp, sz, u32, vp]
     lib.wick_contract_host.argtypes = [vp, vp, vp, vp, i32, i32, i32, vp, vp, u32]
     lib.wick_minor_dets.argtypes = [vp, i64, i32, vp, vp, i64, vp, vp]
+    lib.wick_terms_minor_table.argtypes = [vp, i64, vp, i32, u32, vp, vp]
     lib.wick_profile_enable.argtypes = [i32]
     lib.wick_profile_read.argtypes = [C.POINTER(Profile)]
     lib.wick_measure_fp64_peak.argtypes = [C.POINTER(C.c_double), vp]
@@ -236,11 +237,17 @@ def contract(U, D, terms: Terms, momenta, L: int, T: int, workspace=None, want_s
     _check_dev(D, "D", (T, V, 12, 12))
     mom = np.ascontiguousarray(momenta, dtype=np.int32).reshape(-1, 3)
     n_mom = mom.shape[0]
-    if workspace is None:
-        workspace = torch.empty(contract_workspace_bytes(terms, L, T, n_mom), dtype=torch.uint8, device=U.device)
-    Cout = torch.empty((n_mom, T), dtype=torch.complex128, device=U.device) if out is None else out
-    sigma = torch.empty((T, V), dtype=torch.complex128, device=U.device) if want_sigma else None
-    with torch.cuda.device(U.device):
+    if out is not None:
+        _check_dev(out, "out", (n_mom, T))
+    if workspace is not None and not (isinstance(workspace, torch.Tensor) and workspace.is_cuda and workspace.is_contiguous()):
+        raise WickError("workspace must be a contiguous CUDA tensor")
+    # buffers created here are allocated on the stream the work is enqueued on, so the caching allocator cannot hand
+    # them to another stream's allocation while the kernels still run
+    with torch.cuda.device(U.device), torch.cuda.stream(torch.cuda.current_stream() if stream is None else stream):
+        if workspace is None:
+            workspace = torch.empty(contract_workspace_bytes(terms, L, T, n_mom), dtype=torch.uint8, device=U.device)
+        Cout = torch.empty((n_mom, T), dtype=torch.complex128, device=U.device) if out is None else out
+        sigma = torch.empty((T, V), dtype=torch.complex128, device=U.device) if want_sigma else None
         rc = lib.wick_contract(U.data_ptr(), D.data_ptr(), terms._h, _np_ptr(mom), n_mom, L, T, Cout.data_ptr(),
                                None if sigma is None else sigma.data_ptr(), workspace.data_ptr(),
                                workspace.numel() * workspace.element_size(), flags, _stream_ptr(stream))
@@ -259,7 +266,8 @@ def contract_host(U: np.ndarray, D: np.ndarray, terms: Terms, momenta, L: int, T
             if a.dtype != np.complex128 or not a.flags.c_contiguous or a.shape != (T, V, 12, 12):
                 raise WickError(f"{name} must be a C-contiguous complex128 array [T][L^3][12][12]")
             return a.ctypes.data_as(C.c_void_p)
-        if tuple(a.shape) != (T, V, 12, 12) or not a.is_contiguous() or a.is_cuda:
+        import torch
+        if tuple(a.shape) != (T, V, 12, 12) or not a.is_contiguous() or a.is_cuda or a.dtype != torch.complex128:
             raise WickError(f"{name} must be a contiguous CPU complex128 tensor [T][L^3][12][12]")
         return C.c_void_p(a.data_ptr())
 
@@ -287,6 +295,22 @@ def minor_dets(P, rows, cols, stream=None):
                                  _stream_ptr(stream))
     _check(rc, "wick_minor_dets")
     return out
+
+
+def minor_table(P, terms: Terms, flavour: int, flags: int = 0, stream=None):
+    """Unique-minor table of one flavour (0 = u, 1 = d) for the matrices P [n_sites][12][12], through the kernels
+    wick_contract uses for this handle.  Returns CUDA complex128 [n_minors][n_sites]."""
+    import torch
+    lib = load_library()
+    _check_dev(P, "P")
+    n_sites = P.shape[0]
+    n_pad = (n_sites + 31) // 32 * 32
+    nm = terms.info.n_minors_u if flavour == 0 else terms.info.n_minors_d
+    out = torch.zeros((nm, n_pad), dtype=torch.complex128, device=P.device)
+    with torch.cuda.device(P.device):
+        rc = lib.wick_terms_minor_table(P.data_ptr(), n_sites, terms._h, flavour, flags, out.data_ptr(), _stream_ptr(stream))
+    _check(rc, "wick_terms_minor_table")
+    return out[:, :n_sites]
 
 
 def release_cached_buffers() -> None:

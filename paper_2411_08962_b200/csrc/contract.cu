@@ -3,6 +3,7 @@
 // Every arithmetic step of the path runs in the kernels of kernels.cu.
 #include <algorithm>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <map>
 #include <string>
@@ -844,6 +845,9 @@ extern "C" int wick_contract(const void* U_dev, const void* D_dev, const wick_te
     if ((reinterpret_cast<uintptr_t>(U_dev) | reinterpret_cast<uintptr_t>(D_dev) | reinterpret_cast<uintptr_t>(C_out_dev) |
          reinterpret_cast<uintptr_t>(sigma_out_dev)) & 15) { set_error("wick_contract: buffers must be 16-byte aligned"); return WICK_ERR_ARG; }
     if (reinterpret_cast<uintptr_t>(workspace_dev) & 255) { set_error("wick_contract: workspace must be 256-byte aligned"); return WICK_ERR_ARG; }
+    if (t->needs_u_equals_d && U_dev != D_dev) {
+        set_error("wick_contract: this term list was built with WICK_BUILD_ISOSPIN (terms merged that are equal only for U == D); pass U_dev == D_dev");
+        return WICK_ERR_ARG; }
     Plan p;
     if (!make_plan(t, L, T, n_mom, workspace_bytes, false, &p)) { set_error("wick_contract: need L >= 1, T >= 1, n_mom >= 0"); return WICK_ERR_ARG; }
     if (p.S_b < GROUP) { set_error("wick_contract: workspace smaller than wick_contract_min_workspace_bytes()"); return WICK_ERR_WORKSPACE; }
@@ -932,6 +936,30 @@ extern "C" int wick_contract(const void* U_dev, const void* D_dev, const wick_te
     return WICK_OK;
 }
 
+// Step a4 for one flavour of a handle, through exactly the kernels wick_contract launches for it (tests: every minor of
+// the library's own tables against the oracle's elimination).
+extern "C" int wick_terms_minor_table(const void* P_dev, int64_t n_sites, const wick_terms* t, int flavour, unsigned flags,
+                                      void* out_dev, void* cuda_stream) {
+    if (!P_dev || !t || !out_dev || n_sites < 1 || n_sites > (int64_t(1) << 22) || (flavour != 0 && flavour != 1)) {
+        set_error("wick_terms_minor_table: bad argument"); return WICK_ERR_ARG; }
+    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    int rc = ensure_configured();
+    if (rc != WICK_OK) return rc;
+    if ((rc = upload_tables(t, stream)) != WICK_OK) return rc;
+    const FlavourTables& ft = t->f[flavour];
+    const int n_groups = int((n_sites + GROUP - 1) / GROUP);
+    const int S_b = n_groups * GROUP;
+    const int reg_bins = std::max(1, (148 + n_groups - 1) / n_groups) * (REG_THREADS / 32);
+    RegTables rt;
+    rc = (t->outer && !(flags & WICK_CONTRACT_NO_REG_MINORS)) ? ensure_reg(t, flavour, reg_bins, stream, &rt) : 0;
+    if (rc < 0) return rc;
+    if (rc == 1) WICK_CUDA(launch_minors_reg(ft.n, static_cast<const double2*>(P_dev), 0, n_sites, n_groups, S_b, rt,
+                                             static_cast<double2*>(out_dev), PROF_MINORS_U, stream));
+    else WICK_CUDA(launch_minors(ft.n, static_cast<const double2*>(P_dev), 0, n_sites, n_groups, S_b, t->dev.minor_desc[flavour],
+                                 int64_t(ft.minor_row.size()), true, static_cast<double2*>(out_dev), PROF_MINORS_U, stream));
+    return WICK_OK;
+}
+
 namespace {
 struct HostPathCache {
     enum Slot { U0 = 0, U1, D0, D1, WS, C, S, N_SLOTS };
@@ -992,7 +1020,12 @@ extern "C" int wick_contract_host(const void* U_host, const void* D_host, const 
     // Each block is an independent wick_contract over Tb timeslices (per-timeslice results do not
     // depend on the blocking: the reduction over sites of one timeslice always has the same shape).
     const size_t slice_bytes = size_t(V) * 144 * 16;
-    int Tb = int(std::max<size_t>(1, (size_t(256) << 20) / slice_bytes));
+    size_t block_bytes = size_t(256) << 20;
+    if (const char* ev = std::getenv("WICK_HOST_BLOCK_BYTES")) {   // test hook: small blocks exercise the double-buffered path
+        const long long v = std::atoll(ev);
+        if (v > 0) block_bytes = size_t(v);
+    }
+    int Tb = int(std::max<size_t>(1, block_bytes / slice_bytes));
     Tb = std::min(Tb, T);
     const size_t ws_bytes = wick_contract_workspace_bytes(t, L, Tb, n_mom);
     if (!ws_bytes) { set_error("wick_contract_host: bad sizes"); return WICK_ERR_ARG; }
@@ -1001,7 +1034,8 @@ extern "C" int wick_contract_host(const void* U_host, const void* D_host, const 
     // more than the contraction of a small lattice
     HostPathCache& hc = host_path_cache();
     int rc = WICK_OK;
-    auto cleanup = [&]() {};
+    // on any exit both streams are drained: no copy from the caller's host buffers may still be pending
+    auto cleanup = [&]() { if (hc.sc) cudaStreamSynchronize(hc.sc); if (hc.sx) cudaStreamSynchronize(hc.sx); };
 #define WICK_CUDA_H(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) { set_error(std::string(#call) + ": " + cudaGetErrorString(e_)); cleanup(); return WICK_ERR_CUDA; } } while (0)
     WICK_CUDA_H(hc.prepare());
     void *dU[2], *dD[2], *ws = nullptr, *dC = nullptr, *dS = nullptr;
@@ -1017,13 +1051,14 @@ extern "C" int wick_contract_host(const void* U_host, const void* D_host, const 
     if (sigma_out_host) WICK_CUDA_H(hc.acquire(HostPathCache::S, size_t(V) * Tb * 16, &dS));
     const unsigned char* Uh = static_cast<const unsigned char*>(U_host);
     const unsigned char* Dh = static_cast<const unsigned char*>(D_host);
+    const bool alias = (U_host == D_host);                     // isospin limit: one propagator, copied once, U_dev == D_dev
     std::vector<double> Cblk(size_t(std::max(n_mom, 1)) * Tb * 2);
     const int n_blocks = (T + Tb - 1) / Tb;
     auto issue_copy = [&](int b) -> cudaError_t {
         const int k = b & 1, t0 = b * Tb, nt = std::min(Tb, T - t0);
         cudaError_t e = cudaStreamWaitEvent(sx, consumed[k], 0);
         if (e == cudaSuccess) e = cudaMemcpyAsync(dU[k], Uh + size_t(t0) * slice_bytes, slice_bytes * nt, cudaMemcpyHostToDevice, sx);
-        if (e == cudaSuccess) e = cudaMemcpyAsync(dD[k], Dh + size_t(t0) * slice_bytes, slice_bytes * nt, cudaMemcpyHostToDevice, sx);
+        if (e == cudaSuccess && !alias) e = cudaMemcpyAsync(dD[k], Dh + size_t(t0) * slice_bytes, slice_bytes * nt, cudaMemcpyHostToDevice, sx);
         if (e == cudaSuccess) e = cudaEventRecord(copied[k], sx);
         return e;
     };
@@ -1032,7 +1067,7 @@ extern "C" int wick_contract_host(const void* U_host, const void* D_host, const 
         const int k = b & 1, t0 = b * Tb, nt = std::min(Tb, T - t0);
         if (b + 1 < n_blocks) WICK_CUDA_H(issue_copy(b + 1));
         WICK_CUDA_H(cudaStreamWaitEvent(sc, copied[k], 0));
-        rc = wick_contract(dU[k], dD[k], t, momenta, n_mom, L, nt, dC, dS, ws, ws_bytes, flags, sc);
+        rc = wick_contract(dU[k], alias ? dU[k] : dD[k], t, momenta, n_mom, L, nt, dC, dS, ws, ws_bytes, flags, sc);
         if (rc != WICK_OK) break;
         WICK_CUDA_H(cudaEventRecord(consumed[k], sc));
         WICK_CUDA_H(cudaMemcpyAsync(Cblk.data(), dC, size_t(n_mom) * nt * 16, cudaMemcpyDeviceToHost, sc));
@@ -1043,7 +1078,6 @@ extern "C" int wick_contract_host(const void* U_host, const void* D_host, const 
         for (int m = 0; m < n_mom; ++m)
             std::memcpy(Co + (size_t(m) * T + t0) * 2, Cblk.data() + size_t(m) * nt * 2, size_t(nt) * 16);
     }
-    WICK_CUDA_H(cudaStreamSynchronize(sx));
     cleanup();
 #undef WICK_CUDA_H
     return rc;

@@ -297,6 +297,43 @@ static void grid_minors(FlavourTables& ft) {
 
 // ---------------------------------------------------------------------------------------------
 // C-ABI
+// Isospin limit U == D (the paper's m_u = m_d) for an outer-product list whose flavours share their row
+// tuples: with M = MU = MD the product of sink term (a_u, a_d) and source term (b_u, b_d) equals the product of the
+// swapped terms (a_d, a_u), (b_d, b_u).  If the sink list is symmetric under the swap up to one global sign s
+// (c(a_d, a_u) = s c(a_u, a_d); the source list is its conjugate), the sum over sink terms with a_u > a_d equals the
+// sum over those with a_u < a_d, so the list   { 2 c_i : a_u < a_d } + { c_i : a_u = a_d }   x   full source list
+// gives the same correlator with about half the products -- and it is still an outer product, so it runs through the
+// factorised reduction.  This is the swap-class merge the randomised identity test finds (Sec. III B),
+// applied in factorised form.  Returns false (list untouched) when the symmetry does not hold.
+static bool symmetrise_isospin(wick_terms* t) {
+    if (!t->outer || t->n_u != t->n_d || t->f[0].rows != t->f[1].rows || t->f[0].cols != t->f[1].cols) return false;
+    std::map<std::pair<int32_t, int32_t>, cplx> c;
+    for (const FactorTerm& f : t->sink) c[{f.qu, f.qd}] = f.c;
+    double s = 0.0;
+    for (const FactorTerm& f : t->sink) {
+        auto it = c.find({f.qd, f.qu});
+        if (it == c.end()) return false;
+        if (f.qu == f.qd) continue;
+        const double want = (it->second == f.c) ? 1.0 : (it->second == -f.c ? -1.0 : 0.0);
+        if (want == 0.0 || (s != 0.0 && want != s)) return false;
+        s = want;
+    }
+    if (s < 0.0)
+        for (const FactorTerm& f : t->sink) if (f.qu == f.qd) return false;   // c = -c: cannot be present
+    std::vector<FactorTerm> half;
+    for (const FactorTerm& f : t->sink) {
+        if (f.qu > f.qd) continue;
+        FactorTerm g = f;
+        if (f.qu < f.qd) g.c *= 2.0;
+        half.push_back(g);
+    }
+    t->sink.swap(half);
+    t->n_terms = int64_t(t->sink.size()) * int64_t(t->source.size());
+    t->flat_ready = false;
+    t->needs_u_equals_d = true;
+    return true;
+}
+
 // ---------------------------------------------------------------------------------------------
 
 extern "C" const char* wick_last_error(void) { return g_error.c_str(); }
@@ -362,7 +399,11 @@ extern "C" int wick_build_terms(const wick_nucleon* nucleons, int n_nucleons, un
         t->n_terms = int64_t(t->sink.size()) * int64_t(t->source.size());
         grid_minors(t->f[0]);
         grid_minors(t->f[1]);
-        if (flags & WICK_BUILD_IDENTITY_TEST) t->n_identity_merged = identity_test(t, flags, seed);
+        if ((flags & WICK_BUILD_ISOSPIN) && !(flags & WICK_BUILD_IDENTITY_TEST)) symmetrise_isospin(t);
+        if (flags & WICK_BUILD_IDENTITY_TEST) {
+            t->n_identity_merged = identity_test(t, flags, seed);
+            if ((flags & WICK_BUILD_ISOSPIN) && t->n_identity_merged > 0) t->needs_u_equals_d = true;
+        }
         *out = t;
         return WICK_OK;
     } catch (const std::bad_alloc&) {
@@ -450,7 +491,10 @@ extern "C" int wick_build_terms_from_list(int n_u, int n_d, int64_t n_raw, const
         t->flat_ready = true;
         t->outer = false;
         t->n_terms = int64_t(t->t_w.size());
-        if (flags & WICK_BUILD_IDENTITY_TEST) t->n_identity_merged = identity_test(t, flags, seed);
+        if (flags & WICK_BUILD_IDENTITY_TEST) {
+            t->n_identity_merged = identity_test(t, flags, seed);
+            if ((flags & WICK_BUILD_ISOSPIN) && t->n_identity_merged > 0) t->needs_u_equals_d = true;
+        }
         *out = t;
         return WICK_OK;
     } catch (const std::bad_alloc&) {

@@ -85,6 +85,7 @@ struct wick_terms {
     int n_u = 0, n_d = 0;
     wick::FlavourTables f[2];                   // 0 = u, 1 = d
     bool outer = false;
+    bool needs_u_equals_d = false;              // built with WICK_BUILD_ISOSPIN and changed by it: only valid for U == D
     std::vector<wick::FactorTerm> sink, source; // outer-product factor lists (source holds conj c_j)
     int64_t n_terms = 0, n_raw = 0, n_identity_merged = 0;
     // flat list: always present for generic lists, materialised on demand for outer-product lists
