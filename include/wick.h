@@ -54,6 +54,9 @@ extern "C" {
 #define WICK_CONTRACT_FORCE_FLAT 1u  /* use the flat (uid, did, w) term list even if a factorised form exists */
 #define WICK_CONTRACT_COMPLEX_COEFFS 4u /* staged reduction: do not use the cheaper entries for all-real factor coefficients */
 #define WICK_CONTRACT_NO_REG_MINORS 8u /* 6x6 grid tables: use the shared-memory Schur-column cache kernel instead of the register-resident one */
+#define WICK_CONTRACT_JACOBI    16u  /* flavours with 8 <= n <= 11: Jacobi's complementary-minor identity (one 12x12 inverse + determinant */
+                                     /* per site, then (12-n) x (12-n) minors of the inverse) instead of an LU per minor.  Error grows  */
+                                     /* with the condition number of the propagator and a singular propagator contributes 0: opt-in.   */
 #define WICK_CONTRACT_NO_STAGED  2u  /* factorised lists: walk the block items from L1/L2 instead of staging them in shared memory */
 
 #define WICK_NUCLEON_PROTON  0
@@ -105,6 +108,33 @@ int wick_build_terms_from_list(int n_u, int n_d, int64_t n_raw,
                                const uint8_t* a_u, const uint8_t* b_u,
                                const uint8_t* a_d, const uint8_t* b_d,
                                const double* w_reim, unsigned flags, uint64_t seed, wick_terms** out);
+
+/* ---- general interpolators and correlation matrices (GEVP, Sec. V, Eq. 36-38) ----------------------
+ * A wick_operator is an interpolator in canonical form: monomial (u tuple, d tuple) -> complex coefficient.
+ *   _from_nucleons : the ordered product of BASELINE nucleons (the sink list wick_build_terms uses);
+ *   _from_raw      : any operator given as raw monomials: n_raw products of n_quarks quark fields in operator order,
+ *                    flavour[k][q] in {0 = u, 1 = d}, chi[k][q] = 3*spin + colour, coefficient coef_reim[k];
+ *                    sorted with the permutation sign (Eq. 19), merged, Pauli zeros dropped;
+ *   _paper         : the paper's own interpolators built from the nucleons of Eq. (4)/(5) and the
+ *                    projected ones of Eq. (26)/(27) (:271-273): WICK_OP_DEUTERON_EQ20 = n^T (C g5 P+) p  (Eq. 20 :256, 356
+ *                    terms, Table II :305); WICK_OP_HELIUM3_EQ21 = p_-^T (C g5) n_+ p_+^J  (Eq. 21 :258; 1026 terms per
+ *                    spin component for J = 2, 3, Table II :306).
+ * wick_build_terms_matrix: n_ops operators with the same quark content -> n_ops^2 handles, out[k * n_ops + k'] =
+ * (operator k at the sink) x conj(operator k' at the source), all over ONE pair of unique-minor tables (union of the row /
+ * column tuples), so that wick_contract_many evaluates every determinant once for the whole correlation matrix.
+ * Each handle is an ordinary wick_terms (free every one with wick_terms_free). */
+typedef struct wick_operator wick_operator;
+#define WICK_OP_DEUTERON_EQ20 1
+#define WICK_OP_HELIUM3_EQ21  2
+int  wick_operator_from_nucleons(const wick_nucleon* nucleons, int n_nucleons, wick_operator** out);
+int  wick_operator_from_raw(int n_quarks, int64_t n_raw, const uint8_t* flavour, const uint8_t* chi, const double* coef_reim,
+                            wick_operator** out);
+int  wick_operator_paper(int which, int J, wick_operator** out);
+int  wick_operator_info(const wick_operator* op, int32_t* n_u, int32_t* n_d, int64_t* n_terms);
+/* u_tuples uint8 [n_terms][n_u], d_tuples uint8 [n_terms][n_d] (ascending), coef_reim double [n_terms][2]; any may be NULL */
+int  wick_operator_export(const wick_operator* op, uint8_t* u_tuples, uint8_t* d_tuples, double* coef_reim);
+void wick_operator_free(wick_operator* op);
+int  wick_build_terms_matrix(const wick_operator* const* ops, int n_ops, unsigned flags, wick_terms** out);
 
 int  wick_terms_get_info(const wick_terms* terms, wick_terms_info* info);
 
@@ -168,6 +198,16 @@ int wick_contract(const void* U_dev, const void* D_dev, const wick_terms* terms,
                   const int32_t* momenta, int n_mom, int L, int T,
                   void* C_out_dev, void* sigma_out_dev,
                   void* workspace_dev, size_t workspace_bytes, unsigned flags, void* cuda_stream);
+
+/* Correlation matrix (GEVP, Sec. V, Eq. 36-38): n_lists term lists that share their unique-minor tables
+ * (wick_build_terms_matrix).  Per site batch every determinant is evaluated ONCE (step a4), then each list runs its own
+ * weighted-product kernel (a5) and projection (a6).  C_out_dev: device complex128 [n_lists][n_mom][T]; sigma_out_dev: NULL or
+ * [n_lists][T][L^3]; workspace of at least wick_contract_many_workspace_bytes (the single-list sizes plus one sigma buffer per
+ * extra list).  Everything else as wick_contract.  WICK_ERR_UNSUPPORTED if the lists do not share their tables. */
+size_t wick_contract_many_workspace_bytes(const wick_terms* terms0, int n_lists, int L, int T, int n_mom);
+int wick_contract_many(const void* U_dev, const void* D_dev, const wick_terms* const* lists, int n_lists,
+                       const int32_t* momenta, int n_mom, int L, int T, void* C_out_dev, void* sigma_out_dev,
+                       void* workspace_dev, size_t workspace_bytes, unsigned flags, void* cuda_stream);
 
 /* Same computation from HOST buffers (U_host, D_host, C_out_host, sigma_out_host: host memory,
  * pinned or pageable, same layouts).  Allocates device memory itself, streams the propagators

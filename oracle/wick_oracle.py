@@ -110,6 +110,81 @@ def nucleus_raw_terms(nucleus: Sequence[Tuple[str, int]]) -> List[RawTerm]:
     return terms
 
 
+# ---- the paper's own interpolators (Eq. 4, 5, 20, 21, 26, 27): used for the GEVP correlation-matrix checks ----------------
+
+def spin_projector(sign: int) -> np.ndarray:
+    """P_+- = (1 +- gamma4) / 2 (below Eq. 27): diag(1,1,0,0) / diag(0,0,1,1) in the Dirac-Pauli basis."""
+    g4 = gamma_matrices()[3]
+    return ((np.eye(4) + sign * g4) / 2).real
+
+
+def paper_nucleon_raw_terms(kind: str, alpha: int, projector: int = 0) -> List[RawTerm]:
+    """Eq. (4)/(5):  p_alpha = eps_abc u^a_alpha u^b_beta (C gamma5)_{beta eta} d^c_eta  (n: u <-> d),
+    quark order as written; projector = +-1 inserts P_+- as in Eq. (26)/(27), PAPER.md:271-273:
+    (p_+-)_alpha = eps_abc u^a_alpha u^b_beta (C gamma5 P_+-)_{beta delta} d^c_delta."""
+    f1, f2 = ("u", "d") if kind == "p" else ("d", "u")
+    eps = levi_civita()
+    M = c_gamma5() if projector == 0 else c_gamma5() @ spin_projector(projector)
+    out: List[RawTerm] = []
+    for a in range(3):
+        for b in range(3):
+            for c in range(3):
+                if eps[a, b, c] == 0:
+                    continue
+                for beta in range(4):
+                    for delta in range(4):
+                        if M[beta, delta] == 0:
+                            continue
+                        out.append((eps[a, b, c] * M[beta, delta], ((f1, 3 * alpha + a), (f1, 3 * beta + b), (f2, 3 * delta + c))))
+    return out
+
+
+def _raw_product(*factors: Sequence[RawTerm]) -> List[RawTerm]:
+    terms: List[RawTerm] = [(1.0, ())]
+    for f in factors:
+        terms = [(c1 * c2, q1 + q2) for (c1, q1) in terms for (c2, q2) in f]
+    return terms
+
+
+def deuteron_eq20_raw_terms() -> List[RawTerm]:
+    """Eq. (20):  O_2H = n^T (C gamma5 P_+) p = sum_{alpha beta} n_alpha (C gamma5 P_+)_{alpha beta} p_beta
+    with the nucleons of Eq. (4)/(5)."""
+    M = c_gamma5() @ spin_projector(+1)
+    out: List[RawTerm] = []
+    for alpha in range(4):
+        for beta in range(4):
+            if M[alpha, beta] != 0:
+                out += [(M[alpha, beta] * c, q) for (c, q) in
+                        _raw_product(paper_nucleon_raw_terms("n", alpha), paper_nucleon_raw_terms("p", beta))]
+    return out
+
+
+def helium3_eq21_raw_terms(J: int) -> List[RawTerm]:
+    """Eq. (21), PAPER.md:258:  O^J_3He = p_-^T (C gamma5) n_+ p_+^J = sum_{alpha beta} (p_-)_alpha (C gamma5)_{alpha beta}
+    (n_+)_beta (p_+)_J  with the projected nucleons of Eq. (26)/(27).  The paper does not say which Dirac components the
+    open index J runs over; the printed 1026 terms per spin component select J in {2, 3} (DESIGN.md reading)."""
+    M = c_gamma5()
+    out: List[RawTerm] = []
+    for alpha in range(4):
+        for beta in range(4):
+            if M[alpha, beta] != 0:
+                out += [(M[alpha, beta] * c, q) for (c, q) in
+                        _raw_product(paper_nucleon_raw_terms("p", alpha, -1), paper_nucleon_raw_terms("n", beta, +1),
+                                     paper_nucleon_raw_terms("p", J, +1))]
+    return out
+
+
+def merged_from_raw(raw: Sequence[RawTerm]):
+    """Polynomial normal form of any raw operator: canonical monomials with their accumulated coefficients, zeros
+    dropped, sorted by (u_tuple, d_tuple) -- "the number of terms in the operator" of Table II."""
+    acc: Dict[Tuple[tuple, tuple], complex] = {}
+    for c, q in raw:
+        sign, u, d = canonical_monomial(q)
+        if sign:
+            acc[(u, d)] = acc.get((u, d), 0.0) + sign * c
+    return [(u, d, acc[(u, d)]) for (u, d) in sorted(acc) if acc[(u, d)] != 0]
+
+
 def sort_with_sign(seq: Sequence) -> Tuple[int, tuple]:
     """Sort a sequence of distinct comparable items ascending; return (sign, sorted tuple), sign =
     parity of the number of inversions (Eq. 19).  A repeated item gives sign 0

@@ -21,6 +21,7 @@ CONTRACT_FORCE_FLAT = 1
 CONTRACT_NO_STAGED = 2
 CONTRACT_COMPLEX_COEFFS = 4
 CONTRACT_NO_REG_MINORS = 8
+CONTRACT_JACOBI = 16
 
 EXPORTED_SYMBOLS = (
     "wick_build_terms", "wick_build_terms_from_list", "wick_terms_get_info", "wick_terms_export_tuples",
@@ -28,6 +29,8 @@ EXPORTED_SYMBOLS = (
     "wick_terms_staged_schedule_check", "wick_terms_export_minor_order", "wick_terms_free",
     "wick_contract_min_workspace_bytes", "wick_contract_workspace_bytes", "wick_contract",
     "wick_contract_host", "wick_release_cached_buffers", "wick_minor_dets", "wick_terms_minor_table", "wick_launch_count", "wick_launch_count_reset",
+    "wick_operator_from_nucleons", "wick_operator_from_raw", "wick_operator_paper", "wick_operator_info", "wick_operator_export",
+    "wick_operator_free", "wick_build_terms_matrix", "wick_contract_many", "wick_contract_many_workspace_bytes",
     "wick_last_error", "wick_version", "wick_profile_enable", "wick_profile_read", "wick_measure_fp64_peak",
 )
 
@@ -88,6 +91,17 @@ def load_library():
     lib.wick_contract_host.argtypes = [vp, vp, vp, vp, i32, i32, i32, vp, vp, u32]
     lib.wick_minor_dets.argtypes = [vp, i64, i32, vp, vp, i64, vp, vp]
     lib.wick_terms_minor_table.argtypes = [vp, i64, vp, i32, u32, vp, vp]
+    lib.wick_operator_from_nucleons.argtypes = [C.POINTER(_Nucleon), i32, C.POINTER(vp)]
+    lib.wick_operator_from_raw.argtypes = [i32, i64, vp, vp, vp, C.POINTER(vp)]
+    lib.wick_operator_paper.argtypes = [i32, i32, C.POINTER(vp)]
+    lib.wick_operator_info.argtypes = [vp, C.POINTER(C.c_int32), C.POINTER(C.c_int32), C.POINTER(i64)]
+    lib.wick_operator_export.argtypes = [vp, vp, vp, vp]
+    lib.wick_operator_free.argtypes = [vp]
+    lib.wick_operator_free.restype = None
+    lib.wick_build_terms_matrix.argtypes = [C.POINTER(vp), i32, u32, C.POINTER(vp)]
+    lib.wick_contract_many_workspace_bytes.argtypes = [vp, i32, i32, i32, i32]
+    lib.wick_contract_many_workspace_bytes.restype = sz
+    lib.wick_contract_many.argtypes = [vp, vp, C.POINTER(vp), i32, vp, i32, i32, i32, vp, vp, vp, sz, u32, vp]
     lib.wick_profile_enable.argtypes = [i32]
     lib.wick_profile_read.argtypes = [C.POINTER(Profile)]
     lib.wick_measure_fp64_peak.argtypes = [C.POINTER(C.c_double), vp]
@@ -204,6 +218,99 @@ def build_terms_from_list(a_u, b_u, a_d, b_d, w, flags: int = 0, seed: int = 0) 
     _check(lib.wick_build_terms_from_list(n_u, n_d, n_raw, _np_ptr(a_u), _np_ptr(b_u), _np_ptr(a_d), _np_ptr(b_d),
                                           _np_ptr(w), flags, seed, C.byref(h)), "wick_build_terms_from_list")
     return Terms(h.value)
+
+
+OP_DEUTERON_EQ20 = 1
+OP_HELIUM3_EQ21 = 2
+
+
+class Operator:
+    """Handle of an interpolator in canonical form (wick_operator*): monomial (u tuple, d tuple) -> coefficient."""
+
+    def __init__(self, handle):
+        self._h = C.c_void_p(handle)
+        nu, nd, nt = C.c_int32(0), C.c_int32(0), C.c_int64(0)
+        _check(load_library().wick_operator_info(self._h, C.byref(nu), C.byref(nd), C.byref(nt)), "wick_operator_info")
+        self.n_u, self.n_d, self.n_terms = int(nu.value), int(nd.value), int(nt.value)
+
+    def __del__(self):
+        h, self._h = getattr(self, "_h", None), None
+        if h and _lib is not None:
+            _lib.wick_operator_free(h)
+
+    def terms(self):
+        """(u_tuples [n_terms][n_u], d_tuples [n_terms][n_d], coefficients [n_terms])."""
+        u = np.zeros((self.n_terms, self.n_u), np.uint8)
+        d = np.zeros((self.n_terms, self.n_d), np.uint8)
+        c = np.zeros(self.n_terms, np.complex128)
+        _check(_lib.wick_operator_export(self._h, _np_ptr(u), _np_ptr(d), _np_ptr(c)), "wick_operator_export")
+        return u, d, c
+
+
+def operator_from_nucleons(nucleus: Sequence[Tuple[str, int]]) -> Operator:
+    lib = load_library()
+    arr = (_Nucleon * max(len(nucleus), 1))()
+    for k, (kind, gamma) in enumerate(nucleus):
+        if kind not in ("p", "n"):
+            raise WickError(f"nucleon kind must be 'p' or 'n', got {kind!r}")
+        arr[k].kind = 0 if kind == "p" else 1
+        arr[k].gamma = int(gamma)
+    h = C.c_void_p()
+    _check(lib.wick_operator_from_nucleons(arr, len(nucleus), C.byref(h)), "wick_operator_from_nucleons")
+    return Operator(h.value)
+
+
+def operator_from_raw(flavour, chi, coef) -> Operator:
+    """flavour, chi: [n_raw][n_quarks] (0 = u, 1 = d; chi = 3*spin + colour) in operator order; coef [n_raw] complex."""
+    lib = load_library()
+    flavour = np.ascontiguousarray(flavour, dtype=np.uint8)
+    chi = np.ascontiguousarray(chi, dtype=np.uint8)
+    coef = np.ascontiguousarray(coef, dtype=np.complex128)
+    n_raw = len(coef)
+    n_q = flavour.shape[1] if flavour.ndim == 2 else 0
+    h = C.c_void_p()
+    _check(lib.wick_operator_from_raw(n_q, n_raw, _np_ptr(flavour), _np_ptr(chi), _np_ptr(coef), C.byref(h)), "wick_operator_from_raw")
+    return Operator(h.value)
+
+
+def operator_paper(which: int, J: int = 0) -> Operator:
+    """The paper's interpolators: OP_DEUTERON_EQ20 (Eq. 20) or OP_HELIUM3_EQ21 (Eq. 21, open index J)."""
+    h = C.c_void_p()
+    _check(load_library().wick_operator_paper(which, J, C.byref(h)), "wick_operator_paper")
+    return Operator(h.value)
+
+
+def build_terms_matrix(ops: Sequence[Operator], flags: int = 0):
+    """K operators -> K x K nested list of Terms, [k][k'] = (operator k at the sink) x conj(operator k' at the source),
+    all over one pair of unique-minor tables (for contract_many)."""
+    lib = load_library()
+    K = len(ops)
+    arr = (C.c_void_p * max(K, 1))(*[o._h for o in ops])
+    out = (C.c_void_p * max(K * K, 1))()
+    _check(lib.wick_build_terms_matrix(arr, K, flags, out), "wick_build_terms_matrix")
+    return [[Terms(out[k * K + kp]) for kp in range(K)] for k in range(K)]
+
+
+def contract_many(U, D, terms_list: Sequence[Terms], momenta, L: int, T: int, want_sigma: bool = False, flags: int = 0,
+                  stream=None):
+    """C[list][p][t] for term lists that share their unique-minor tables (wick_contract_many): the determinants are
+    evaluated once per site for all lists.  Returns C (CUDA complex128 [n_lists][n_mom][T]) or (C, sigma [n_lists][T][L^3])."""
+    import torch
+    lib = load_library()
+    V = L ** 3
+    _check_dev(U, "U", (T, V, 12, 12))
+    _check_dev(D, "D", (T, V, 12, 12))
+    mom = np.ascontiguousarray(momenta, dtype=np.int32).reshape(-1, 3)
+    n_mom, n = mom.shape[0], len(terms_list)
+    arr = (C.c_void_p * max(n, 1))(*[t._h for t in terms_list])
+    with torch.cuda.device(U.device), torch.cuda.stream(torch.cuda.current_stream() if stream is None else stream):
+        ws = torch.empty(int(lib.wick_contract_many_workspace_bytes(terms_list[0]._h, n, L, T, n_mom)), dtype=torch.uint8, device=U.device)
+        Cout = torch.empty((n, n_mom, T), dtype=torch.complex128, device=U.device)
+        sigma = torch.empty((n, T, V), dtype=torch.complex128, device=U.device) if want_sigma else None
+        rc = lib.wick_contract_many(U.data_ptr(), D.data_ptr(), arr, n, _np_ptr(mom), n_mom, L, T, Cout.data_ptr(),
+                                    None if sigma is None else sigma.data_ptr(), ws.data_ptr(), ws.numel(), flags, _stream_ptr(stream))
+    _check(rc, "wick_contract_many")
+    return (Cout, sigma) if want_sigma else Cout
 
 
 def _stream_ptr(stream):

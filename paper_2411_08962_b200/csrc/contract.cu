@@ -143,6 +143,22 @@ std::vector<uint64_t> build_minor_descs(const FlavourTables& ft) {
     return desc;
 }
 
+// Jacobi path (flag WICK_CONTRACT_JACOBI, n >= 8): descriptors of the complementary minors.  Minor (I, J) of A equals
+// (-1)^(sum I + sum J) det A det (A^-1)[J^c, I^c] (0-based index sums): rows J^c, columns I^c, the sign in bit 31.
+std::vector<uint64_t> build_jacobi_descs(const FlavourTables& ft) {
+    const int m = 12 - ft.n;
+    std::vector<uint64_t> desc(ft.minor_row.size());
+    for (size_t k = 0; k < desc.size(); ++k) {
+        const uint16_t I = ft.rows[size_t(ft.minor_row[k])], J = ft.cols[size_t(ft.minor_col[k])];
+        int sum = 0;
+        for (int b = 0; b < 12; ++b) sum += ((I >> b) & 1) * b + ((J >> b) & 1) * b;
+        const uint64_t rows = nibbles_of_mask(uint16_t(~J & 0xfff)), cols = nibbles_of_mask(uint16_t(~I & 0xfff));
+        pack_minor_desc(m, rows, cols, uint32_t(k), false, &desc[k]);
+        if (sum & 1) desc[k] |= uint64_t(1) << 31;
+    }
+    return desc;
+}
+
 // Connected components of the bipartite graph (qu -- qd) of a factor list.  Physical sink lists are
 // block diagonal (He-4: 199 blocks of at most 15 x 15 tuples), so the factorised reduction
 //   sigma = sum_{ru,cd} (sum_i c_i MD[rd_i,cd]) (sum_j cbar_j MU[ru,cu_j])
@@ -253,12 +269,16 @@ int upload_tables(const wick_terms* t, cudaStream_t stream) {
     if (d.blob && d.device == dev) return WICK_OK;
     if (d.blob) { set_error("wick_terms handle was first used on another device"); return WICK_ERR_ARG; }
     BlobBuilder bb;
-    size_t o_desc[2];
+    size_t o_desc[2], o_jac[2] = {0, 0};
     for (int f = 0; f < 2; ++f) {
         const FlavourTables& ft = t->f[f];
         if (ft.minor_row.size() >= (size_t(1) << 31)) { set_error("more than 2^31 unique minors"); return WICK_ERR_UNSUPPORTED; }
         const std::vector<uint64_t> desc = build_minor_descs(ft);
         o_desc[f] = bb.add(desc.data(), desc.size() * 8);
+        if (ft.n >= 8 && ft.n <= 11) {
+            const std::vector<uint64_t> jd = build_jacobi_descs(ft);
+            o_jac[f] = bb.add(jd.data(), jd.size() * 8);
+        }
     }
     size_t o_sp = 0, o_srd = 0, o_sc = 0, o_qp = 0, o_qcu = 0, o_qc = 0;
     size_t o_srdoff = 0, o_rup = 0, o_rul = 0, o_cdp = 0, o_cdl = 0, o_binp = 0, o_items = 0;
@@ -305,7 +325,10 @@ int upload_tables(const wick_terms* t, cudaStream_t stream) {
     if (e == cudaSuccess) e = cudaStreamSynchronize(stream);   // bb.host dies at scope exit
     if (e != cudaSuccess) { cudaFree(blob); set_error(std::string("table upload: ") + cudaGetErrorString(e)); return WICK_ERR_CUDA; }
     unsigned char* b = static_cast<unsigned char*>(blob);
-    for (int f = 0; f < 2; ++f) d.minor_desc[f] = b + o_desc[f];
+    for (int f = 0; f < 2; ++f) {
+        d.minor_desc[f] = b + o_desc[f];
+        d.jacobi_desc[f] = (t->f[f].n >= 8 && t->f[f].n <= 11) ? b + o_jac[f] : nullptr;
+    }
     if (t->outer) {
         d.sink_ptr = reinterpret_cast<const int32_t*>(b + o_sp);
         d.sink_rd = reinterpret_cast<const int32_t*>(b + o_srd);
@@ -701,6 +724,7 @@ int upload_flat(const wick_terms* t, cudaStream_t stream) {
 // ---- workspace plan --------------------------------------------------------------------------
 constexpr int MAX_CHUNKS = 256;                  // rows of the partial buffer
 constexpr size_t TARGET_MINOR_BYTES = size_t(2) << 30;
+constexpr int64_t JACOBI_BYTES_PER_ST = (144 + 1) * 16;   // inverse propagator + determinant of one flavour
 
 struct Plan {
     int64_t n_st = 0;                            // site-times T * L^3
@@ -709,12 +733,12 @@ struct Plan {
     int64_t S_b = 0;                             // site-times per batch (multiple of 32)
 };
 
-bool make_plan(const wick_terms* t, int L, int T, int n_mom, size_t workspace_bytes, bool want_max, Plan* p) {
-    if (!t || L < 1 || T < 1 || n_mom < 0 || int64_t(L) * L * L > (int64_t(1) << 31) - 1) return false;
+bool make_plan(const wick_terms* t, int n_lists, int L, int T, int n_mom, size_t workspace_bytes, bool want_max, Plan* p) {
+    if (!t || n_lists < 1 || L < 1 || T < 1 || n_mom < 0 || int64_t(L) * L * L > (int64_t(1) << 31) - 1) return false;
     p->n_st = int64_t(T) * L * L * L;
     const int64_t nm = int64_t(t->f[0].minor_row.size()) + int64_t(t->f[1].minor_row.size());
-    p->per_st = (nm + MAX_CHUNKS) * 16;
-    p->sigma_bytes = align_up(size_t(p->n_st) * 16, 256);
+    p->per_st = (nm + MAX_CHUNKS) * 16 + 2 * JACOBI_BYTES_PER_ST;   // the Jacobi buffers are always planned for, so one size serves every flag
+    p->sigma_bytes = align_up(size_t(n_lists) * size_t(p->n_st) * 16, 256);
     const int64_t n_st_pad = (p->n_st + GROUP - 1) / GROUP * GROUP;
     int64_t sb;
     if (want_max) {
@@ -827,42 +851,56 @@ extern "C" int wick_measure_fp64_peak(double* tflops_out, void* cuda_stream) {
 
 extern "C" size_t wick_contract_min_workspace_bytes(const wick_terms* t, int L, int T, int n_mom) {
     Plan p;
-    if (!make_plan(t, L, T, n_mom, 0, true, &p)) return 0;
+    if (!make_plan(t, 1, L, T, n_mom, 0, true, &p)) return 0;
     return plan_bytes(p, GROUP);
 }
 
 extern "C" size_t wick_contract_workspace_bytes(const wick_terms* t, int L, int T, int n_mom) {
     Plan p;
-    if (!make_plan(t, L, T, n_mom, 0, true, &p)) return 0;
+    if (!make_plan(t, 1, L, T, n_mom, 0, true, &p)) return 0;
     return plan_bytes(p, p.S_b);
 }
 
-extern "C" int wick_contract(const void* U_dev, const void* D_dev, const wick_terms* t, const int32_t* momenta,
-                             int n_mom, int L, int T, void* C_out_dev, void* sigma_out_dev, void* workspace_dev,
-                             size_t workspace_bytes, unsigned flags, void* cuda_stream) {
-    if (!U_dev || !D_dev || !t || !C_out_dev || !workspace_dev || (n_mom > 0 && !momenta)) {
-        set_error("wick_contract: NULL argument"); return WICK_ERR_ARG; }
+namespace {
+
+// The hot path for n_lists term lists over ONE pair of unique-minor tables (lists[0]'s): per site batch the minors are
+// evaluated once, then every list runs its own weighted-product kernel into its own sigma; n_lists = 1 is wick_contract.
+int contract_lists(const void* U_dev, const void* D_dev, const wick_terms* const* lists, int n_lists, const int32_t* momenta,
+                   int n_mom, int L, int T, void* C_out_dev, void* sigma_out_dev, void* workspace_dev,
+                   size_t workspace_bytes, unsigned flags, void* cuda_stream, const char* who) {
+    auto fail = [&](const char* msg, int code) { set_error(std::string(who) + ": " + msg); return code; };
+    if (!U_dev || !D_dev || !lists || n_lists < 1 || !C_out_dev || !workspace_dev || (n_mom > 0 && !momenta)) return fail("NULL argument", WICK_ERR_ARG);
+    for (int k = 0; k < n_lists; ++k) if (!lists[k]) return fail("NULL argument", WICK_ERR_ARG);
     if ((reinterpret_cast<uintptr_t>(U_dev) | reinterpret_cast<uintptr_t>(D_dev) | reinterpret_cast<uintptr_t>(C_out_dev) |
-         reinterpret_cast<uintptr_t>(sigma_out_dev)) & 15) { set_error("wick_contract: buffers must be 16-byte aligned"); return WICK_ERR_ARG; }
-    if (reinterpret_cast<uintptr_t>(workspace_dev) & 255) { set_error("wick_contract: workspace must be 256-byte aligned"); return WICK_ERR_ARG; }
-    if (t->needs_u_equals_d && U_dev != D_dev) {
-        set_error("wick_contract: this term list was built with WICK_BUILD_ISOSPIN (terms merged that are equal only for U == D); pass U_dev == D_dev");
-        return WICK_ERR_ARG; }
+         reinterpret_cast<uintptr_t>(sigma_out_dev)) & 15) return fail("buffers must be 16-byte aligned", WICK_ERR_ARG);
+    if (reinterpret_cast<uintptr_t>(workspace_dev) & 255) return fail("workspace must be 256-byte aligned", WICK_ERR_ARG);
+    const wick_terms* t = lists[0];
+    for (int k = 0; k < n_lists; ++k) {
+        const wick_terms* tk = lists[k];
+        if (tk->needs_u_equals_d && U_dev != D_dev)
+            return fail("this term list was built with WICK_BUILD_ISOSPIN (terms merged that are equal only for U == D); pass U_dev == D_dev", WICK_ERR_ARG);
+        if (k > 0 && (tk->n_u != t->n_u || tk->n_d != t->n_d || tk->f[0].rows != t->f[0].rows || tk->f[0].cols != t->f[0].cols ||
+                      tk->f[1].rows != t->f[1].rows || tk->f[1].cols != t->f[1].cols || tk->f[0].minor_row != t->f[0].minor_row ||
+                      tk->f[0].minor_col != t->f[0].minor_col || tk->f[1].minor_row != t->f[1].minor_row || tk->f[1].minor_col != t->f[1].minor_col))
+            return fail("the term lists do not share their unique-minor tables (build them with wick_build_terms_matrix)", WICK_ERR_UNSUPPORTED);
+    }
     Plan p;
-    if (!make_plan(t, L, T, n_mom, workspace_bytes, false, &p)) { set_error("wick_contract: need L >= 1, T >= 1, n_mom >= 0"); return WICK_ERR_ARG; }
-    if (p.S_b < GROUP) { set_error("wick_contract: workspace smaller than wick_contract_min_workspace_bytes()"); return WICK_ERR_WORKSPACE; }
+    if (!make_plan(t, n_lists, L, T, n_mom, workspace_bytes, false, &p)) return fail("need L >= 1, T >= 1, n_mom >= 0", WICK_ERR_ARG);
+    if (p.S_b < GROUP) return fail("workspace smaller than the minimum workspace", WICK_ERR_WORKSPACE);
     cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
     int rc = ensure_configured();
     if (rc != WICK_OK) return rc;
-    if ((rc = upload_tables(t, stream)) != WICK_OK) return rc;
-    const bool use_outer = t->outer && !(flags & WICK_CONTRACT_FORCE_FLAT);
-    if (!use_outer && (rc = upload_flat(t, stream)) != WICK_OK) return rc;
+    for (int k = 0; k < n_lists; ++k) {
+        if ((rc = upload_tables(lists[k], stream)) != WICK_OK) return rc;
+        const bool outer_k = lists[k]->outer && !(flags & WICK_CONTRACT_FORCE_FLAT);
+        if (!outer_k && (rc = upload_flat(lists[k], stream)) != WICK_OK) return rc;
+    }
 
     const DeviceTables& d = t->dev;
     const int64_t nmu = int64_t(t->f[0].minor_row.size()), nmd = int64_t(t->f[1].minor_row.size());
     const int S_b = int(p.S_b);
     unsigned char* ws = static_cast<unsigned char*>(workspace_dev);
-    double2* sigma = reinterpret_cast<double2*>(ws);
+    double2* sigma_all = reinterpret_cast<double2*>(ws);                   // [n_lists][T * L^3]
     double2* MU = reinterpret_cast<double2*>(ws + p.sigma_bytes);          // sigma_bytes is a multiple of 256
     double2* MD = MU + nmu * S_b;
     // isospin limit (the paper's m_u = m_d): one propagator for both flavours.  When the two flavours
@@ -872,21 +910,30 @@ extern "C" int wick_contract(const void* U_dev, const void* D_dev, const wick_te
                                t->f[0].minor_col == t->f[1].minor_col;
     if (shared_minors) MD = MU;
     double2* partial = MD + nmd * S_b;
+    double2* jac_inv[2], *jac_det[2];
+    jac_inv[0] = partial + int64_t(MAX_CHUNKS) * S_b; jac_det[0] = jac_inv[0] + int64_t(144) * S_b;
+    jac_inv[1] = jac_det[0] + S_b; jac_det[1] = jac_inv[1] + int64_t(144) * S_b;
     const double2* U = static_cast<const double2*>(U_dev);
     const double2* D = static_cast<const double2*>(D_dev);
 
     // staged factorised reduction: one CTA per SM, n_groups x n_bins CTAs ~ one wave of 148
-    StagedTables stg;
-    bool have_staged = false;
-    if (use_outer && t->n_terms > 0 && !(flags & WICK_CONTRACT_NO_STAGED) &&
-        std::max(nmu, nmd) * int64_t(S_b) < (int64_t(1) << 31)) {   // the staged kernel keeps 32-bit element offsets
-        const int groups_full = int(std::min<int64_t>(S_b, (p.n_st + GROUP - 1) / GROUP * GROUP) / GROUP);
-        const int n_bins = std::max(1, std::min(MAX_CHUNKS, 148 * STG_CTAS_PER_SM / std::max(1, groups_full)));
-        rc = ensure_staged(t, n_bins, (flags & WICK_CONTRACT_COMPLEX_COEFFS) != 0, stream, &stg);
-        if (rc < 0) return rc;
-        have_staged = (rc == 1);
+    std::vector<StagedTables> stg(static_cast<size_t>(n_lists));
+    std::vector<char> have_staged(size_t(n_lists), 0), use_outer(size_t(n_lists), 0);
+    for (int k = 0; k < n_lists; ++k) {
+        const wick_terms* tk = lists[k];
+        use_outer[size_t(k)] = tk->outer && !(flags & WICK_CONTRACT_FORCE_FLAT);
+        if (use_outer[size_t(k)] && tk->n_terms > 0 && !(flags & WICK_CONTRACT_NO_STAGED) &&
+            std::max(nmu, nmd) * int64_t(S_b) < (int64_t(1) << 31)) {   // the staged kernel keeps 32-bit element offsets
+            const int groups_full = int(std::min<int64_t>(S_b, (p.n_st + GROUP - 1) / GROUP * GROUP) / GROUP);
+            const int n_bins = std::max(1, std::min(MAX_CHUNKS, 148 * STG_CTAS_PER_SM / std::max(1, groups_full)));
+            rc = ensure_staged(tk, n_bins, (flags & WICK_CONTRACT_COMPLEX_COEFFS) != 0, stream, &stg[size_t(k)]);
+            if (rc < 0) return rc;
+            have_staged[size_t(k)] = (rc == 1);
+        }
     }
     const bool try_reg = t->outer && !(flags & WICK_CONTRACT_NO_REG_MINORS);
+    bool use_jacobi[2];
+    for (int f = 0; f < 2; ++f) use_jacobi[f] = (flags & WICK_CONTRACT_JACOBI) && d.jacobi_desc[f] != nullptr;
     for (int64_t st0 = 0; st0 < p.n_st; st0 += S_b) {
         const int64_t n_valid = std::min<int64_t>(S_b, p.n_st - st0);
         const int n_groups = int((n_valid + GROUP - 1) / GROUP);
@@ -896,44 +943,81 @@ extern "C" int wick_contract(const void* U_dev, const void* D_dev, const wick_te
             const int n = f == 0 ? t->n_u : t->n_d;
             const double2* Pf = f == 0 ? U : D;
             double2* Mf = f == 0 ? MU : MD;
+            const int pc = f == 0 ? PROF_MINORS_U : PROF_MINORS_D;
+            if (use_jacobi[f]) {
+                // one 12x12 inverse + determinant per site, then the (12-n) x (12-n) complementary minors of the inverse
+                WICK_CUDA(launch_inverse12(Pf, st0, p.n_st, n_groups, jac_inv[f], jac_det[f], pc, stream));
+                WICK_CUDA(launch_minors(12 - n, jac_inv[f], 0, n_valid, n_groups, S_b, d.jacobi_desc[f], f == 0 ? nmu : nmd, false, Mf, pc, stream));
+                continue;
+            }
             RegTables rt;
             rc = try_reg ? ensure_reg(t, f, reg_bins, stream, &rt) : 0;
             if (rc < 0) return rc;
-            if (rc == 1) WICK_CUDA(launch_minors_reg(n, Pf, st0, p.n_st, n_groups, S_b, rt, Mf, f == 0 ? PROF_MINORS_U : PROF_MINORS_D, stream));
-            else WICK_CUDA(launch_minors(n, Pf, st0, p.n_st, n_groups, S_b, d.minor_desc[f], f == 0 ? nmu : nmd, true, Mf,
-                                         f == 0 ? PROF_MINORS_U : PROF_MINORS_D, stream));
+            if (rc == 1) WICK_CUDA(launch_minors_reg(n, Pf, st0, p.n_st, n_groups, S_b, rt, Mf, pc, stream));
+            else WICK_CUDA(launch_minors(n, Pf, st0, p.n_st, n_groups, S_b, d.minor_desc[f], f == 0 ? nmu : nmd, true, Mf, pc, stream));
         }
-        int n_chunks = 1;
-        if (t->n_terms == 0) {
-            WICK_CUDA(cudaMemsetAsync(sigma + st0, 0, size_t(n_valid) * 16, stream));
-        } else {
-            if (use_outer && have_staged) {
-                WICK_CUDA(launch_reduce_staged(MU, MD, n_groups, S_b, stg, partial, &n_chunks, stream));
-            } else if (use_outer) {
+        for (int k = 0; k < n_lists; ++k) {
+            const wick_terms* tk = lists[k];
+            const DeviceTables& dk = tk->dev;
+            double2* sigma = sigma_all + int64_t(k) * p.n_st;
+            int n_chunks = 1;
+            if (tk->n_terms == 0) {
+                WICK_CUDA(cudaMemsetAsync(sigma + st0, 0, size_t(n_valid) * 16, stream));
+                continue;
+            }
+            if (use_outer[size_t(k)] && have_staged[size_t(k)]) {
+                WICK_CUDA(launch_reduce_staged(MU, MD, n_groups, S_b, stg[size_t(k)], partial, &n_chunks, stream));
+            } else if (use_outer[size_t(k)]) {
                 OuterTables ot;
-                ot.n_cols_u = int(t->f[0].cols.size()); ot.n_cols_d = int(t->f[1].cols.size());
-                ot.sink_ptr = d.sink_ptr; ot.sink_rdoff = d.sink_rdoff; ot.sink_c = reinterpret_cast<const double2*>(d.sink_c);
-                ot.src_ptr = d.src_ptr; ot.src_cu = d.src_cu; ot.src_c = reinterpret_cast<const double2*>(d.src_c);
-                ot.ru_ptr = d.ru_ptr; ot.ru_list = d.ru_list; ot.cd_ptr = d.cd_ptr; ot.cd_list = d.cd_list;
-                ot.bin_ptr = d.red_bin_ptr; ot.items = reinterpret_cast<const int2*>(d.red_items); ot.n_bins = d.n_red_bins;
+                ot.n_cols_u = int(tk->f[0].cols.size()); ot.n_cols_d = int(tk->f[1].cols.size());
+                ot.sink_ptr = dk.sink_ptr; ot.sink_rdoff = dk.sink_rdoff; ot.sink_c = reinterpret_cast<const double2*>(dk.sink_c);
+                ot.src_ptr = dk.src_ptr; ot.src_cu = dk.src_cu; ot.src_c = reinterpret_cast<const double2*>(dk.src_c);
+                ot.ru_ptr = dk.ru_ptr; ot.ru_list = dk.ru_list; ot.cd_ptr = dk.cd_ptr; ot.cd_list = dk.cd_list;
+                ot.bin_ptr = dk.red_bin_ptr; ot.items = reinterpret_cast<const int2*>(dk.red_items); ot.n_bins = dk.n_red_bins;
                 WICK_CUDA(launch_reduce_outer(MU, MD, n_groups, S_b, ot, partial, &n_chunks, stream));
             } else {
-                WICK_CUDA(launch_reduce_flat(MU, MD, n_groups, S_b, d.t_uid, d.t_did, reinterpret_cast<const double2*>(d.t_w),
-                                             t->n_terms, partial, &n_chunks, MAX_CHUNKS, stream));
+                WICK_CUDA(launch_reduce_flat(MU, MD, n_groups, S_b, dk.t_uid, dk.t_did, reinterpret_cast<const double2*>(dk.t_w),
+                                             tk->n_terms, partial, &n_chunks, MAX_CHUNKS, stream));
             }
-            WICK_CUDA(launch_finalize_sigma(partial, n_chunks, S_b, n_valid, sigma + st0, stream));
+            const double2* sc_u = use_jacobi[0] ? jac_det[0] : nullptr;
+            const double2* sc_d = use_jacobi[1] ? (shared_minors ? jac_det[0] : jac_det[1]) : nullptr;
+            WICK_CUDA(launch_finalize_sigma(partial, n_chunks, S_b, n_valid, sigma + st0, sc_u, sc_d, stream));
         }
     }
-    for (int m0 = 0; m0 < n_mom; m0 += MAX_MOMENTA) {
-        MomentumList ml;
-        ml.n = std::min(MAX_MOMENTA, n_mom - m0);
-        for (int k = 0; k < ml.n; ++k)
-            for (int c = 0; c < 3; ++c) ml.v[k][c] = momenta[3 * (m0 + k) + c];
-        WICK_CUDA(launch_project(sigma, L, T, ml, static_cast<double2*>(C_out_dev) + int64_t(m0) * T, stream));
-    }
+    for (int k = 0; k < n_lists; ++k)
+        for (int m0 = 0; m0 < n_mom; m0 += MAX_MOMENTA) {
+            MomentumList ml;
+            ml.n = std::min(MAX_MOMENTA, n_mom - m0);
+            for (int q = 0; q < ml.n; ++q)
+                for (int c = 0; c < 3; ++c) ml.v[q][c] = momenta[3 * (m0 + q) + c];
+            WICK_CUDA(launch_project(sigma_all + int64_t(k) * p.n_st, L, T, ml,
+                                     static_cast<double2*>(C_out_dev) + (int64_t(k) * n_mom + m0) * T, stream));
+        }
     if (sigma_out_dev)
-        WICK_CUDA(cudaMemcpyAsync(sigma_out_dev, sigma, size_t(p.n_st) * 16, cudaMemcpyDeviceToDevice, stream));
+        WICK_CUDA(cudaMemcpyAsync(sigma_out_dev, sigma_all, size_t(n_lists) * size_t(p.n_st) * 16, cudaMemcpyDeviceToDevice, stream));
     return WICK_OK;
+}
+
+}  // namespace
+
+extern "C" int wick_contract(const void* U_dev, const void* D_dev, const wick_terms* t, const int32_t* momenta,
+                             int n_mom, int L, int T, void* C_out_dev, void* sigma_out_dev, void* workspace_dev,
+                             size_t workspace_bytes, unsigned flags, void* cuda_stream) {
+    return contract_lists(U_dev, D_dev, &t, 1, momenta, n_mom, L, T, C_out_dev, sigma_out_dev, workspace_dev, workspace_bytes,
+                          flags, cuda_stream, "wick_contract");
+}
+
+extern "C" size_t wick_contract_many_workspace_bytes(const wick_terms* t, int n_lists, int L, int T, int n_mom) {
+    Plan p;
+    if (n_lists < 1 || !make_plan(t, n_lists, L, T, n_mom, 0, true, &p)) return 0;
+    return plan_bytes(p, p.S_b);
+}
+
+extern "C" int wick_contract_many(const void* U_dev, const void* D_dev, const wick_terms* const* lists, int n_lists,
+                                  const int32_t* momenta, int n_mom, int L, int T, void* C_out_dev, void* sigma_out_dev,
+                                  void* workspace_dev, size_t workspace_bytes, unsigned flags, void* cuda_stream) {
+    return contract_lists(U_dev, D_dev, lists, n_lists, momenta, n_mom, L, T, C_out_dev, sigma_out_dev, workspace_dev, workspace_bytes,
+                          flags, cuda_stream, "wick_contract_many");
 }
 
 // Step a4 for one flavour of a handle, through exactly the kernels wick_contract launches for it (tests: every minor of

@@ -76,14 +76,19 @@ template <int N> struct Desc {
         else { const ulonglong2 v = __ldg(reinterpret_cast<const ulonglong2*>(tab) + m); d.w[0] = v.x; d.w[1] = v.y; }
         return d;
     }
-    __device__ __forceinline__ unsigned long long rows_bits() const { return kWords == 1 ? (w[0] & 0xffffffffull) : (w[0] & 0xffffffffffffull); }
+    __device__ __forceinline__ unsigned long long rows_bits() const { return kWords == 1 ? (w[0] & (N <= 4 ? 0x7fffffffull : 0xffffffffull)) : (w[0] & 0xffffffffffffull); }
     __device__ __forceinline__ unsigned long long cols_bits() const { return kWords == 1 ? (w[0] >> 32) : (w[kWords - 1] & 0xffffffffffffull); }
     // where the determinant goes (m = position of the descriptor) and whether it is negated
     __device__ __forceinline__ int out_index(int m) const {
         if constexpr (kWords == 1) return m;
         else return int(w[0] >> 48) | (int((w[kWords - 1] >> 48) & 0x7fffull) << 16);
     }
-    __device__ __forceinline__ bool negate() const { return kWords == 1 ? false : (w[kWords - 1] >> 63) != 0; }
+    // n <= 4: bit 31 of the word (above the 4 row fields) flags a negated result (Jacobi complementary minors, contract.cu)
+    __device__ __forceinline__ bool negate() const {
+        if constexpr (kWords == 1) return N <= 4 ? ((w[0] >> 31) & 1ull) != 0 : false;
+        else return (w[kWords - 1] >> 63) != 0;
+    }
+    __device__ __forceinline__ c128 signed_result(c128 det) const { return negate() ? make_double2(-det.x, -det.y) : det; }
     __device__ __forceinline__ uint32_t row(int i) const {
         if constexpr (kWords == 1) return (uint32_t(w[0]) >> (4 * i)) & 15u;
         else return uint32_t(w[0] >> (4 * i)) & 15u;
@@ -141,7 +146,7 @@ minors_kernel(const c128* __restrict__ P, int64_t st0, int64_t n_st_total, int S
             const int c2 = int(dc.col(2));
             const c128 det = cfma(ld(tl, re[2], c2), cof[2], cfma(ld(tl, re[1], c2), cof[1], cmul(ld(tl, re[0], c2), cof[0])));
             prow = rws; pcol = cls;
-            if (valid) outp[int64_t(m) * S_b] = det;
+            if (valid) outp[int64_t(m) * S_b] = dc.signed_result(det);
         }
     } else if constexpr (N <= 2) {
         for (; m < m_stop; m += kStride) {
@@ -151,7 +156,7 @@ minors_kernel(const c128* __restrict__ P, int64_t st0, int64_t n_st_total, int S
 #pragma unroll
             for (int i = 0; i < N; ++i) { ix.re[i] = int(dc.row(i)) * 12; ix.ce[i] = int(dc.col(i)); }
             const c128 det = det_small<N>(tl, ix);
-            if (valid) outp[int64_t(m) * S_b] = det;
+            if (valid) outp[int64_t(m) * S_b] = dc.signed_result(det);
         }
     } else {
         constexpr int K = N - 4;
@@ -178,9 +183,102 @@ minors_kernel(const c128* __restrict__ P, int64_t st0, int64_t n_st_total, int S
             if (new_pair || (diff & kLead3) != 0) lu.third_column(tb, Ls, dc.col(K + 2) * kColStep);
             const c128 det = lu.finish(tb, Ls, dc.col(K + 3) * kColStep);
             prow = rws; pcol = dc.cols_bits();
-            if (valid) outp[int64_t(dc.out_index(m)) * S_b] = dc.negate() ? make_double2(-det.x, -det.y) : det;
+            if (valid) outp[int64_t(dc.out_index(m)) * S_b] = dc.signed_result(det);
         }
     }
+}
+
+// ---------------------------------------------------------------------------------------------
+// a4 for minors of size n >= 8 through Jacobi's complementary-minor identity (optional, flag
+// WICK_CONTRACT_JACOBI):  det A[I, J] = (-1)^(sum I + sum J) det A  det (A^-1)[J^c, I^c].
+// inverse12_kernel: one thread per site inverts its 12x12 propagator in place in shared memory (Gauss-Jordan with
+// partial pivoting, same pivot rule as the LU kernels; the tile layout makes the per-lane row exchanges conflict free)
+// and returns det A; the (12-n) x (12-n) minors of the inverse then go through minors_kernel<12-n>.
+// A singular propagator has no inverse: its site gets det = 0 and a zero matrix (every minor 0); use the LU path for such data.
+// ---------------------------------------------------------------------------------------------
+constexpr int INV_THREADS = 64;
+
+__global__ void __launch_bounds__(INV_THREADS)
+inverse12_kernel(const c128* __restrict__ P, int64_t st0, int64_t n_st_total, c128* __restrict__ inv_out, c128* __restrict__ det_out) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    c128* tile = reinterpret_cast<c128*>(smem_raw) + size_t(warp) * TILE_ELEMS;
+    const int64_t g = int64_t(blockIdx.x) * (INV_THREADS / 32) + warp;      // 32-site group within the batch
+    const int64_t st_first = st0 + g * GROUP;
+    // stage (per warp): consecutive lanes read consecutive 16-byte elements of one site
+    for (int idx = lane; idx < TILE_ELEMS; idx += 32) {
+        const int site = idx / 144, e = idx - site * 144;
+        const int64_t st = st_first + site;
+        c128 v = make_double2(0.0, 0.0);
+        if (st < n_st_total) v = __ldg(P + st * 144 + e);
+        tile[e * GROUP + site] = v;
+    }
+    __syncwarp();
+    c128* A = tile + lane;                                                  // A[r][c] at A[(12 r + c) * GROUP]
+    c128 det = make_double2(1.0, 0.0);
+    unsigned long long piv_rows = 0;                                        // pivot row of step k, 4 bits each
+    bool singular = false;
+#pragma unroll 1
+    for (int k = 0; k < 12; ++k) {
+        int p = k;
+        int best = -1;
+        for (int r = k; r < 12; ++r) {
+            const c128 v = A[(12 * r + k) * GROUP];
+            const int m = pivot_key(v.x, v.y);
+            if (m > best) { best = m; p = r; }
+        }
+        piv_rows |= (unsigned long long)p << (4 * k);
+        c128 rowk[12];
+#pragma unroll
+        for (int c = 0; c < 12; ++c) {                                      // exchange rows k and p, keep row k in registers
+            const c128 a = A[(12 * k + c) * GROUP], b = A[(12 * p + c) * GROUP];
+            A[(12 * p + c) * GROUP] = a;
+            rowk[c] = b;
+        }
+        const c128 piv = rowk[k];
+        det = cmul(det, piv);
+        if (p != k) { det.x = -det.x; det.y = -det.y; }
+        const c128 ip = crecip(piv);
+        singular = singular || (piv.x == 0.0 && piv.y == 0.0);
+        rowk[k] = make_double2(1.0, 0.0);
+#pragma unroll
+        for (int c = 0; c < 12; ++c) { rowk[c] = cmul(rowk[c], ip); A[(12 * k + c) * GROUP] = rowk[c]; }
+        for (int r = 0; r < 12; ++r) {
+            if (r == k) continue;
+            const c128 f = A[(12 * r + k) * GROUP];
+            A[(12 * r + k) * GROUP] = make_double2(0.0, 0.0);
+#pragma unroll
+            for (int c = 0; c < 12; ++c) A[(12 * r + c) * GROUP] = cfnma(f, rowk[c], A[(12 * r + c) * GROUP]);
+        }
+    }
+    for (int k = 11; k >= 0; --k) {                                         // undo the row exchanges on the columns
+        const int p = int(piv_rows >> (4 * k)) & 15;
+        if (p != k)
+            for (int r = 0; r < 12; ++r) {
+                const c128 a = A[(12 * r + k) * GROUP], b = A[(12 * r + p) * GROUP];
+                A[(12 * r + k) * GROUP] = b; A[(12 * r + p) * GROUP] = a;
+            }
+    }
+    if (singular) {
+        det = make_double2(0.0, 0.0);
+        for (int e = 0; e < 144; ++e) A[e * GROUP] = make_double2(0.0, 0.0);
+    }
+    if (st_first + lane < n_st_total) det_out[g * GROUP + lane] = det;
+    __syncwarp();
+    for (int idx = lane; idx < TILE_ELEMS; idx += 32) {                     // coalesced write-back, [site][12][12]
+        const int site = idx / 144, e = idx - site * 144;
+        if (st_first + site < n_st_total) inv_out[(g * GROUP + site) * 144 + e] = tile[e * GROUP + site];
+    }
+}
+
+cudaError_t launch_inverse12(const double2* P, int64_t st0, int64_t n_st_total, int n_groups, double2* inv_out, double2* det_out,
+                             int prof_cls, cudaStream_t stream) {
+    if (n_groups == 0) return cudaSuccess;
+    const int per_cta = INV_THREADS / 32;
+    ProfScope prof(prof_cls, stream);
+    inverse12_kernel<<<(n_groups + per_cta - 1) / per_cta, INV_THREADS, size_t(per_cta) * TILE_BYTES, stream>>>(P, st0, n_st_total, inv_out, det_out);
+    ++g_launches;
+    return cudaGetLastError();
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -841,20 +939,22 @@ cudaError_t launch_reduce_outer(const double2* MU, const double2* MD, int n_grou
 // a6: sigma = fixed-order sum of the chunk partials; C(t,p) = sum_x e^{ip.x} sigma(x,t), fixed tree
 // ---------------------------------------------------------------------------------------------
 __global__ void finalize_sigma_kernel(const c128* __restrict__ partial, int n_chunks, int S_b, int64_t n_valid,
-                                      c128* __restrict__ sigma_batch) {
+                                      c128* __restrict__ sigma_batch, const c128* __restrict__ scale_a, const c128* __restrict__ scale_b) {
     const int64_t s = int64_t(blockIdx.x) * blockDim.x + threadIdx.x;
     if (s >= n_valid) return;
     c128 acc = partial[s];
     for (int c = 1; c < n_chunks; ++c) acc = cadd(acc, partial[int64_t(c) * S_b + s]);
+    if (scale_a) acc = cmul(acc, scale_a[s]);                   // Jacobi path: the common factor det U (det D) of every term of the site
+    if (scale_b) acc = cmul(acc, scale_b[s]);
     sigma_batch[s] = acc;
 }
 
 cudaError_t launch_finalize_sigma(const double2* partial, int n_chunks, int S_b, int64_t n_valid,
-                                  double2* sigma_batch, cudaStream_t stream) {
+                                  double2* sigma_batch, const double2* scale_a, const double2* scale_b, cudaStream_t stream) {
     if (n_valid <= 0) return cudaSuccess;
     const int threads = 128;
     ProfScope prof(PROF_PROJECT, stream);
-    finalize_sigma_kernel<<<unsigned((n_valid + threads - 1) / threads), threads, 0, stream>>>(partial, n_chunks, S_b, n_valid, sigma_batch);
+    finalize_sigma_kernel<<<unsigned((n_valid + threads - 1) / threads), threads, 0, stream>>>(partial, n_chunks, S_b, n_valid, sigma_batch, scale_a, scale_b);
     ++g_launches;
     return cudaGetLastError();
 }
@@ -954,6 +1054,7 @@ template <int N> static cudaError_t set_smem_attr() {
 cudaError_t configure_kernels() {
     cudaError_t e;
     if ((e = configure_reg_kernels()) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(inverse12_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, int(INV_THREADS / 32 * TILE_BYTES))) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(minors_large_cached_kernel<10, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(mlc_smem<10, 0>()))) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(minors_large_cached_kernel<11, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(mlc_smem<11, 1>()))) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(minors6_cached_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, int(M6C_SMEM))) != cudaSuccess) return e;

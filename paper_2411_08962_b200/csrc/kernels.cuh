@@ -35,7 +35,8 @@ cudaError_t launch_minors(int n, const double2* P, int64_t st0, int64_t n_st_tot
 // columns, up to REG_NC_MAX candidate columns behind them, and the trie of the instance's column tuples over candidate
 // POSITIONS as a word program.  The minors of a job are stored in trie order from column position out_base of the row
 // tuple's list.
-constexpr int REG_THREADS = 256;
+constexpr int REG_THREADS = 384;          // 12 warps: 3 per scheduler
+constexpr int REG_NS = 6;                 // candidate positions kept in the per-thread shared-memory copy; the rest in registers
 constexpr int REG_NC_MAX = 10;
 struct RegJob {
     unsigned long long lead, cand;        // column indices as 4-bit fields: leading (K), candidates (ncand)
@@ -94,8 +95,12 @@ struct StagedTables {
 };
 cudaError_t launch_reduce_staged(const double2* MU, const double2* MD, int n_groups, int S_b, const StagedTables& st,
                                  double2* partial, int* n_chunks_out, cudaStream_t stream);
+// scale_a / scale_b: NULL or per-site factors multiplied into sigma (Jacobi path: det U, det D)
 cudaError_t launch_finalize_sigma(const double2* partial, int n_chunks, int S_b, int64_t n_valid,
-                                  double2* sigma_batch, cudaStream_t stream);
+                                  double2* sigma_batch, const double2* scale_a, const double2* scale_b, cudaStream_t stream);
+// Jacobi path: inverse [site in batch][12][12] and determinant [site in batch] of the propagators st0 .. of a site batch
+cudaError_t launch_inverse12(const double2* P, int64_t st0, int64_t n_st_total, int n_groups, double2* inv_out, double2* det_out,
+                             int prof_cls, cudaStream_t stream);
 cudaError_t launch_project(const double2* sigma, int L, int T, const MomentumList& mom, double2* C_out,
                            cudaStream_t stream);
 cudaError_t configure_kernels();          // cudaFuncSetAttribute for the large-shared-memory kernels (once per device)

@@ -335,6 +335,81 @@ static bool symmetrise_isospin(wick_terms* t) {
 }
 
 // ---------------------------------------------------------------------------------------------
+// General interpolators (GEVP correlation matrices, Sec. V): an operator is a polynomial in the
+// exterior algebra, canonical monomial (u mask, d mask) -> complex coefficient.
+// ---------------------------------------------------------------------------------------------
+typedef std::map<uint32_t, cplx> Poly;
+
+// canonical monomial a times canonical monomial b: the quarks of b are appended one by one (u ascending, then d ascending)
+static int mono_mul(Mono a, Mono b, Mono* out) {
+    int sign = 1;
+    for (int chi = 0; chi < 12 && sign; ++chi) if (b.u & (1u << chi)) sign *= append_quark(a, 0, chi);
+    for (int chi = 0; chi < 12 && sign; ++chi) if (b.d & (1u << chi)) sign *= append_quark(a, 1, chi);
+    *out = a;
+    return sign;
+}
+
+static Poly poly_mul(const Poly& A, const Poly& B, cplx scale) {
+    Poly out;
+    for (const auto& a : A)
+        for (const auto& b : B) {
+            Mono ma = {uint16_t(a.first >> 16), uint16_t(a.first & 0xffff)}, mb = {uint16_t(b.first >> 16), uint16_t(b.first & 0xffff)}, m;
+            const int sign = mono_mul(ma, mb, &m);
+            if (sign) out[key_of(m)] += scale * double(sign) * a.second * b.second;
+        }
+    return out;
+}
+
+static void poly_add(Poly& A, const Poly& B) { for (const auto& b : B) A[b.first] += b.second; }
+static void poly_prune(Poly& A) { for (auto it = A.begin(); it != A.end();) it = (it->second == cplx(0.0, 0.0)) ? A.erase(it) : std::next(it); }
+
+// (C gamma5 P)_{beta delta}: P = 1 (proj 0), P_+ = diag(1,1,0,0) (proj +1), P_- = diag(0,0,1,1) (proj -1)
+static int cg5_projected(int beta, int delta, int proj) {
+    if (proj > 0 && delta >= 2) return 0;
+    if (proj < 0 && delta < 2) return 0;
+    return c_gamma5(beta, delta);
+}
+
+// Eq. (4)/(5) PAPER.md:105-107, with the projector of Eq. (26)/(27) :271-273:
+// (N)_alpha = eps_abc q1^a_alpha q1^b_beta (C gamma5 P)_{beta delta} q2^c_delta,  q1 = u, q2 = d for the proton
+static Poly paper_nucleon(int kind, int alpha, int proj) {
+    const int f1 = kind == WICK_NUCLEON_PROTON ? 0 : 1, f2 = 1 - f1;
+    Poly out;
+    for (int a = 0; a < 3; ++a)
+        for (int b = 0; b < 3; ++b)
+            for (int c = 0; c < 3; ++c) {
+                const int e = levi_civita(a, b, c);
+                if (!e) continue;
+                for (int be = 0; be < 4; ++be)
+                    for (int de = 0; de < 4; ++de) {
+                        const int g = cg5_projected(be, de, proj);
+                        if (!g) continue;
+                        Mono m = {0, 0};
+                        int sign = append_quark(m, f1, 3 * alpha + a);
+                        if (sign) sign *= append_quark(m, f1, 3 * be + b);
+                        if (sign) sign *= append_quark(m, f2, 3 * de + c);
+                        if (sign) out[key_of(m)] += double(e * g * sign);
+                    }
+            }
+    poly_prune(out);
+    return out;
+}
+
+struct wick_operator { int n_u = 0, n_d = 0; Poly poly; };
+
+static bool operator_finish(wick_operator* op) {
+    poly_prune(op->poly);
+    op->n_u = op->n_d = 0;
+    bool first = true;
+    for (const auto& kv : op->poly) {
+        const int nu = popc(kv.first >> 16), nd = popc(kv.first & 0xffff);
+        if (first) { op->n_u = nu; op->n_d = nd; first = false; }
+        else if (nu != op->n_u || nd != op->n_d) return false;
+    }
+    return true;
+}
+
+// ---------------------------------------------------------------------------------------------
 
 extern "C" const char* wick_last_error(void) { return g_error.c_str(); }
 extern "C" const char* wick_version(void) { return "wick-b200 0.1 (sm_100a)"; }
@@ -499,6 +574,149 @@ extern "C" int wick_build_terms_from_list(int n_u, int n_d, int64_t n_raw, const
         return WICK_OK;
     } catch (const std::bad_alloc&) {
         set_error("wick_build_terms_from_list: out of host memory");
+        return WICK_ERR_NOMEM;
+    }
+}
+
+extern "C" int wick_operator_from_nucleons(const wick_nucleon* nucleons, int n_nucleons, wick_operator** out) {
+    if (!nucleons || !out || n_nucleons < 1) { set_error("wick_operator_from_nucleons: NULL argument or n_nucleons < 1"); return WICK_ERR_ARG; }
+    *out = nullptr;
+    for (int k = 0; k < n_nucleons; ++k)
+        if ((nucleons[k].kind != WICK_NUCLEON_PROTON && nucleons[k].kind != WICK_NUCLEON_NEUTRON) || nucleons[k].gamma < 0 || nucleons[k].gamma > 3) {
+            set_error("wick_operator_from_nucleons: kind must be 0 / 1 and gamma 0..3"); return WICK_ERR_ARG; }
+    try {
+        wick_operator* op = new wick_operator();
+        op->poly[0] = 1.0;
+        for (int k = 0; k < n_nucleons; ++k) {
+            Poly nuc;
+            for (const RawNucleonTerm& rt : nucleon_terms(nucleons[k].kind, nucleons[k].gamma)) {
+                Mono m = {0, 0};
+                int sign = 1;
+                for (int q = 0; q < 3 && sign; ++q) sign *= append_quark(m, rt.f[q], rt.chi[q]);
+                if (sign) nuc[key_of(m)] += double(rt.coef * sign);
+            }
+            op->poly = poly_mul(op->poly, nuc, 1.0);
+            poly_prune(op->poly);
+        }
+        operator_finish(op);
+        *out = op;
+        return WICK_OK;
+    } catch (const std::bad_alloc&) { set_error("wick_operator_from_nucleons: out of host memory"); return WICK_ERR_NOMEM; }
+}
+
+extern "C" int wick_operator_from_raw(int n_quarks, int64_t n_raw, const uint8_t* flavour, const uint8_t* chi, const double* coef_reim,
+                                      wick_operator** out) {
+    if (!out || n_quarks < 0 || n_quarks > 24 || n_raw < 0 || (n_raw > 0 && (!coef_reim || (n_quarks > 0 && (!flavour || !chi))))) {
+        set_error("wick_operator_from_raw: bad argument"); return WICK_ERR_ARG; }
+    *out = nullptr;
+    for (int64_t k = 0; k < n_raw * n_quarks; ++k)
+        if (flavour[k] > 1 || chi[k] > 11) { set_error("wick_operator_from_raw: flavour must be 0 / 1 and chi < 12"); return WICK_ERR_ARG; }
+    try {
+        wick_operator* op = new wick_operator();
+        for (int64_t k = 0; k < n_raw; ++k) {
+            Mono m = {0, 0};
+            int sign = 1;
+            for (int q = 0; q < n_quarks && sign; ++q) sign *= append_quark(m, flavour[k * n_quarks + q], chi[k * n_quarks + q]);
+            if (sign) op->poly[key_of(m)] += double(sign) * cplx(coef_reim[2 * k], coef_reim[2 * k + 1]);
+        }
+        if (!operator_finish(op)) { delete op; set_error("wick_operator_from_raw: terms with different quark content"); return WICK_ERR_ARG; }
+        *out = op;
+        return WICK_OK;
+    } catch (const std::bad_alloc&) { set_error("wick_operator_from_raw: out of host memory"); return WICK_ERR_NOMEM; }
+}
+
+extern "C" int wick_operator_paper(int which, int J, wick_operator** out) {
+    if (!out || (which != WICK_OP_DEUTERON_EQ20 && which != WICK_OP_HELIUM3_EQ21) || J < 0 || J > 3) {
+        set_error("wick_operator_paper: which must be WICK_OP_DEUTERON_EQ20 or WICK_OP_HELIUM3_EQ21, J 0..3"); return WICK_ERR_ARG; }
+    *out = nullptr;
+    try {
+        wick_operator* op = new wick_operator();
+        for (int al = 0; al < 4; ++al)
+            for (int be = 0; be < 4; ++be) {
+                if (which == WICK_OP_DEUTERON_EQ20) {
+                    const int g = cg5_projected(al, be, +1);           // n^T (C g5 P+) p, Eq. (20)
+                    if (g) poly_add(op->poly, poly_mul(paper_nucleon(WICK_NUCLEON_NEUTRON, al, 0), paper_nucleon(WICK_NUCLEON_PROTON, be, 0), double(g)));
+                } else {
+                    const int g = c_gamma5(al, be);                    // p_-^T (C g5) n_+ p_+^J, Eq. (21)
+                    if (g) poly_add(op->poly, poly_mul(poly_mul(paper_nucleon(WICK_NUCLEON_PROTON, al, -1), paper_nucleon(WICK_NUCLEON_NEUTRON, be, +1), double(g)),
+                                                       paper_nucleon(WICK_NUCLEON_PROTON, J, +1), 1.0));
+                }
+            }
+        operator_finish(op);
+        *out = op;
+        return WICK_OK;
+    } catch (const std::bad_alloc&) { set_error("wick_operator_paper: out of host memory"); return WICK_ERR_NOMEM; }
+}
+
+extern "C" int wick_operator_info(const wick_operator* op, int32_t* n_u, int32_t* n_d, int64_t* n_terms) {
+    if (!op) { set_error("wick_operator_info: NULL argument"); return WICK_ERR_ARG; }
+    if (n_u) *n_u = op->n_u;
+    if (n_d) *n_d = op->n_d;
+    if (n_terms) *n_terms = int64_t(op->poly.size());
+    return WICK_OK;
+}
+
+extern "C" int wick_operator_export(const wick_operator* op, uint8_t* u_tuples, uint8_t* d_tuples, double* coef_reim) {
+    if (!op) { set_error("wick_operator_export: NULL argument"); return WICK_ERR_ARG; }
+    size_t k = 0;
+    for (const auto& kv : op->poly) {
+        if (u_tuples) mask_to_tuple(uint16_t(kv.first >> 16), op->n_u, u_tuples + k * size_t(op->n_u));
+        if (d_tuples) mask_to_tuple(uint16_t(kv.first & 0xffff), op->n_d, d_tuples + k * size_t(op->n_d));
+        if (coef_reim) { coef_reim[2 * k] = kv.second.real(); coef_reim[2 * k + 1] = kv.second.imag(); }
+        ++k;
+    }
+    return WICK_OK;
+}
+
+extern "C" void wick_operator_free(wick_operator* op) { delete op; }
+
+// K interpolators with the same quark content -> K x K term lists  (sink k) x conj(source k')  over ONE pair of
+// unique-minor tables (the union of all row / column tuples): the determinants are shared by the whole correlation
+// matrix (Sec. V, Eq. 36-38).
+extern "C" int wick_build_terms_matrix(const wick_operator* const* ops, int n_ops, unsigned flags, wick_terms** out) {
+    (void)flags;
+    if (!ops || !out || n_ops < 1) { set_error("wick_build_terms_matrix: bad argument"); return WICK_ERR_ARG; }
+    for (int k = 0; k < n_ops * n_ops; ++k) out[k] = nullptr;
+    for (int k = 0; k < n_ops; ++k)
+        if (!ops[k] || ops[k]->n_u != ops[0]->n_u || ops[k]->n_d != ops[0]->n_d || ops[k]->poly.empty()) {
+            set_error("wick_build_terms_matrix: operators must be non-empty and share their quark content"); return WICK_ERR_ARG; }
+    try {
+        std::vector<uint16_t> us, ds;
+        for (int k = 0; k < n_ops; ++k)
+            for (const auto& kv : ops[k]->poly) { us.push_back(uint16_t(kv.first >> 16)); ds.push_back(uint16_t(kv.first & 0xffff)); }
+        const std::vector<uint16_t> ru = distinct_sorted(us), rd = distinct_sorted(ds);
+        const auto iu = index_of(ru), id = index_of(rd);
+        std::vector<std::vector<FactorTerm>> lists(static_cast<size_t>(n_ops));
+        for (int k = 0; k < n_ops; ++k) {
+            for (const auto& kv : ops[k]->poly) {
+                FactorTerm ft;
+                ft.qu = iu.at(uint16_t(kv.first >> 16)); ft.qd = id.at(uint16_t(kv.first & 0xffff)); ft.c = kv.second;
+                lists[size_t(k)].push_back(ft);
+            }
+            std::sort(lists[size_t(k)].begin(), lists[size_t(k)].end(), [](const FactorTerm& a, const FactorTerm& b) {
+                return a.qu != b.qu ? a.qu < b.qu : a.qd < b.qd; });
+        }
+        for (int k = 0; k < n_ops; ++k)
+            for (int kp = 0; kp < n_ops; ++kp) {
+                wick_terms* t = new wick_terms();
+                out[k * n_ops + kp] = t;
+                t->n_u = ops[0]->n_u; t->n_d = ops[0]->n_d;
+                t->f[0].n = t->n_u; t->f[1].n = t->n_d;
+                t->f[0].rows = t->f[0].cols = ru;
+                t->f[1].rows = t->f[1].cols = rd;
+                t->sink = lists[size_t(k)];
+                t->source = lists[size_t(kp)];
+                for (FactorTerm& s : t->source) s.c = std::conj(s.c);       // C' = conj(C) (reading 3)
+                t->outer = true;
+                t->n_terms = int64_t(t->sink.size()) * int64_t(t->source.size());
+                t->n_raw = t->n_terms;
+                grid_minors(t->f[0]);
+                grid_minors(t->f[1]);
+            }
+        return WICK_OK;
+    } catch (const std::bad_alloc&) {
+        for (int k = 0; k < n_ops * n_ops; ++k) { delete out[k]; out[k] = nullptr; }
+        set_error("wick_build_terms_matrix: out of host memory");
         return WICK_ERR_NOMEM;
     }
 }

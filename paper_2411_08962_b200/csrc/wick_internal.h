@@ -48,6 +48,7 @@ struct RegDev {
 struct DeviceTables {
     int device = -1;
     void* blob = nullptr;                       // one allocation holding the minor tables + factor lists
+    const void* jacobi_desc[2] = {nullptr, nullptr};    // n = 8..11: complementary-minor descriptors (contract.cu: build_jacobi_descs)
     const void* minor_desc[2] = {nullptr, nullptr};     // [n_minors] packed (row indices, column indices), kernels.cu: struct Desc
     // factorised reduction: sink CSR over u row-tuple id, source CSR over d column-tuple id
     const int32_t* sink_ptr = nullptr;          // [n_rows_u + 1]

@@ -253,3 +253,107 @@ def test_minor_order_is_a_signed_permutation(cfg):
         assert np.all(np.diff(mrow[mid]) >= 0)                               # row tuple by row tuple
         if pc.shape[1] <= 8:                                                 # small minors: minor order, ascending columns
             assert np.array_equal(mid, np.arange(len(mid))) and not neg.any()
+
+
+# ---------------------------------------------------------------------------------------------
+# isospin limit U == D: factorised swap symmetrisation and the merged flat list
+# ---------------------------------------------------------------------------------------------
+
+def test_isospin_counts_of_the_deuteron():
+    """with U == D the identity test collapses the deuteron's 53 361 products to 26 721 and both
+    flavours share one table of 14 641 minors; the factorised symmetrisation keeps 120 of the 231 sink terms."""
+    nuc = NUCLEI["cfg1"]
+    merged = wk.build_terms(nuc, flags=wk.BUILD_IDENTITY_TEST | wk.BUILD_ISOSPIN, seed=3)
+    assert merged.info.n_terms == 26721 and merged.info.is_outer_product == 0
+    assert merged.info.n_minors_u == 14641 and merged.info.n_minors_d == 14641
+    ur, uc, dr, dc = merged.tuples()
+    assert np.array_equal(ur, dr) and np.array_equal(uc, dc)                 # one table serves both flavours
+    half = wk.build_terms(nuc, flags=wk.BUILD_ISOSPIN)
+    assert half.info.is_outer_product == 1 and half.info.n_sink == 120 and half.info.n_source == 231
+    assert half.info.n_terms == 120 * 231
+    # (231 + 9 self-conjugate sink terms) / 2 = 120; the minimal count differs only by the 9 x 111 products that pair a
+    # self-conjugate sink term with both members of a source pair
+    assert 120 * 231 - 26721 == 9 * 111
+
+
+@pytest.mark.parametrize("cfg", ["cfg1", "cfg3"])
+def test_isospin_symmetrised_list_equals_the_full_list_at_u_equals_d(cfg):
+    nuc = NUCLEI[cfg]
+    full, half = wk.build_terms(nuc), wk.build_terms(nuc, flags=wk.BUILD_ISOSPIN)
+    assert half.info.n_sink < full.info.n_sink and half.info.n_source == full.info.n_source
+    rng = np.random.default_rng(31)
+    U = _rand(rng, 12, 12)
+    ur, uc, dr, dc = full.tuples()
+
+    def value(t):
+        sru, srd, sc, qcu, qcd, qc = t.factors()
+        MU = wo.det_elim(U[ur[:, None, :, None], uc[None, :, None, :]])      # [row tuple][column tuple], U == D
+        MD = wo.det_elim(U[dr[:, None, :, None], dc[None, :, None, :]])
+        tot, tot_abs = 0.0, 0.0
+        for i in range(len(sc)):
+            v = sc[i] * qc * MU[sru[i], qcu] * MD[srd[i], qcd]
+            tot += v.sum()
+            tot_abs += np.abs(v).sum()
+        return tot, tot_abs
+    a, sabs = value(full)
+    b, _ = value(half)
+    assert abs(a - b) <= 1e-12 * sabs
+    # the symmetrisation is only valid for U == D and must not be applied silently otherwise
+    assert wk.build_terms(NUCLEI["cfg2"], flags=wk.BUILD_ISOSPIN).info.n_sink == wk.build_terms(NUCLEI["cfg2"]).info.n_sink
+
+
+# ---------------------------------------------------------------------------------------------
+# general interpolators and correlation matrices (GEVP, Sec. V PAPER.md:394-420)
+# ---------------------------------------------------------------------------------------------
+
+def _as_list(op):
+    u, d, c = op.terms()
+    return sorted((tuple(int(x) for x in a), tuple(int(x) for x in b), complex(z)) for a, b, z in zip(u, d, c))
+
+
+def test_paper_operators_match_the_oracle_and_the_printed_counts(golden):
+    """Eq. (20) and Eq. (21) in the builder: the printed 356 / 1026 terms (Table II, :305-306) and,
+    monomial by monomial, the oracle's independent expansion."""
+    d = wk.operator_paper(wk.OP_DEUTERON_EQ20)
+    assert (d.n_u, d.n_d, d.n_terms) == (3, 3, int(golden["h2_terms_eq20"]))
+    assert _as_list(d) == [(u, dd, complex(c)) for u, dd, c in wo.merged_from_raw(wo.deuteron_eq20_raw_terms())]
+    for J in (2, 3):
+        h = wk.operator_paper(wk.OP_HELIUM3_EQ21, J)
+        assert (h.n_u, h.n_d, h.n_terms) == (5, 4, int(golden["he3_terms_eq21"]))
+        assert _as_list(h) == [(u, dd, complex(c)) for u, dd, c in wo.merged_from_raw(wo.helium3_eq21_raw_terms(J))]
+    assert wk.operator_paper(wk.OP_HELIUM3_EQ21, 0).n_terms == 744       # J in the projector's own sector: not the paper's count
+    with pytest.raises(wk.WickError):
+        wk.operator_paper(7)
+
+
+def test_operator_from_raw_and_from_nucleons_agree():
+    nuc = NUCLEI["cfg1"]
+    raw = wo.nucleus_raw_terms(nuc)
+    fl = np.array([[0 if f == "u" else 1 for f, _ in q] for _, q in raw], np.uint8)
+    chi = np.array([[x for _, x in q] for _, q in raw], np.uint8)
+    coef = np.array([c for c, _ in raw], complex)
+    a, b = wk.operator_from_raw(fl, chi, coef), wk.operator_from_nucleons(nuc)
+    assert _as_list(a) == _as_list(b) == [(u, d, complex(c)) for u, d, c in wo.merged_terms(nuc)]
+    with pytest.raises(wk.WickError, match="quark content"):
+        wk.operator_from_raw(np.array([[0, 0], [0, 1]], np.uint8), np.array([[0, 1], [0, 1]], np.uint8), np.ones(2, complex))
+
+
+def test_terms_matrix_shares_one_pair_of_minor_tables():
+    ops = [wk.operator_from_nucleons(NUCLEI["cfg1"]), wk.operator_paper(wk.OP_DEUTERON_EQ20)]
+    m = wk.build_terms_matrix(ops)
+    tup = [m[k][kp].tuples() for k in range(2) for kp in range(2)]
+    for other in tup[1:]:
+        assert all(np.array_equal(x, y) for x, y in zip(tup[0], other))
+    assert [[m[k][kp].info.n_terms for kp in range(2)] for k in range(2)] == [[231 * 231, 231 * 356], [356 * 231, 356 * 356]]
+    assert all(m[k][kp].info.is_outer_product == 1 for k in range(2) for kp in range(2))
+    # the diagonal entry of the product operator evaluates like the plain handle
+    rng = np.random.default_rng(41)
+    U, D = _rand(rng, 12, 12), _rand(rng, 12, 12)
+    ref, sabs = wo.site_terms_value(U, D, *wk.build_terms(NUCLEI["cfg1"]).term_tuples())
+    got, _ = wo.site_terms_value(U, D, *m[0][0].term_tuples())
+    assert abs(got - ref) <= 1e-12 * sabs
+    # an off-diagonal entry against the oracle's own sink x conj(source) expansion
+    sink, src = wo.merged_terms(NUCLEI["cfg1"]), wo.merged_from_raw(wo.deuteron_eq20_raw_terms())
+    ref, sabs = wo.site_value_outer(U, D, sink, src)
+    got, _ = wo.site_terms_value(U, D, *m[0][1].term_tuples())
+    assert abs(got - ref) <= 1e-12 * sabs

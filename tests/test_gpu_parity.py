@@ -82,6 +82,38 @@ def test_minor_dets_vs_oracle(n, n_sites, cuda_device):
     assert np.all(np.isfinite(got.view(np.float64)))
 
 
+@pytest.mark.parametrize("cfg,flags", [("cfg3", 0), ("cfg3", wk.CONTRACT_NO_REG_MINORS), ("cfg2", 0), ("cfg1", 0),
+                                       ("cfg4", 0), ("cfg4b", 0)])
+@pytest.mark.parametrize("n_sites", [70, 64])
+def test_library_minor_tables_vs_oracle(cfg, flags, n_sites, cuda_device):
+    """The kernels wick_contract launches for the library's OWN tables (register-resident instance kernel and Schur-column
+    cache kernel for 6x6, cached kernels for 10x10 / 11x11, column-trie kernels below), minor by minor against the oracle's
+    elimination: every minor of the first, a middle and the last row tuple plus a seeded sample, on a ragged and a full
+    site count, with a tiny-scale site and a site with an exactly zero row."""
+    t = _terms_for(cfg)
+    rng = np.random.default_rng(300 + n_sites)
+    P = rng.standard_normal((n_sites, 12, 12)) + 1j * rng.standard_normal((n_sites, 12, 12))
+    P[3] *= 1e-3
+    P[5, 2, :] = 0.0
+    tup = t.tuples()
+    mins = t.minors()
+    for fl in (0, 1):
+        rows, cols, mrow, mcol = tup[2 * fl], tup[2 * fl + 1], mins[2 * fl], mins[2 * fl + 1]
+        n = rows.shape[1]
+        got = wk.minor_table(_dev(P, cuda_device), t, fl, flags=flags).cpu().numpy()
+        nm = len(mrow)
+        assert got.shape == (nm, n_sites)
+        pick = np.flatnonzero(np.isin(mrow, [mrow.min(), int(np.median(mrow)), mrow.max()]))
+        pick = np.union1d(pick, rng.choice(nm, size=min(nm, 4000), replace=False))
+        sub = P[:, rows[mrow[pick]][:, :, None], cols[mcol[pick]][:, None, :]]          # [site][minor][n][n]
+        ref = wo.det_elim(sub).T
+        scale = np.prod(np.linalg.norm(sub, axis=3), axis=2).T
+        assert np.all(np.abs(got[pick] - ref) <= 1e-13 * n * scale + 1e-300), (cfg, fl)
+        zero_row = np.any(rows[mrow[pick]] == 2, axis=1)
+        assert np.all(got[pick][zero_row, 5] == 0.0)
+        assert np.all(np.isfinite(got.view(np.float64)))
+
+
 def test_minor_dets_repeated_index_is_zero(cuda_device):
     rng = np.random.default_rng(7)
     P = rng.standard_normal((32, 12, 12)) + 1j * rng.standard_normal((32, 12, 12))
@@ -175,8 +207,8 @@ def test_generic_lists_of_large_minors(n_u, n_d, cuda_device):
 
 FULL = {  # cfg -> (timeslices to run, sites sampled per timeslice)
     "cfg1": ([0, 16, 31], 6),
-    "cfg2": ([47], 4),
-    "cfg3": ([63], 3),
+    "cfg2": ([0, 47], 4),
+    "cfg3": ([0, 32, 63], 3),
     "cfg4": ([0, 47], 8),
     "cfg4b": ([24], 8),
 }
@@ -292,3 +324,133 @@ def test_contract_host_matches_device_call(cuda_device):
     assert np.array_equal(Ch, Cd.cpu().numpy())
     n0 = wk.launch_count(reset=True)
     assert n0 > 0
+
+
+def test_contract_host_multi_block_overlap(cuda_device, monkeypatch):
+    """wick_contract_host over several timeslice blocks (H2D of block b+1 on the copy stream while block b computes,
+    PAPER.md:663; short last block): bitwise equal to the device call, and within 1e-10 of the oracle on sampled sites."""
+    c = CONFIGS["cfg1"]
+    L, T = 4, 7
+    U, D = make_propagators_numpy(c.seed, L, T)
+    t = wk.build_terms(c.nucleus)
+    mom = [(0, 0, 0), (1, 0, 3)]
+    monkeypatch.setenv("WICK_HOST_BLOCK_BYTES", str(2 * L ** 3 * 144 * 16))   # 2 timeslices per block: blocks of 2, 2, 2, 1
+    wk.launch_count(reset=True)
+    Ch, sh = wk.contract_host(U, D, t, mom, L, T, want_sigma=True)
+    n_multi = wk.launch_count(reset=True)
+    monkeypatch.delenv("WICK_HOST_BLOCK_BYTES")
+    Ch1 = wk.contract_host(U, D, t, mom, L, T)
+    n_single = wk.launch_count(reset=True)
+    assert n_multi > n_single                                   # the hook really cut the call into several blocks
+    # bitwise equal to device calls on the same blocks (the order of the sums inside a site depends on the number of
+    # 32-site groups of a batch, so calls of different shape agree to rounding, calls of equal shape bit for bit)
+    for t0 in (0, 2, 4, 6):
+        nt = min(2, T - t0)
+        Cd, sd = wk.contract(_dev(U[t0:t0 + nt], cuda_device), _dev(D[t0:t0 + nt], cuda_device), t, mom, L, nt, want_sigma=True)
+        assert np.array_equal(Ch[:, t0:t0 + nt], Cd.cpu().numpy()) and np.array_equal(sh[t0:t0 + nt], sd.cpu().numpy())
+    Cfull, sfull = wk.contract(_dev(U, cuda_device), _dev(D, cuda_device), t, mom, L, T, want_sigma=True)
+    assert np.array_equal(Ch1, Cfull.cpu().numpy())
+    assert np.all(np.abs(sh - sfull.cpu().numpy()) <= 1e-13 * np.abs(sh).max(axis=1, keepdims=True) * 1e3)
+    for (tt, x) in ((0, 0), (1, 63), (2, 17), (5, 40), (6, 5), (6, 63)):
+        ref, sabs = _oracle_site("cfg1", U[tt, x], D[tt, x])
+        assert abs(sh[tt, x] - ref) <= REL_TOL * sabs
+
+
+@pytest.mark.parametrize("cfg,L,T", [("cfg1", 3, 2), ("cfg3", 2, 1)])
+def test_isospin_lists_on_the_gpu(cfg, L, T, cuda_device):
+    """U == D (the paper's m_u = m_d): the swap-symmetrised factorised list (WICK_BUILD_ISOSPIN) and, for
+    the deuteron, the flat list merged by the randomised identity test (IDENTITY_TEST | ISOSPIN) against the oracle's
+    full expansion evaluated with D = U; and such handles refuse U != D."""
+    c = CONFIGS[cfg]
+    mom = [(0, 0, 0), (1, 0, 1)]
+    U, Dother = make_propagators_numpy(c.seed, L, T)
+    Ud = _dev(U, cuda_device)
+    Cr, sr, sabs = _oracle_lattice(cfg, U, U, mom, L)
+    handles = [wk.build_terms(c.nucleus, flags=wk.BUILD_ISOSPIN)]
+    if cfg == "cfg1":
+        handles.append(wk.build_terms(c.nucleus, flags=wk.BUILD_IDENTITY_TEST | wk.BUILD_ISOSPIN, seed=9))
+        assert handles[1].info.n_terms == 26721 and handles[1].info.is_outer_product == 0
+    for t in handles:
+        Cg, sg = wk.contract(Ud, Ud, t, mom, L, T, want_sigma=True)
+        assert np.all(np.abs(sg.cpu().numpy() - sr) <= REL_TOL * sabs), (np.abs(sg.cpu().numpy() - sr) / sabs).max()
+        _check_C(Cg.cpu().numpy(), Cr, sabs.sum(axis=1))
+        with pytest.raises(wk.WickError, match="U_dev == D_dev"):
+            wk.contract(Ud, _dev(Dother, cuda_device), t, mom, L, T)
+
+
+@pytest.mark.parametrize("cfg", ["cfg4", "cfg4b"])
+def test_jacobi_complementary_minor_path(cfg, cuda_device):
+    """WICK_CONTRACT_JACOBI: 10x10 / 11x11 minors as det A times a 2x2 / 1x1 minor of the inverse, against the
+    oracle (which eliminates every minor itself) on a small lattice with the full list, on sampled sites at full size, and
+    against the LU path of the library."""
+    c = CONFIGS[cfg]
+    L, T, mom = SHRUNK[cfg]
+    U, D = make_propagators_numpy(c.seed, L, T)
+    t = _terms_for(cfg)
+    Ud, Dd = _dev(U, cuda_device), _dev(D, cuda_device)
+    Cg, sg = wk.contract(Ud, Dd, t, mom, L, T, want_sigma=True, flags=wk.CONTRACT_JACOBI)
+    Cg, sg = Cg.cpu().numpy(), sg.cpu().numpy()
+    Cr, sr, sabs = _oracle_lattice(cfg, U, D, mom, L)
+    assert np.all(np.abs(sg - sr) <= REL_TOL * sabs), (np.abs(sg - sr) / sabs).max()
+    _check_C(Cg, Cr, sabs.sum(axis=1))
+    Clu = wk.contract(Ud, Dd, t, mom, L, T).cpu().numpy()
+    _check_C(Cg, Clu, sabs.sum(axis=1))
+    tt = 0
+    U1, D1 = make_propagators_numpy(c.seed, c.L, c.T, t0=tt, nt=1)
+    _, s1 = wk.contract(_dev(U1, cuda_device), _dev(D1, cuda_device), t, c.momenta, c.L, 1, want_sigma=True, flags=wk.CONTRACT_JACOBI)
+    s1 = s1.cpu().numpy()
+    for (_, s) in sample_site_times(c.seed, c.L, c.T, 6, times=[tt]):
+        ref, sa = _oracle_site(cfg, U1[0, s], D1[0, s])
+        assert abs(s1[0, s] - ref) <= REL_TOL * sa
+
+
+@pytest.mark.parametrize("n_u,n_d", [(9, 10), (8, 11), (11, 7)])
+def test_jacobi_path_on_generic_lists(n_u, n_d, cuda_device):
+    """Complement sizes 1..4 on one side, an LU-only size (7) on the other: the two paths mix per flavour."""
+    L, T, mom = 2, 2, [(0, 0, 0), (1, 0, 1)]
+    U, D = make_propagators_numpy(950 + n_u, L, T)
+    lst = make_random_term_list(70 + n_d, n_u, n_d, 300)
+    t = wk.build_terms_from_list(*lst)
+    Cg, sg = wk.contract(_dev(U, cuda_device), _dev(D, cuda_device), t, mom, L, T, want_sigma=True, flags=wk.CONTRACT_JACOBI)
+    sg = sg.cpu().numpy()
+    sr, sabs = np.zeros((T, L ** 3), complex), np.zeros((T, L ** 3))
+    for tt in range(T):
+        for x in range(L ** 3):
+            sr[tt, x], sabs[tt, x] = wo.site_terms_value(U[tt, x], D[tt, x], *lst)
+    assert np.all(np.abs(sg - sr) <= REL_TOL * sabs), (np.abs(sg - sr) / sabs).max()
+    _check_C(Cg.cpu().numpy(), wo.reduce_sites(sr, mom, L), sabs.sum(axis=1))
+
+
+def test_correlation_matrix_shares_the_determinants(cuda_device):
+    """wick_contract_many (GEVP, Sec. V PAPER.md:394-420): the 2x2 correlation matrix of {p n product operator, Eq. (20)}
+    against the oracle's sink x conj(source) expansion for every entry, with the minors launched once for all four."""
+    L, T, mom = 3, 2, [(0, 0, 0), (1, 0, 2)]
+    U, D = make_propagators_numpy(4321, L, T)
+    Ud, Dd = _dev(U, cuda_device), _dev(D, cuda_device)
+    ops = [wk.operator_from_nucleons(CONFIGS["cfg1"].nucleus), wk.operator_paper(wk.OP_DEUTERON_EQ20)]
+    m = wk.build_terms_matrix(ops)
+    lists = [m[k][kp] for k in range(2) for kp in range(2)]
+    wk.contract_many(Ud, Dd, lists, mom, L, T)                   # uploads the tables
+    wk.profile_enable(True)
+    Cg, sg = wk.contract_many(Ud, Dd, lists, mom, L, T, want_sigma=True)
+    prof = wk.profile_read()
+    wk.profile_enable(False)
+    assert prof["minors_u"][1] == 1 and prof["minors_d"][1] == 1 and prof["reduce"][1] == 4   # a4 once, a5 per entry
+    Cg, sg = Cg.cpu().numpy(), sg.cpu().numpy()
+    osink = [wo.merged_terms(CONFIGS["cfg1"].nucleus), wo.merged_from_raw(wo.deuteron_eq20_raw_terms())]
+    for k in range(2):
+        for kp in range(2):
+            sr, sabs = np.zeros((T, L ** 3), complex), np.zeros((T, L ** 3))
+            for tt in range(T):
+                for x in range(L ** 3):
+                    sr[tt, x], sabs[tt, x] = wo.site_value_outer(U[tt, x], D[tt, x], osink[k], osink[kp])
+            e = 2 * k + kp
+            assert np.all(np.abs(sg[e] - sr) <= REL_TOL * sabs), (k, kp, (np.abs(sg[e] - sr) / sabs).max())
+            _check_C(Cg[e], wo.reduce_sites(sr, mom, L), sabs.sum(axis=1))
+    # hermiticity of the correlation matrix entries that are each other's conjugate transpose only holds for U, D from a
+    # gauge average; what must hold exactly is that single-list calls reproduce the entries
+    C01 = wk.contract(Ud, Dd, m[0][1], mom, L, T).cpu().numpy()
+    assert np.allclose(C01, Cg[1], rtol=1e-12, atol=0)
+    other = wk.build_terms(CONFIGS["cfg0"].nucleus)
+    with pytest.raises(wk.WickError, match="share"):
+        wk.contract_many(Ud, Dd, [lists[0], other], mom, L, T)
