@@ -57,6 +57,8 @@ extern "C" {
 #define WICK_CONTRACT_JACOBI    16u  /* flavours with 8 <= n <= 11: Jacobi's complementary-minor identity (one 12x12 inverse + determinant */
                                      /* per site, then (12-n) x (12-n) minors of the inverse) instead of an LU per minor.  Error grows  */
                                      /* with the condition number of the propagator and a singular propagator contributes 0: opt-in.   */
+#define WICK_CONTRACT_JACOBI_UNFUSED 32u /* with JACOBI: keep the minor tables (inverse kernel + minors of the inverse + reduction) even  */
+                                     /* where the fused per-site kernel applies (both flavours 8..11, terms <= 8 x unique minors)        */
 #define WICK_CONTRACT_NO_STAGED  2u  /* factorised lists: walk the block items from L1/L2 instead of staging them in shared memory */
 
 #define WICK_NUCLEON_PROTON  0

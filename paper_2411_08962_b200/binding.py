@@ -22,6 +22,7 @@ CONTRACT_NO_STAGED = 2
 CONTRACT_COMPLEX_COEFFS = 4
 CONTRACT_NO_REG_MINORS = 8
 CONTRACT_JACOBI = 16
+CONTRACT_JACOBI_UNFUSED = 32
 
 EXPORTED_SYMBOLS = (
     "wick_build_terms", "wick_build_terms_from_list", "wick_terms_get_info", "wick_terms_export_tuples",

@@ -159,6 +159,36 @@ std::vector<uint64_t> build_jacobi_descs(const FlavourTables& ft) {
     return desc;
 }
 
+// Fused Jacobi path: flat term table with complementary index sets and the signs folded into the weights.
+int ensure_jacobi_fused(const wick_terms* t, cudaStream_t stream, const JacobiTerm** out) {
+    try { t->ensure_flat(); } catch (const std::bad_alloc&) { set_error("flat term list: out of host memory"); return WICK_ERR_NOMEM; }
+    std::lock_guard<std::mutex> lock(t->mu);
+    DeviceTables& d = t->dev;
+    if (d.jf_blob) { *out = static_cast<const JacobiTerm*>(d.jf_blob); return WICK_OK; }
+    std::vector<JacobiTerm> tab(size_t(t->n_terms));
+    auto comp = [](const FlavourTables& ft, int32_t m, int* sum) {
+        const uint16_t I = ft.rows[size_t(ft.minor_row[size_t(m)])], J = ft.cols[size_t(ft.minor_col[size_t(m)])];
+        for (int b = 0; b < 12; ++b) *sum += ((I >> b) & 1) * b + ((J >> b) & 1) * b;
+        return uint32_t(nibbles_of_mask(uint16_t(~J & 0xfff)) & 0xffffu) | (uint32_t(nibbles_of_mask(uint16_t(~I & 0xfff)) & 0xffffu) << 16);
+    };
+    for (size_t k = 0; k < tab.size(); ++k) {
+        int sum = 0;
+        tab[k].u_idx = comp(t->f[0], t->t_uid[k], &sum);
+        tab[k].d_idx = comp(t->f[1], t->t_did[k], &sum);
+        tab[k].pad[0] = tab[k].pad[1] = 0;
+        const double sg = (sum & 1) ? -1.0 : 1.0;
+        tab[k].w = make_double2(sg * t->t_w[k].real(), sg * t->t_w[k].imag());
+    }
+    void* blob = nullptr;
+    WICK_CUDA(cudaMalloc(&blob, std::max<size_t>(tab.size() * sizeof(JacobiTerm), 256)));
+    cudaError_t e = cudaMemcpyAsync(blob, tab.data(), tab.size() * sizeof(JacobiTerm), cudaMemcpyHostToDevice, stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(stream);
+    if (e != cudaSuccess) { cudaFree(blob); set_error(std::string("Jacobi term table upload: ") + cudaGetErrorString(e)); return WICK_ERR_CUDA; }
+    d.jf_blob = blob;
+    *out = static_cast<const JacobiTerm*>(blob);
+    return WICK_OK;
+}
+
 // Connected components of the bipartite graph (qu -- qd) of a factor list.  Physical sink lists are
 // block diagonal (He-4: 199 blocks of at most 15 x 15 tuples), so the factorised reduction
 //   sigma = sum_{ru,cd} (sum_i c_i MD[rd_i,cd]) (sum_j cbar_j MU[ru,cu_j])
@@ -770,6 +800,7 @@ size_t plan_bytes(const Plan& p, int64_t S_b) { return p.sigma_bytes + 1024 + si
 extern "C" void wick_terms_release_device(DeviceTables* d) {
     if (d->blob) cudaFree(d->blob);
     if (d->flat_blob) cudaFree(d->flat_blob);
+    if (d->jf_blob) cudaFree(d->jf_blob);
     for (auto& kv : d->staged) cudaFree(kv.second.blob);
     for (int f = 0; f < 2; ++f) for (auto& kv : d->reg[f]) cudaFree(kv.second.blob);
     *d = DeviceTables();
@@ -934,7 +965,21 @@ int contract_lists(const void* U_dev, const void* D_dev, const wick_terms* const
     const bool try_reg = t->outer && !(flags & WICK_CONTRACT_NO_REG_MINORS);
     bool use_jacobi[2];
     for (int f = 0; f < 2; ++f) use_jacobi[f] = (flags & WICK_CONTRACT_JACOBI) && d.jacobi_desc[f] != nullptr;
-    for (int64_t st0 = 0; st0 < p.n_st; st0 += S_b) {
+    // both flavours in the Jacobi range and a term list of the order of the minor tables (Li-7-sized lists): one fused kernel
+    // per list, no minor table at all
+    bool fused_jacobi = use_jacobi[0] && use_jacobi[1] && !(flags & WICK_CONTRACT_JACOBI_UNFUSED);
+    for (int k = 0; k < n_lists && fused_jacobi; ++k)
+        if (lists[k]->n_terms > 8 * (nmu + nmd) || lists[k]->n_terms >= (int64_t(1) << 31)) fused_jacobi = false;
+    if (fused_jacobi) {
+        for (int k = 0; k < n_lists; ++k) {
+            double2* sigma = sigma_all + int64_t(k) * p.n_st;
+            if (lists[k]->n_terms == 0) { WICK_CUDA(cudaMemsetAsync(sigma, 0, size_t(p.n_st) * 16, stream)); continue; }
+            const JacobiTerm* jt = nullptr;
+            if ((rc = ensure_jacobi_fused(lists[k], stream, &jt)) != WICK_OK) return rc;
+            WICK_CUDA(launch_jacobi_fused(t->n_u, t->n_d, U, D, 0, p.n_st, jt, lists[k]->n_terms, sigma, stream));
+        }
+    }
+    for (int64_t st0 = 0; st0 < p.n_st && !fused_jacobi; st0 += S_b) {
         const int64_t n_valid = std::min<int64_t>(S_b, p.n_st - st0);
         const int n_groups = int((n_valid + GROUP - 1) / GROUP);
         // grid tables of 6x6 minors: register-resident instance kernel, one wave of CTAs (8 warp bins each)

@@ -191,92 +191,222 @@ minors_kernel(const c128* __restrict__ P, int64_t st0, int64_t n_st_total, int S
 // ---------------------------------------------------------------------------------------------
 // a4 for minors of size n >= 8 through Jacobi's complementary-minor identity (optional, flag
 // WICK_CONTRACT_JACOBI):  det A[I, J] = (-1)^(sum I + sum J) det A  det (A^-1)[J^c, I^c].
-// inverse12_kernel: one thread per site inverts its 12x12 propagator in place in shared memory (Gauss-Jordan with
-// partial pivoting, same pivot rule as the LU kernels; the tile layout makes the per-lane row exchanges conflict free)
-// and returns det A; the (12-n) x (12-n) minors of the inverse then go through minors_kernel<12-n>.
+// inverse12_kernel: 16 lanes per site invert its 12x12 propagator in registers (Gauss-Jordan with partial pivoting, same
+// pivot rule as the LU kernels, pivot row broadcast by shuffles) and return det A; the (12-n) x (12-n) minors of the
+// inverse then go through minors_kernel<12-n>.
 // A singular propagator has no inverse: its site gets det = 0 and a zero matrix (every minor 0); use the LU path for such data.
 // ---------------------------------------------------------------------------------------------
-constexpr int INV_THREADS = 64;
+constexpr int INV_THREADS = 128;
+
+__device__ __forceinline__ double shfl16(double v, int src) { return __shfl_sync(0xffffffffu, v, src, 16); }
+
+// 16 lanes per site (12 used): lane = row of the propagator, its 12 entries in registers.  Gauss-Jordan in place without
+// moving rows: step k picks, among the lanes that have not been a pivot row yet, the one with the largest |re| + |im| in
+// column k (first wins); every lane then does  own[c] -= g * pivot_row[c]  with g = own[k] / piv (the pivot lane itself with
+// g = 1 - 1/piv, which scales it by 1/piv), and column k is replaced by the column of the inverse.  With p_k the pivot
+// lane of step k the lane p_i ends up holding (A^-1)[i][p_m] in register m.
+// Result of invert12 for one lane: row `my_step` of the inverse, entry m belongs to column p_m (4-bit fields of perm).
+struct InvRow { double re[12], im[12]; int my_step; unsigned long long perm; c128 det; bool singular; };
+
+// `bc`: 12 complex of shared memory per site, through which the pivot row of a step reaches the other lanes (one broadcast
+// LDS.128 per entry instead of four shuffles)
+__device__ __forceinline__ void invert12(const c128* __restrict__ P, int64_t st, bool row_ok, int sub, c128* bc, InvRow& R) {
+    double (&re)[12] = R.re;
+    double (&im)[12] = R.im;
+#pragma unroll
+    for (int c = 0; c < 12; ++c) {
+        c128 v = make_double2(0.0, 0.0);
+        if (row_ok) v = __ldg(P + st * 144 + sub * 12 + c);
+        re[c] = v.x; im[c] = v.y;
+    }
+    bool used = sub >= 12;                                                  // idle lanes never become pivots
+    int my_step = 0;                                                        // the step at which this lane was the pivot row
+    unsigned long long perm = 0;                                            // p_k, 4 bits each (the same on all lanes of a site)
+    c128 det = make_double2(1.0, 0.0);
+    bool singular = false;
+#pragma unroll
+    for (int k = 0; k < 12; ++k) {
+        // argmax of the pivot key over the 16 lanes of the site, smaller lane wins ties
+        int key = used ? -1 : pivot_key(re[k], im[k]);
+        int who = sub;
+#pragma unroll
+        for (int off = 8; off > 0; off >>= 1) {
+            const int k2 = __shfl_xor_sync(0xffffffffu, key, off, 16), w2 = __shfl_xor_sync(0xffffffffu, who, off, 16);
+            if (k2 > key || (k2 == key && w2 < who)) { key = k2; who = w2; }
+        }
+        const int p = who;
+        perm |= (unsigned long long)p << (4 * k);
+        const bool is_p = (sub == p);
+        if (is_p) { used = true; my_step = k; }
+        double pr[12], pi[12];
+        __syncwarp();                                                       // the previous step's reads of bc are done
+        if (is_p) {
+#pragma unroll
+            for (int c = 0; c < 12; ++c) bc[c] = make_double2(re[c], im[c]);
+        }
+        __syncwarp();
+#pragma unroll
+        for (int c = 0; c < 12; ++c) { const c128 v = bc[c]; pr[c] = v.x; pi[c] = v.y; }
+        const c128 piv = make_double2(pr[k], pi[k]);
+        singular = singular || (piv.x == 0.0 && piv.y == 0.0);
+        det = cmul(det, piv);
+        const c128 ip = crecip(piv);
+        // g = own[k] / piv for the other rows, 1 - 1/piv for the pivot row
+        c128 g = cmul(make_double2(re[k], im[k]), ip);
+        if (is_p) g = make_double2(1.0 - ip.x, -ip.y);
+#pragma unroll
+        for (int c = 0; c < 12; ++c) {
+            if (c == k) continue;
+            re[c] = fma(-g.x, pr[c], fma(g.y, pi[c], re[c]));
+            im[c] = fma(-g.x, pi[c], fma(-g.y, pr[c], im[c]));
+        }
+        re[k] = is_p ? ip.x : -g.x;
+        im[k] = is_p ? ip.y : -g.y;
+    }
+    // sign of the permutation k -> p_k
+    int inv_count = 0;
+#pragma unroll
+    for (int a = 0; a < 12; ++a)
+#pragma unroll
+        for (int b = a + 1; b < 12; ++b) inv_count += (int(perm >> (4 * a)) & 15) > (int(perm >> (4 * b)) & 15);
+    if (inv_count & 1) { det.x = -det.x; det.y = -det.y; }
+    if (singular) det = make_double2(0.0, 0.0);
+    R.my_step = my_step; R.perm = perm; R.det = det; R.singular = singular;
+}
+
+// store the lane's row of the inverse into a [12][12] matrix (global or shared)
+__device__ __forceinline__ void store_inv_row(const InvRow& R, c128* dst_matrix) {
+    c128* dst = dst_matrix + R.my_step * 12;
+#pragma unroll
+    for (int m = 0; m < 12; ++m) {
+        const int col = int(R.perm >> (4 * m)) & 15;
+        dst[col] = R.singular ? make_double2(0.0, 0.0) : make_double2(R.re[m], R.im[m]);
+    }
+}
 
 __global__ void __launch_bounds__(INV_THREADS)
-inverse12_kernel(const c128* __restrict__ P, int64_t st0, int64_t n_st_total, c128* __restrict__ inv_out, c128* __restrict__ det_out) {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    c128* tile = reinterpret_cast<c128*>(smem_raw) + size_t(warp) * TILE_ELEMS;
-    const int64_t g = int64_t(blockIdx.x) * (INV_THREADS / 32) + warp;      // 32-site group within the batch
-    const int64_t st_first = st0 + g * GROUP;
-    // stage (per warp): consecutive lanes read consecutive 16-byte elements of one site
-    for (int idx = lane; idx < TILE_ELEMS; idx += 32) {
-        const int site = idx / 144, e = idx - site * 144;
-        const int64_t st = st_first + site;
-        c128 v = make_double2(0.0, 0.0);
-        if (st < n_st_total) v = __ldg(P + st * 144 + e);
-        tile[e * GROUP + site] = v;
+inverse12_kernel(const c128* __restrict__ P, int64_t st0, int64_t n_st_total, int64_t n_batch, c128* __restrict__ inv_out, c128* __restrict__ det_out) {
+    const int sub = threadIdx.x & 15;                                       // row
+    const int64_t site = (int64_t(blockIdx.x) * INV_THREADS + threadIdx.x) >> 4;   // site within the batch
+    const int64_t st = st0 + site;
+    const bool live = site < n_batch && st < n_st_total;
+    const bool row_ok = live && sub < 12;
+    __shared__ __align__(16) c128 bcast[INV_THREADS / 16][12];
+    InvRow R;
+    invert12(P, st, row_ok, sub, bcast[threadIdx.x >> 4], R);
+    if (live && sub == 0) det_out[site] = R.det;
+    if (row_ok) store_inv_row(R, inv_out + site * 144);
+}
+
+// Fused Jacobi path for lists whose BOTH flavours have 8 <= n <= 11 and whose term count is of the order of the number of
+// unique minors (Li-7-sized lists): per site both propagators are inverted (16 lanes per site, registers), the inverses
+// go to shared memory, and the 16 lanes share the flat term list:
+//   sigma = det U det D sum_k w'_k det (U^-1)[J_u^c, I_u^c] det (D^-1)[J_d^c, I_d^c],   w'_k = w_k (-1)^(sum of the index sets)
+// Nothing but the propagators is read from and sigma written to global memory: 4608 B per site-time.
+constexpr int JF_SITES = INV_THREADS / 16;
+
+template <int M>
+__device__ __forceinline__ c128 small_minor(const c128* A, uint32_t idx) {   // rows = nibbles 0..3, columns = nibbles 4..7 of idx
+    if constexpr (M == 0) return make_double2(1.0, 0.0);
+    else {
+        int r[M], c[M];
+#pragma unroll
+        for (int i = 0; i < M; ++i) { r[i] = int(idx >> (4 * i)) & 15; c[i] = int(idx >> (16 + 4 * i)) & 15; }
+        auto a = [&](int i, int j) { return A[r[i] * 12 + c[j]]; };
+        if constexpr (M == 1) return a(0, 0);
+        else if constexpr (M == 2) return det2(a(0, 0), a(0, 1), a(1, 0), a(1, 1));
+        else if constexpr (M == 3) {
+            const c128 m0 = det2(a(1, 1), a(1, 2), a(2, 1), a(2, 2)), m1 = det2(a(1, 0), a(1, 2), a(2, 0), a(2, 2)), m2 = det2(a(1, 0), a(1, 1), a(2, 0), a(2, 1));
+            return cfma(a(0, 2), m2, cfnma(a(0, 1), m1, cmul(a(0, 0), m0)));
+        } else {
+            // Laplace expansion over the row pairs (0,1) x (2,3): six products of complementary 2x2 minors
+            const c128 s01 = det2(a(0, 0), a(0, 1), a(1, 0), a(1, 1)), s02 = det2(a(0, 0), a(0, 2), a(1, 0), a(1, 2)), s03 = det2(a(0, 0), a(0, 3), a(1, 0), a(1, 3));
+            const c128 s12 = det2(a(0, 1), a(0, 2), a(1, 1), a(1, 2)), s13 = det2(a(0, 1), a(0, 3), a(1, 1), a(1, 3)), s23 = det2(a(0, 2), a(0, 3), a(1, 2), a(1, 3));
+            const c128 t01 = det2(a(2, 0), a(2, 1), a(3, 0), a(3, 1)), t02 = det2(a(2, 0), a(2, 2), a(3, 0), a(3, 2)), t03 = det2(a(2, 0), a(2, 3), a(3, 0), a(3, 3));
+            const c128 t12 = det2(a(2, 1), a(2, 2), a(3, 1), a(3, 2)), t13 = det2(a(2, 1), a(2, 3), a(3, 1), a(3, 3)), t23 = det2(a(2, 2), a(2, 3), a(3, 2), a(3, 3));
+            c128 d = cmul(s01, t23);
+            d = cfnma(s02, t13, d); d = cfma(s03, t12, d); d = cfma(s12, t03, d); d = cfnma(s13, t02, d); d = cfma(s23, t01, d);
+            return d;
+        }
+    }
+}
+
+template <int MU_, int MD_>
+__global__ void __launch_bounds__(INV_THREADS, 4)
+jacobi_fused_kernel(const c128* __restrict__ U, const c128* __restrict__ D, bool same, int64_t st0, int64_t n_valid,
+                    const JacobiTerm* __restrict__ terms, int n_terms, c128* __restrict__ sigma) {
+    __shared__ __align__(16) c128 inv_s[JF_SITES][2][144];
+    const int sub = threadIdx.x & 15, ls = threadIdx.x >> 4;
+    const int64_t site = int64_t(blockIdx.x) * JF_SITES + ls;
+    const bool live = site < n_valid;
+    const bool row_ok = live && sub < 12;
+    __shared__ __align__(16) c128 bcast[JF_SITES][12];
+    c128 dets;
+    {
+        InvRow R;
+        invert12(U, st0 + site, row_ok, sub, bcast[ls], R);
+        if (row_ok) store_inv_row(R, inv_s[ls][0]);
+        dets = R.det;
+        if (!same) {
+            invert12(D, st0 + site, row_ok, sub, bcast[ls], R);
+            if (row_ok) store_inv_row(R, inv_s[ls][1]);
+            dets = cmul(dets, R.det);
+        } else dets = cmul(dets, dets);
     }
     __syncwarp();
-    c128* A = tile + lane;                                                  // A[r][c] at A[(12 r + c) * GROUP]
-    c128 det = make_double2(1.0, 0.0);
-    unsigned long long piv_rows = 0;                                        // pivot row of step k, 4 bits each
-    bool singular = false;
-#pragma unroll 1
-    for (int k = 0; k < 12; ++k) {
-        int p = k;
-        int best = -1;
-        for (int r = k; r < 12; ++r) {
-            const c128 v = A[(12 * r + k) * GROUP];
-            const int m = pivot_key(v.x, v.y);
-            if (m > best) { best = m; p = r; }
-        }
-        piv_rows |= (unsigned long long)p << (4 * k);
-        c128 rowk[12];
-#pragma unroll
-        for (int c = 0; c < 12; ++c) {                                      // exchange rows k and p, keep row k in registers
-            const c128 a = A[(12 * k + c) * GROUP], b = A[(12 * p + c) * GROUP];
-            A[(12 * p + c) * GROUP] = a;
-            rowk[c] = b;
-        }
-        const c128 piv = rowk[k];
-        det = cmul(det, piv);
-        if (p != k) { det.x = -det.x; det.y = -det.y; }
-        const c128 ip = crecip(piv);
-        singular = singular || (piv.x == 0.0 && piv.y == 0.0);
-        rowk[k] = make_double2(1.0, 0.0);
-#pragma unroll
-        for (int c = 0; c < 12; ++c) { rowk[c] = cmul(rowk[c], ip); A[(12 * k + c) * GROUP] = rowk[c]; }
-        for (int r = 0; r < 12; ++r) {
-            if (r == k) continue;
-            const c128 f = A[(12 * r + k) * GROUP];
-            A[(12 * r + k) * GROUP] = make_double2(0.0, 0.0);
-#pragma unroll
-            for (int c = 0; c < 12; ++c) A[(12 * r + c) * GROUP] = cfnma(f, rowk[c], A[(12 * r + c) * GROUP]);
-        }
+    const c128* Ui = inv_s[ls][0];
+    const c128* Di = same ? inv_s[ls][0] : inv_s[ls][1];
+    c128 acc = make_double2(0.0, 0.0);
+    for (int k = sub; k < n_terms; k += 16) {
+        const uint4 h = __ldg(reinterpret_cast<const uint4*>(terms + k));
+        const c128 w = __ldg(reinterpret_cast<const c128*>(terms + k) + 1);
+        acc = cfma(cmul(w, small_minor<MU_>(Ui, h.x)), small_minor<MD_>(Di, h.y), acc);
     }
-    for (int k = 11; k >= 0; --k) {                                         // undo the row exchanges on the columns
-        const int p = int(piv_rows >> (4 * k)) & 15;
-        if (p != k)
-            for (int r = 0; r < 12; ++r) {
-                const c128 a = A[(12 * r + k) * GROUP], b = A[(12 * r + p) * GROUP];
-                A[(12 * r + k) * GROUP] = b; A[(12 * r + p) * GROUP] = a;
-            }
+    // fixed-shape tree over the 16 lanes of the site
+#pragma unroll
+    for (int off = 8; off > 0; off >>= 1) {
+        acc.x += __shfl_xor_sync(0xffffffffu, acc.x, off, 16);
+        acc.y += __shfl_xor_sync(0xffffffffu, acc.y, off, 16);
     }
-    if (singular) {
-        det = make_double2(0.0, 0.0);
-        for (int e = 0; e < 144; ++e) A[e * GROUP] = make_double2(0.0, 0.0);
+    if (live && sub == 0) sigma[site] = cmul(acc, dets);
+}
+
+template <int MU_>
+static cudaError_t launch_jf_d(int md, const c128* U, const c128* D, int64_t st0, int64_t n_valid, const JacobiTerm* terms, int n_terms,
+                               c128* sigma, cudaStream_t stream) {
+    const unsigned grid = unsigned((n_valid + JF_SITES - 1) / JF_SITES);
+    const bool same = (U == D);
+    switch (md) {
+        case 1: jacobi_fused_kernel<MU_, 1><<<grid, INV_THREADS, 0, stream>>>(U, D, same, st0, n_valid, terms, n_terms, sigma); break;
+        case 2: jacobi_fused_kernel<MU_, 2><<<grid, INV_THREADS, 0, stream>>>(U, D, same, st0, n_valid, terms, n_terms, sigma); break;
+        case 3: jacobi_fused_kernel<MU_, 3><<<grid, INV_THREADS, 0, stream>>>(U, D, same, st0, n_valid, terms, n_terms, sigma); break;
+        case 4: jacobi_fused_kernel<MU_, 4><<<grid, INV_THREADS, 0, stream>>>(U, D, same, st0, n_valid, terms, n_terms, sigma); break;
+        default: return cudaErrorInvalidValue;
     }
-    if (st_first + lane < n_st_total) det_out[g * GROUP + lane] = det;
-    __syncwarp();
-    for (int idx = lane; idx < TILE_ELEMS; idx += 32) {                     // coalesced write-back, [site][12][12]
-        const int site = idx / 144, e = idx - site * 144;
-        if (st_first + site < n_st_total) inv_out[(g * GROUP + site) * 144 + e] = tile[e * GROUP + site];
+    return cudaGetLastError();
+}
+
+cudaError_t launch_jacobi_fused(int n_u, int n_d, const double2* U, const double2* D, int64_t st0, int64_t n_valid,
+                                const JacobiTerm* terms, int64_t n_terms, double2* sigma, cudaStream_t stream) {
+    if (n_valid <= 0) return cudaSuccess;
+    ProfScope prof(PROF_MINORS_U, stream);
+    ++g_launches;
+    switch (12 - n_u) {
+        case 1: return launch_jf_d<1>(12 - n_d, U, D, st0, n_valid, terms, int(n_terms), sigma, stream);
+        case 2: return launch_jf_d<2>(12 - n_d, U, D, st0, n_valid, terms, int(n_terms), sigma, stream);
+        case 3: return launch_jf_d<3>(12 - n_d, U, D, st0, n_valid, terms, int(n_terms), sigma, stream);
+        case 4: return launch_jf_d<4>(12 - n_d, U, D, st0, n_valid, terms, int(n_terms), sigma, stream);
+        default: return cudaErrorInvalidValue;
     }
 }
 
 cudaError_t launch_inverse12(const double2* P, int64_t st0, int64_t n_st_total, int n_groups, double2* inv_out, double2* det_out,
                              int prof_cls, cudaStream_t stream) {
     if (n_groups == 0) return cudaSuccess;
-    const int per_cta = INV_THREADS / 32;
+    const int64_t n_batch = int64_t(n_groups) * GROUP;
+    const int sites_per_cta = INV_THREADS / 16;
     ProfScope prof(prof_cls, stream);
-    inverse12_kernel<<<(n_groups + per_cta - 1) / per_cta, INV_THREADS, size_t(per_cta) * TILE_BYTES, stream>>>(P, st0, n_st_total, inv_out, det_out);
+    inverse12_kernel<<<unsigned((n_batch + sites_per_cta - 1) / sites_per_cta), INV_THREADS, 0, stream>>>(P, st0, n_st_total, n_batch, inv_out, det_out);
     ++g_launches;
     return cudaGetLastError();
 }
@@ -959,7 +1089,7 @@ cudaError_t launch_finalize_sigma(const double2* partial, int n_chunks, int S_b,
     return cudaGetLastError();
 }
 
-constexpr int PROJ_THREADS = 256;
+constexpr int PROJ_THREADS = 1024;      // one CTA per (momentum, timeslice): latency bound, so as many threads as a CTA can have
 
 // one CTA per (momentum, timeslice): each thread sums its sites in index order, then a fixed tree
 __global__ void __launch_bounds__(PROJ_THREADS)
@@ -1054,7 +1184,6 @@ template <int N> static cudaError_t set_smem_attr() {
 cudaError_t configure_kernels() {
     cudaError_t e;
     if ((e = configure_reg_kernels()) != cudaSuccess) return e;
-    if ((e = cudaFuncSetAttribute(inverse12_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, int(INV_THREADS / 32 * TILE_BYTES))) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(minors_large_cached_kernel<10, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(mlc_smem<10, 0>()))) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(minors_large_cached_kernel<11, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(mlc_smem<11, 1>()))) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(minors6_cached_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, int(M6C_SMEM))) != cudaSuccess) return e;

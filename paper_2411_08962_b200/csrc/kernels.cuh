@@ -35,8 +35,7 @@ cudaError_t launch_minors(int n, const double2* P, int64_t st0, int64_t n_st_tot
 // columns, up to REG_NC_MAX candidate columns behind them, and the trie of the instance's column tuples over candidate
 // POSITIONS as a word program.  The minors of a job are stored in trie order from column position out_base of the row
 // tuple's list.
-constexpr int REG_THREADS = 384;          // 12 warps: 3 per scheduler
-constexpr int REG_NS = 6;                 // candidate positions kept in the per-thread shared-memory copy; the rest in registers
+constexpr int REG_THREADS = 256;
 constexpr int REG_NC_MAX = 10;
 struct RegJob {
     unsigned long long lead, cand;        // column indices as 4-bit fields: leading (K), candidates (ncand)
@@ -98,6 +97,12 @@ cudaError_t launch_reduce_staged(const double2* MU, const double2* MD, int n_gro
 // scale_a / scale_b: NULL or per-site factors multiplied into sigma (Jacobi path: det U, det D)
 cudaError_t launch_finalize_sigma(const double2* partial, int n_chunks, int S_b, int64_t n_valid,
                                   double2* sigma_batch, const double2* scale_a, const double2* scale_b, cudaStream_t stream);
+// Fused Jacobi path (both flavours 8 <= n <= 11): one term = complementary index sets of both minors (rows J^c in nibbles
+// 0..3, columns I^c in nibbles 4..7) and the weight with the Jacobi signs folded in; sigma[site] for sites st0 .. st0 + n_valid - 1
+struct JacobiTerm { uint32_t u_idx, d_idx, pad[2]; double2 w; };
+static_assert(sizeof(JacobiTerm) == 32, "JacobiTerm is read with 16-byte loads");
+cudaError_t launch_jacobi_fused(int n_u, int n_d, const double2* U, const double2* D, int64_t st0, int64_t n_valid,
+                                const JacobiTerm* terms, int64_t n_terms, double2* sigma, cudaStream_t stream);
 // Jacobi path: inverse [site in batch][12][12] and determinant [site in batch] of the propagators st0 .. of a site batch
 cudaError_t launch_inverse12(const double2* P, int64_t st0, int64_t n_st_total, int n_groups, double2* inv_out, double2* det_out,
                              int prof_cls, cudaStream_t stream);

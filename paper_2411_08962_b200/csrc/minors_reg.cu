@@ -152,154 +152,11 @@ minors_reg_kernel(const c128* __restrict__ P, int64_t st0, int64_t n_st_total, i
     }
 }
 
-// ---------------------------------------------------------------------------------------------
-// Variant with 12 warps per SM: only the LAST NC - NS candidate positions live in registers (they are the last columns of
-// most minors: static last level), the first NS positions live in the per-thread shared-memory copy and are fetched by
-// dynamic index.  A register position used as i3 / i4 is reached through a uniform switch over static code.
-// ---------------------------------------------------------------------------------------------
-template <int NC, int NS>
-struct Trie12 {
-    static constexpr int NR = NC - NS;
-    c128 T[NR][4];                    // Schur columns of positions NS .. NC-1
-    c128 s[6];
-    c128 c3[4];
-    c128* o;
-    size_t step;
-    bool valid;
-    __device__ __forceinline__ void emit(const c128 (&t)[4]) {
-        const c128 e0 = cfma(t[1], c3[1], cmul(t[0], c3[0]));
-        const c128 e1 = cfma(t[3], c3[3], cmul(t[2], c3[2]));
-        if (valid) *o = cadd(e0, e1);
-        o += step;
-    }
-};
-
-template <int NC, int NS, int I5>
-__device__ __forceinline__ void finish_regs(Trie12<NC, NS>& c, uint32_t mask5) {
-    if constexpr (I5 < NC) {
-        if ((mask5 >> I5) & 1u) c.emit(c.T[I5 - NS]);
-        finish_regs<NC, NS, I5 + 1>(c, mask5);
-    }
-}
-
-template <int NC, int NS, int P>
-__device__ __forceinline__ void reg_column(const Trie12<NC, NS>& c, uint32_t pos, c128 (&t)[4]) {   // uniform switch, static register reads
-    if constexpr (P < NC - 1) {
-        if (pos == uint32_t(P)) {
-#pragma unroll
-            for (int r = 0; r < 4; ++r) t[r] = c.T[P - NS][r];
-        } else reg_column<NC, NS, P + 1>(c, pos, t);
-    }
-}
-
-template <int N, int NC, int NS, int NT, int J>
-__device__ __forceinline__ void schur_columns12(const LuState<N, 0, NT>& lu, const unsigned char* tb, unsigned long long cand,
-                                                int ncand, Trie12<NC, NS>& c, c128* Sc) {
-    if constexpr (J < NC) {
-        if (J < ncand) {
-            if constexpr (J < NS) {
-                c128 t[4];
-                lu.schur_column(tb, nullptr, (uint32_t(cand >> (4 * J)) & 15u) * uint32_t(GROUP * 16), t);
-#pragma unroll
-                for (int r = 0; r < 4; ++r) Sc[(J * 4 + r) * NT] = t[r];
-            } else {
-                lu.schur_column(tb, nullptr, (uint32_t(cand >> (4 * J)) & 15u) * uint32_t(GROUP * 16), c.T[J - NS]);
-            }
-        }
-        schur_columns12<N, NC, NS, NT, J + 1>(lu, tb, cand, ncand, c, Sc);
-    }
-}
-
-template <int NS, int NT> constexpr size_t reg12_smem() { return size_t(TILE_BYTES) + size_t(NS) * 4 * 16 * NT; }
-
-template <int N, int NC, int NS, int NT>
-__global__ void __launch_bounds__(NT, 1)
-minors_reg12_kernel(const c128* __restrict__ P, int64_t st0, int64_t n_st_total, int S_b, RegTables rt, c128* __restrict__ out) {
-    constexpr int K = N - 4;
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    c128* tile = reinterpret_cast<c128*>(smem_raw);
-    c128* Sc = tile + TILE_ELEMS + threadIdx.x;
-    const int g = blockIdx.x;
-    const int64_t st_first = st0 + int64_t(g) * GROUP;
-    const int lane = threadIdx.x & 31;
-    const int warp = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0);
-    stage_tile(tile, P, st_first, n_st_total, NT);
-    __syncthreads();
-    const unsigned char* tb = reinterpret_cast<const unsigned char*>(tile + lane);
-    constexpr uint32_t kRowStep = 12 * GROUP * 16, kColStep = GROUP * 16;
-    const int bin = blockIdx.y * (NT / 32) + warp;
-    const int j0 = __ldg(rt.bin_ptr + bin), j1 = __ldg(rt.bin_ptr + bin + 1);
-    Trie12<NC, NS> c;
-    c.valid = st_first + lane < n_st_total;
-    c.step = size_t(S_b);
-    c128* outp = out + int64_t(g) * GROUP + lane;
-    auto column = [&](uint32_t pos, c128 (&t)[4]) {                    // any position: shared-memory copy or register switch
-        if (pos < uint32_t(NS)) {
-#pragma unroll
-            for (int r = 0; r < 4; ++r) t[r] = Sc[(pos * 4 + r) * NT];
-        } else reg_column<NC, NS, NS>(c, pos, t);
-    };
-    for (int j = j0; j < j1; ++j) {
-        const uint32_t jr = __ldg(rt.bin_jobs + j);
-        const RegJob* job = rt.jobs + (jr & 255u);
-        const uint32_t r = jr >> 8;
-        const uint32_t rows = __ldg(rt.row_nibbles + r);
-        const ulonglong2 h0 = __ldg(reinterpret_cast<const ulonglong2*>(job));
-        const uint4 h1 = __ldg(reinterpret_cast<const uint4*>(job) + 1);
-        c128 detp;
-        {
-            LuState<N, 0, NT> lu;
-            uint32_t rb[N], cb[N];
-#pragma unroll
-            for (int i = 0; i < N; ++i) { rb[i] = ((rows >> (4 * i)) & 15u) * kRowStep; cb[i] = (i < K) ? (uint32_t(h0.x >> (4 * i)) & 15u) * kColStep : 0u; }
-            lu.start(tb, nullptr, rb, cb);
-            schur_columns12<N, NC, NS, NT, 0>(lu, tb, h0.y, int(h1.x), c, Sc);
-            detp = lu.detp;
-        }
-        c.o = outp + (size_t(r) * size_t(rt.n_cols) + size_t(h1.w)) * size_t(S_b);
-        const uint32_t* pw = rt.prog + h1.y;
-        const uint32_t* const pend = rt.prog + h1.z;
-        while (pw < pend) {
-            const uint32_t w = __ldg(pw++);
-            const uint32_t n3 = w >> 8;
-            {
-                c128 a[4], b[4];
-                column(w & 15u, a);
-                column((w >> 4) & 15u, b);
-#pragma unroll
-                for (int q = 0; q < 4; ++q) a[q] = cmul(detp, a[q]);
-                int k = 0;
-#pragma unroll
-                for (int x = 0; x < 4; ++x)
-#pragma unroll
-                    for (int y = x + 1; y < 4; ++y) c.s[k++] = det2(a[x], b[x], a[y], b[y]);
-            }
-            for (uint32_t q = 0; q < n3; ++q) {
-                const uint32_t w3 = __ldg(pw++);
-                {
-                    c128 t[4];
-                    column(w3 & 15u, t);
-                    third_from(c.s, t, c.c3);
-                }
-                const uint32_t mask5 = w3 >> 4;
-                for (uint32_t m = mask5 & ((1u << NS) - 1u); m; m &= m - 1u) {   // last columns that live in shared memory (ascending)
-                    c128 t[4];
-                    const uint32_t pos = uint32_t(__ffs(int(m)) - 1);
-#pragma unroll
-                    for (int rr = 0; rr < 4; ++rr) t[rr] = Sc[(pos * 4 + rr) * NT];
-                    c.emit(t);
-                }
-                finish_regs<NC, NS, NS>(c, mask5);
-            }
-        }
-    }
-}
-
 cudaError_t launch_minors_reg_impl(int n, const double2* P, int64_t st0, int64_t n_st_total, int n_groups, int S_b,
                                    const RegTables& rt, double2* out, cudaStream_t stream) {
     if (n_groups == 0 || rt.n_bins == 0) return cudaSuccess;
     dim3 grid(n_groups, rt.n_bins / (REG_THREADS / 32));
-    if (n == 6) minors_reg12_kernel<6, 10, REG_NS, REG_THREADS><<<grid, REG_THREADS, reg12_smem<REG_NS, REG_THREADS>(), stream>>>(P, st0, n_st_total, S_b, rt, out);
+    if (n == 6) minors_reg_kernel<6, 10><<<grid, REG_THREADS, reg_smem<10>(), stream>>>(P, st0, n_st_total, S_b, rt, out);
     else return cudaErrorInvalidValue;
     return cudaGetLastError();
 }
@@ -307,7 +164,7 @@ cudaError_t launch_minors_reg_impl(int n, const double2* P, int64_t st0, int64_t
 bool minors_reg_supported(int n, int max_candidates) { return n == 6 && max_candidates <= 10; }
 
 cudaError_t configure_reg_kernels() {
-    return cudaFuncSetAttribute(minors_reg12_kernel<6, 10, REG_NS, REG_THREADS>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(reg12_smem<REG_NS, REG_THREADS>()));
+    return cudaFuncSetAttribute(minors_reg_kernel<6, 10>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(reg_smem<10>()));
 }
 
 }  // namespace wick

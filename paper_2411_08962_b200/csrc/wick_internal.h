@@ -72,6 +72,7 @@ struct DeviceTables {
     int reg_state[2] = {0, 0};                  // per flavour: 0 = not checked, 1 = register-resident minors kernel usable, -1 = not
     std::map<int, RegDev> reg[2];               // by number of warp bins per site group
     // flat list (uploaded only when the flat path runs)
+    void* jf_blob = nullptr;                    // fused Jacobi path: flat terms with complementary index sets (contract.cu)
     void* flat_blob = nullptr;
     const int32_t* t_uid = nullptr;
     const int32_t* t_did = nullptr;

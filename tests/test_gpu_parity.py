@@ -395,6 +395,10 @@ def test_jacobi_complementary_minor_path(cfg, cuda_device):
     _check_C(Cg, Cr, sabs.sum(axis=1))
     Clu = wk.contract(Ud, Dd, t, mom, L, T).cpu().numpy()
     _check_C(Cg, Clu, sabs.sum(axis=1))
+    # the same identity through the minor tables (inverse kernel, minors of the inverse, reduction) instead of the fused per-site kernel
+    Cu, su = wk.contract(Ud, Dd, t, mom, L, T, want_sigma=True, flags=wk.CONTRACT_JACOBI | wk.CONTRACT_JACOBI_UNFUSED)
+    assert np.all(np.abs(su.cpu().numpy() - sr) <= REL_TOL * sabs)
+    _check_C(Cu.cpu().numpy(), Cr, sabs.sum(axis=1))
     tt = 0
     U1, D1 = make_propagators_numpy(c.seed, c.L, c.T, t0=tt, nt=1)
     _, s1 = wk.contract(_dev(U1, cuda_device), _dev(D1, cuda_device), t, c.momenta, c.L, 1, want_sigma=True, flags=wk.CONTRACT_JACOBI)
