@@ -370,10 +370,11 @@ def rooflines(wk, cfg, terms, info, prof, ms_step, Tb, fp64_probe, hbm_gbs, d_ru
                             "algorithmic_bytes_per_timeslice": 4608.0 * cfg.volume}
 
 
-def bench_workload(wk, torch, cfg, key, Tb, steps, warmup, dev, fp64_probe, hbm_gbs, isospin=False, sampler=None):
-    """One workload on this rank's GPU, device-resident inputs: timeslices/s, rooflines, launches.  Single-GPU path."""
+def bench_workload(wk, torch, cfg, key, Tb, steps, warmup, dev, fp64_probe, hbm_gbs, isospin=False, sampler=None, flags=0):
+    """One workload on this rank's GPU, device-resident inputs: timeslices/s, rooflines, launches.  Single-GPU path.
+    isospin: one propagator for both flavours and the swap-symmetrised factorised list (WICK_BUILD_ISOSPIN)."""
     from wick_inputs import make_propagators_torch
-    terms = workload_terms(wk, cfg)
+    terms = wk.build_terms(cfg.nucleus, flags=wk.BUILD_ISOSPIN) if isospin else workload_terms(wk, cfg)
     info = terms.info
     n_mom = len(cfg.momenta)
     Tb = min(Tb, cfg.T)
@@ -384,7 +385,7 @@ def bench_workload(wk, torch, cfg, key, Tb, steps, warmup, dev, fp64_probe, hbm_
     Cout = torch.empty((n_mom, Tb), dtype=torch.complex128, device=dev)
 
     def step():
-        wk.contract(U, D, terms, cfg.momenta, cfg.L, Tb, workspace=ws, out=Cout)
+        wk.contract(U, D, terms, cfg.momenta, cfg.L, Tb, workspace=ws, out=Cout, flags=flags)
 
     for _ in range(max(warmup, 3)):
         step()
@@ -404,10 +405,23 @@ def bench_workload(wk, torch, cfg, key, Tb, steps, warmup, dev, fp64_probe, hbm_
     prof = class_times(wk, torch, step, max(1, min(3, steps)))
     wk.launch_count(reset=True)
     d_runs = 1.0 if prof["minors_d"][1] > 0 else 0.0
-    minors, reduce, extra = rooflines(wk, cfg, terms, info, prof, ms_step, Tb, fp64_probe, hbm_gbs, d_runs)
     st = Tb * cfg.volume
+    if (flags & wk.CONTRACT_JACOBI) and prof["reduce"][1] == 0:
+        # fused Jacobi kernel: propagators in, sigma out -- HBM bound by construction (4608 B per site-time)
+        ms_k = prof["minors_u"][0]
+        gbs = st * (4608.0 + 16.0) / (ms_k * 1e-3) / 1e9
+        minors = {"bound": "hbm", "kernel": "jacobi_fused_kernel (a3-a5: two 12x12 inversions per site + complementary minors + term sum)",
+                  "achieved": gbs, "peak": hbm_gbs, "unit": "GB/s", "frac": gbs / hbm_gbs if hbm_gbs else None,
+                  "achieved_is": "4608 B of propagators + 16 B of sigma per site-time / CUDA-event time of the kernel",
+                  "peak_source": "MEASURED_PEAKS.json hbm_gbs", "traffic": None, "launches_per_step": int(prof["minors_u"][1]),
+                  "avg_launch_ms": ms_k / max(prof["minors_u"][1], 1), "kernel_share_of_step": ms_k / ms_step,
+                  "note": "Jacobi complementary minors change the work, not only the rate: compare timeslices/s with the LU record, not FP64 %"}
+        reduce, extra = None, {"project_ms_per_step": prof["project"][0]}
+    else:
+        minors, reduce, extra = rooflines(wk, cfg, terms, info, prof, ms_step, Tb, fp64_probe, hbm_gbs, d_runs)
     rec = {
-        "workload": cfg.name, "value": Tb / (ms_step * 1e-3), "unit": "timeslices/s", "ms_per_step": ms_step, "steps": steps,
+        "workload": cfg.name, "contract_flags": int(flags), "isospin_u_equals_d": bool(isospin),
+        "value": Tb / (ms_step * 1e-3), "unit": "timeslices/s", "ms_per_step": ms_step, "steps": steps,
         "timeslices_per_step": Tb, "L": cfg.L, "n_u": info.n_u, "n_d": info.n_d, "n_terms": int(info.n_terms),
         "unique_minors_per_site": int(info.n_minors_u + info.n_minors_d),
         "minor_dets_per_s": st * (info.n_minors_u + info.n_minors_d) / (ms_step * 1e-3),
@@ -579,6 +593,20 @@ def main():
             if not args.no_cpu_baseline:
                 rec["cpu_baseline"] = cpu_baseline_rows(CONFIGS[key], key, 4, False)
             workloads[CONFIGS[key].name] = rec
+            torch.cuda.empty_cache()
+            if CONFIGS[key].n_u >= 8 and CONFIGS[key].n_d >= 8:
+                # the same workload through Jacobi's complementary-minor identity (opt-in flag)
+                rec, _, _ = bench_workload(wk, torch, CONFIGS[key], key, args.timeslices_per_step, args.side_steps, args.warmup, dev,
+                                           fp64_probe, hbm_gbs, flags=wk.CONTRACT_JACOBI)
+                workloads[CONFIGS[key].name + "+jacobi"] = rec
+                torch.cuda.empty_cache()
+        if not cfg.random_list and cfg.n_u == cfg.n_d and not args.isospin:
+            # isospin limit of the headline workload (the paper's m_u = m_d): one propagator, one minor table,
+            # swap-symmetrised factorised list
+            rec, _, _ = bench_workload(wk, torch, cfg, args.workload, args.timeslices_per_step, max(args.steps, 2), args.warmup, dev,
+                                       fp64_probe, hbm_gbs, isospin=True)
+            rec["speedup_over_two_flavour_run"] = rec["value"] / value
+            workloads[cfg.name + "+isospin"] = rec
             torch.cuda.empty_cache()
 
     cpu_baseline = None

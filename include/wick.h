@@ -124,7 +124,7 @@ int wick_build_terms_from_list(int n_u, int n_d, int64_t n_raw,
  * wick_build_terms_matrix: n_ops operators with the same quark content -> n_ops^2 handles, out[k * n_ops + k'] =
  * (operator k at the sink) x conj(operator k' at the source), all over ONE pair of unique-minor tables (union of the row /
  * column tuples), so that wick_contract_many evaluates every determinant once for the whole correlation matrix.
- * Each handle is an ordinary wick_terms (free every one with wick_terms_free). */
+ * Each handle is an ordinary term-list handle: free every one with wick_terms_free. */
 typedef struct wick_operator wick_operator;
 #define WICK_OP_DEUTERON_EQ20 1
 #define WICK_OP_HELIUM3_EQ21  2

@@ -25,19 +25,19 @@ template <int NC>
 struct Trie {
     c128 T[NC][4];                    // Schur columns of the candidate positions (registers: the static last level)
     c128 s[6];                        // 2x2 minors of (detp * T[i2], T[i3]) over the row pairs 01 02 03 12 13 23
-    c128 c3[4];                       // signed 3x3 minors of (.., T[i4])
+    c128 c3[4];                       // 3x3 minors of (.., T[i4]) over the row triples that leave out row r
     c128* o;                          // where the next minor goes (this lane)
     size_t step;                      // S_b
     bool valid;
 };
 
-// signed 3x3 minors of (.., t): c3[r] = (-1)^(r+3) det(rows != r), expanded along the last column in the 2x2 minors s
+// 3x3 minors of (.., t): c3[r] = det(rows != r), expanded along the last column in the 2x2 minors s
 __device__ __forceinline__ void third_from(const c128 (&s)[6], const c128 (&t)[4], c128 (&c3)[4]) {
     const c128 m0 = cfma(t[3], s[3], cfnma(t[2], s[4], cmul(t[1], s[5])));   // rows 1,2,3
     const c128 m1 = cfma(t[3], s[1], cfnma(t[2], s[2], cmul(t[0], s[5])));   // rows 0,2,3
     const c128 m2 = cfma(t[3], s[0], cfnma(t[1], s[2], cmul(t[0], s[4])));   // rows 0,1,3
     const c128 m3 = cfma(t[2], s[0], cfnma(t[1], s[1], cmul(t[0], s[3])));   // rows 0,1,2
-    c3[0] = make_double2(-m0.x, -m0.y); c3[1] = m1; c3[2] = make_double2(-m2.x, -m2.y); c3[3] = m3;
+    c3[0] = m0; c3[1] = m1; c3[2] = m2; c3[3] = m3;              // UNSIGNED: the alternating sign is taken in the Laplace sum below
 }
 
 // last level, static in the candidate position: det = sum_r T[I5][r] c3[r]
@@ -45,8 +45,8 @@ template <int NC, int I5>
 __device__ __forceinline__ void finish_all(Trie<NC>& c, uint32_t mask5) {
     if constexpr (I5 < NC) {
         if ((mask5 >> I5) & 1u) {
-            const c128 e0 = cfma(c.T[I5][1], c.c3[1], cmul(c.T[I5][0], c.c3[0]));
-            const c128 e1 = cfma(c.T[I5][3], c.c3[3], cmul(c.T[I5][2], c.c3[2]));
+            const c128 e0 = cfnma(c.T[I5][0], c.c3[0], cmul(c.T[I5][1], c.c3[1]));   // -t0 m0 + t1 m1
+            const c128 e1 = cfnma(c.T[I5][2], c.c3[2], cmul(c.T[I5][3], c.c3[3]));   // -t2 m2 + t3 m3
             if (c.valid) *c.o = cadd(e0, e1);
             c.o += c.step;
         }
