@@ -1146,8 +1146,9 @@ extern "C" int wick_contract_host(const void* U_host, const void* D_host, const 
         set_error("wick_contract_host: bad argument"); return WICK_ERR_ARG; }
     const int64_t V = int64_t(L) * L * L;
     // Timeslice blocks: propagators of block b+1 are copied on a second stream while block b computes.
-    // Each block is an independent wick_contract over Tb timeslices (per-timeslice results do not
-    // depend on the blocking: the reduction over sites of one timeslice always has the same shape).
+    // Each block is an independent wick_contract over Tb timeslices.  The sum over the sites of a timeslice always has the
+    // same shape; the order of the partial sums inside a site follows the number of 32-site groups per site batch, so
+    // blockings with different batch shapes agree to rounding and equal shapes bit for bit.
     const size_t slice_bytes = size_t(V) * 144 * 16;
     size_t block_bytes = size_t(256) << 20;
     if (const char* ev = std::getenv("WICK_HOST_BLOCK_BYTES")) {   // test hook: small blocks exercise the double-buffered path

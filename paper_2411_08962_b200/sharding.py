@@ -1,8 +1,9 @@
 """Timeslice sharding over ranks (the paper reports near-linear 2- and 4-node scaling
 without describing the split).  Every (site, timeslice) is independent up to the sum over
 sites of ONE timeslice (Eq. A2), so rank r contracts the timeslices t = r, r + N, r + 2N, ... of its own
-propagator shard with no collective on the data path; the per-timeslice reduction order equals the single-GPU one,
-so results are bitwise equal.  The only exchange is the final gather of C[p][t] (at most a few KB).
+propagator shard with no collective on the data path; the per-timeslice reduction order equals the single-GPU one
+whenever the site batches have the same shape (always at BASELINE's sizes, where the batch is capped by the workspace
+target), and then results are bitwise equal; otherwise they agree to rounding.  The only exchange is the final gather of C[p][t] (at most a few KB).
 
 `torch.distributed` is plumbing here: any backend works (nccl on GPUs, gloo in the CPU tests)."""
 from __future__ import annotations
