@@ -450,6 +450,7 @@ def main():
     ap.add_argument("--side-workloads", default="cfg4,cfg4b", help="comma list measured in the same run and reported under "
                     "'workloads' (north_star names Li-7 next to He-4); '' to skip")
     ap.add_argument("--side-steps", type=int, default=400)
+    ap.add_argument("--no-isospin-record", action="store_true", help="skip the extra U == D record of the headline workload")
     ap.add_argument("--isospin", action="store_true",
                     help="side measurement, not the headline: one propagator for both flavours (the paper's m_u = m_d, "
                          "PAPER.md:518); flavours with equal unique-minor tables then share one evaluation")
@@ -600,7 +601,7 @@ def main():
                                            fp64_probe, hbm_gbs, flags=wk.CONTRACT_JACOBI)
                 workloads[CONFIGS[key].name + "+jacobi"] = rec
                 torch.cuda.empty_cache()
-        if not cfg.random_list and cfg.n_u == cfg.n_d and not args.isospin:
+        if not cfg.random_list and cfg.n_u == cfg.n_d and not args.isospin and not args.no_isospin_record:
             # isospin limit of the headline workload (the paper's m_u = m_d): one propagator, one minor table,
             # swap-symmetrised factorised list
             rec, _, _ = bench_workload(wk, torch, cfg, args.workload, args.timeslices_per_step, max(args.steps, 2), args.warmup, dev,

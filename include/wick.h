@@ -138,6 +138,26 @@ int  wick_operator_export(const wick_operator* op, uint8_t* u_tuples, uint8_t* d
 void wick_operator_free(wick_operator* op);
 int  wick_build_terms_matrix(const wick_operator* const* ops, int n_ops, unsigned flags, wick_terms** out);
 
+/* ---- cluster sinks (the block algorithm of Eq. 6-8 :110-125 when the clusters are single nucleons) -----------
+ * Two clusters A (quarks at sink site x) and B (quarks at sink site y), each projected to its own momentum:
+ *     C(t) = sum_{x,y} e^{i p_A.x} e^{i p_B.y} < O_A(x,t) O_B(y,t)  Obar_source(0) >.
+ * The stacked determinants are expanded along the rows of cluster A (generalised Laplace expansion), so the two site sums
+ * factorise into the block tensors   B_X[t][S_u][S_d] = sum_x e^{i p.x} sum_i c_i det U_x[a_u(i), S_u] det D_x[a_d(i), S_d]
+ * over ALL column subsets S_u, S_d (lexicographic order of the ascending tuples), evaluated on the device by
+ * wick_block_tensor from a block handle (wick_build_block_terms), and combined on the host, lattice independent, by
+ * wick_combine_two_clusters:  C[t] = (-1)^(|d_A||u_B|) sum_j conj(c_j) sum_{S_u, S_d} sign B_A[t][S_u][S_d] B_B[t][b_u(j) \ S_u][b_d(j) \ S_d].
+ * wick_operator_product: the ordered product A.B (the natural source operator).  The device kernel is flat over the sink
+ * terms of the cluster: meant for small clusters (nucleons, deuteron); a He-4-sized cluster needs a factorised kernel (not built).
+ *   out_dev   : device complex128 [T][C(12,n_u)][C(12,n_d)];  momentum: host int32 [3];  workspace >= _workspace_bytes, 256-byte aligned.
+ *   BA_reim, BB_reim: host copies of the two block tensors;  C_reim: host double [T][2]. */
+int  wick_operator_product(const wick_operator* a, const wick_operator* b, wick_operator** out);
+int  wick_build_block_terms(const wick_operator* cluster, wick_terms** out);
+size_t wick_block_tensor_workspace_bytes(const wick_terms* block_terms, int L);
+int  wick_block_tensor(const void* U_dev, const void* D_dev, const wick_terms* block_terms, const int32_t* momentum, int L, int T,
+                       void* out_dev, void* workspace_dev, size_t workspace_bytes, unsigned flags, void* cuda_stream);
+int  wick_combine_two_clusters(const wick_operator* a, const wick_operator* b, const wick_operator* source,
+                               const double* BA_reim, const double* BB_reim, int T, double* C_reim);
+
 int  wick_terms_get_info(const wick_terms* terms, wick_terms_info* info);
 
 /* Copy the tables out (host, caller-allocated; any pointer may be NULL to skip it).

@@ -404,6 +404,53 @@ def site_value_method_b(U: np.ndarray, D: np.ndarray, sink, source=None):
     return complex(_sum_ld(np.array(parts))), float(sum(absparts))
 
 
+# ----------------------------------------------------------------------------------------------
+# Cluster sinks ("a cluster sink can be employed where each cluster ... [is] projected to zero momentum
+# separately"; Eq. 3 / Eq. 8, PAPER.md:100, :125 for two nucleons): cluster A sits at sink site x, cluster B at sink site y
+# ----------------------------------------------------------------------------------------------
+
+def two_cluster_site_pair_value(Ux, Dx, Uy, Dy, sink_a, sink_b, source):
+    """sum over sink terms iA of cluster A (quarks at site x), iB of cluster B (quarks at site y) and source terms j of
+         c_A c_B conj(c_j) <q(A; x) q(B; y)  qbar(source)>
+    in determinant form (Eq. 12-15): the u Wick matrix has the rows a_u(A) taken from U_x followed by the rows
+    a_u(B) taken from U_y, columns b_u(j); likewise d.  Bringing  u_A d_A u_B d_B  to  u_A u_B d_A d_B  moves |u_B| fields past
+    |d_A| fields: sign (-1)^(|d_A| |u_B|).  `source` is the merged list of the product operator A.B at the source.
+    Returns (value, sum of |terms|)."""
+    bu = np.array([t[0] for t in source], dtype=np.intp)
+    bd = np.array([t[1] for t in source], dtype=np.intp)
+    cq = np.conj(np.array([t[2] for t in source], dtype=np.complex128))
+    total, total_abs = [], 0.0
+    for (ua, da, ca) in sink_a:
+        for (ub, db, cb) in sink_b:
+            sign = -1.0 if (len(da) * len(ub)) % 2 else 1.0
+            ua_, ub_, da_, db_ = (np.asarray(v, dtype=np.intp) for v in (ua, ub, da, db))
+            Mu = np.concatenate([Ux[ua_[None, :, None], bu[:, None, :]], Uy[ub_[None, :, None], bu[:, None, :]]], axis=1)
+            Md = np.concatenate([Dx[da_[None, :, None], bd[:, None, :]], Dy[db_[None, :, None], bd[:, None, :]]], axis=1)
+            v = (sign * ca * cb * cq) * det_elim(Mu) * det_elim(Md)
+            total.append(_sum_ld(v))
+            total_abs += float(np.sum(np.abs(v)))
+    return complex(_sum_ld(np.array(total))), total_abs
+
+
+def two_cluster_correlator(U, D, sink_a, sink_b, source, mom_a, mom_b, L: int):
+    """C(t) = sum_{x,y} e^{i p_A.x} e^{i p_B.y} <O_A(x,t) O_B(y,t) Obar(0)>  for U, D of shape [T][L^3][12][12]: every cluster is
+    projected to its own momentum (the plane-wave sink of Eq. 8 when the clusters are single nucleons).
+    Returns (C [T], S_abs [T])."""
+    T, V = U.shape[0], U.shape[1]
+    pa, pb = momentum_phases(L, [mom_a])[0], momentum_phases(L, [mom_b])[0]
+    C = np.zeros(T, dtype=np.complex128)
+    sabs = np.zeros(T)
+    for t in range(T):
+        vals = []
+        for x in range(V):
+            for y in range(V):
+                v, a = two_cluster_site_pair_value(U[t, x], D[t, x], U[t, y], D[t, y], sink_a, sink_b, source)
+                vals.append(pa[x] * pb[y] * v)
+                sabs[t] += a
+        C[t] = _sum_ld(np.array(vals))
+    return C, sabs
+
+
 def momentum_phases(L: int, momenta: Sequence[Tuple[int, int, int]]) -> np.ndarray:
     """e^{+2 pi i (n.x)/L} for every site s = x + L*(y + L*z); shape [n_mom][L^3].  (n.x) is reduced
     mod L in integers first so the phase is exact at multiples of L/4."""

@@ -31,7 +31,8 @@ EXPORTED_SYMBOLS = (
     "wick_contract_min_workspace_bytes", "wick_contract_workspace_bytes", "wick_contract",
     "wick_contract_host", "wick_release_cached_buffers", "wick_minor_dets", "wick_terms_minor_table", "wick_launch_count", "wick_launch_count_reset",
     "wick_operator_from_nucleons", "wick_operator_from_raw", "wick_operator_paper", "wick_operator_info", "wick_operator_export",
-    "wick_operator_free", "wick_build_terms_matrix", "wick_contract_many", "wick_contract_many_workspace_bytes",
+    "wick_operator_free", "wick_operator_product", "wick_build_block_terms", "wick_block_tensor", "wick_block_tensor_workspace_bytes",
+    "wick_combine_two_clusters", "wick_build_terms_matrix", "wick_contract_many", "wick_contract_many_workspace_bytes",
     "wick_last_error", "wick_version", "wick_profile_enable", "wick_profile_read", "wick_measure_fp64_peak",
 )
 
@@ -99,6 +100,12 @@ def load_library():
     lib.wick_operator_export.argtypes = [vp, vp, vp, vp]
     lib.wick_operator_free.argtypes = [vp]
     lib.wick_operator_free.restype = None
+    lib.wick_operator_product.argtypes = [vp, vp, C.POINTER(vp)]
+    lib.wick_build_block_terms.argtypes = [vp, C.POINTER(vp)]
+    lib.wick_block_tensor_workspace_bytes.argtypes = [vp, i32]
+    lib.wick_block_tensor_workspace_bytes.restype = sz
+    lib.wick_block_tensor.argtypes = [vp, vp, vp, vp, i32, i32, vp, vp, sz, u32, vp]
+    lib.wick_combine_two_clusters.argtypes = [vp, vp, vp, vp, vp, i32, vp]
     lib.wick_build_terms_matrix.argtypes = [C.POINTER(vp), i32, u32, C.POINTER(vp)]
     lib.wick_contract_many_workspace_bytes.argtypes = [vp, i32, i32, i32, i32]
     lib.wick_contract_many_workspace_bytes.restype = sz
@@ -279,6 +286,60 @@ def operator_paper(which: int, J: int = 0) -> Operator:
     h = C.c_void_p()
     _check(load_library().wick_operator_paper(which, J, C.byref(h)), "wick_operator_paper")
     return Operator(h.value)
+
+
+def operator_product(a: Operator, b: Operator) -> Operator:
+    """The ordered product A.B of two interpolators (Grassmann product, canonical form)."""
+    h = C.c_void_p()
+    _check(load_library().wick_operator_product(a._h, b._h, C.byref(h)), "wick_operator_product")
+    return Operator(h.value)
+
+
+def build_block_terms(cluster: Operator) -> Terms:
+    """Block handle of one cluster of a cluster sink (wick_build_block_terms): rows = the cluster's row tuples, columns =
+    every subset of the 12 source indices."""
+    h = C.c_void_p()
+    _check(load_library().wick_build_block_terms(cluster._h, C.byref(h)), "wick_build_block_terms")
+    return Terms(h.value)
+
+
+def block_tensor(U, D, block_terms: Terms, momentum, L: int, T: int, flags: int = 0, stream=None):
+    """B[t][S_u][S_d] = sum_x e^{ip.x} sum_i c_i det U_x[a_u(i), S_u] det D_x[a_d(i), S_d] on the device
+    (wick_block_tensor).  Returns CUDA complex128 [T][C(12,n_u)][C(12,n_d)]."""
+    import torch
+    lib = load_library()
+    V = L ** 3
+    _check_dev(U, "U", (T, V, 12, 12))
+    _check_dev(D, "D", (T, V, 12, 12))
+    mom = np.ascontiguousarray(momentum, dtype=np.int32).reshape(3)
+    i = block_terms.info
+    with torch.cuda.device(U.device), torch.cuda.stream(torch.cuda.current_stream() if stream is None else stream):
+        ws = torch.empty(int(lib.wick_block_tensor_workspace_bytes(block_terms._h, L)), dtype=torch.uint8, device=U.device)
+        out = torch.empty((T, i.n_cols_u, i.n_cols_d), dtype=torch.complex128, device=U.device)
+        rc = lib.wick_block_tensor(U.data_ptr(), D.data_ptr(), block_terms._h, _np_ptr(mom), L, T, out.data_ptr(), ws.data_ptr(),
+                                   ws.numel(), flags, _stream_ptr(stream))
+    _check(rc, "wick_block_tensor")
+    return out
+
+
+def combine_two_clusters(a: Operator, b: Operator, source: Operator, BA, BB) -> np.ndarray:
+    """C[t] from the two block tensors (host numpy complex128 [T][..][..]) and the source operator (wick_combine_two_clusters)."""
+    BA = np.ascontiguousarray(BA, dtype=np.complex128)
+    BB = np.ascontiguousarray(BB, dtype=np.complex128)
+    T = BA.shape[0]
+    out = np.zeros(T, np.complex128)
+    _check(load_library().wick_combine_two_clusters(a._h, b._h, source._h, _np_ptr(BA), _np_ptr(BB), T, _np_ptr(out)),
+           "wick_combine_two_clusters")
+    return out
+
+
+def two_cluster_correlator(U, D, a: Operator, b: Operator, mom_a, mom_b, L: int, T: int, source: Optional[Operator] = None):
+    """Cluster-sink correlator C[t] = sum_{x,y} e^{ip_A.x} e^{ip_B.y} <O_A(x) O_B(y) Obar_source(0)>  (the
+    plane-wave sink of Eq. 8 for single nucleons): two block tensors on the device, combined on the host."""
+    source = operator_product(a, b) if source is None else source
+    BA = block_tensor(U, D, build_block_terms(a), mom_a, L, T).cpu().numpy()
+    BB = block_tensor(U, D, build_block_terms(b), mom_b, L, T).cpu().numpy()
+    return combine_two_clusters(a, b, source, BA, BB)
 
 
 def build_terms_matrix(ops: Sequence[Operator], flags: int = 0):

@@ -801,6 +801,7 @@ extern "C" void wick_terms_release_device(DeviceTables* d) {
     if (d->blob) cudaFree(d->blob);
     if (d->flat_blob) cudaFree(d->flat_blob);
     if (d->jf_blob) cudaFree(d->jf_blob);
+    if (d->block_blob) cudaFree(d->block_blob);
     for (auto& kv : d->staged) cudaFree(kv.second.blob);
     for (int f = 0; f < 2; ++f) for (auto& kv : d->reg[f]) cudaFree(kv.second.blob);
     *d = DeviceTables();
@@ -1063,6 +1064,85 @@ extern "C" int wick_contract_many(const void* U_dev, const void* D_dev, const wi
                                   void* workspace_dev, size_t workspace_bytes, unsigned flags, void* cuda_stream) {
     return contract_lists(U_dev, D_dev, lists, n_lists, momenta, n_mom, L, T, C_out_dev, sigma_out_dev, workspace_dev, workspace_bytes,
                           flags, cuda_stream, "wick_contract_many");
+}
+
+// Cluster sinks: block tensor B[t][S_u][S_d] of a block handle (wick_build_block_terms), one timeslice after the other so that
+// a 32-site group never straddles two timeslices.  Workspace: minors of a site batch + per-group partial tensors of a timeslice.
+extern "C" size_t wick_block_tensor_workspace_bytes(const wick_terms* t, int L) {
+    if (!t || !t->block_mode || L < 1) return 0;
+    const int64_t V = int64_t(L) * L * L;
+    const int64_t nm = int64_t(t->f[0].minor_row.size()) + int64_t(t->f[1].minor_row.size());
+    const int64_t n_pairs = int64_t(t->f[0].cols.size()) * int64_t(t->f[1].cols.size());
+    const int64_t groups = (V + GROUP - 1) / GROUP;
+    int64_t sb = std::min<int64_t>(groups * GROUP, std::max<int64_t>(GROUP, int64_t(TARGET_MINOR_BYTES / size_t(nm * 16)) / GROUP * GROUP));
+    return size_t(sb * nm * 16 + groups * n_pairs * 16 + 1024);
+}
+
+extern "C" int wick_block_tensor(const void* U_dev, const void* D_dev, const wick_terms* t, const int32_t* momentum, int L, int T,
+                                 void* out_dev, void* workspace_dev, size_t workspace_bytes, unsigned flags, void* cuda_stream) {
+    if (!U_dev || !D_dev || !t || !momentum || !out_dev || !workspace_dev || L < 1 || T < 1) { set_error("wick_block_tensor: bad argument"); return WICK_ERR_ARG; }
+    if (!t->block_mode) { set_error("wick_block_tensor: not a block handle (wick_build_block_terms)"); return WICK_ERR_ARG; }
+    if ((reinterpret_cast<uintptr_t>(U_dev) | reinterpret_cast<uintptr_t>(D_dev) | reinterpret_cast<uintptr_t>(out_dev)) & 15 ||
+        reinterpret_cast<uintptr_t>(workspace_dev) & 255) { set_error("wick_block_tensor: misaligned buffer"); return WICK_ERR_ARG; }
+    if (workspace_bytes < wick_block_tensor_workspace_bytes(t, L)) { set_error("wick_block_tensor: workspace smaller than wick_block_tensor_workspace_bytes()"); return WICK_ERR_WORKSPACE; }
+    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    int rc = ensure_configured();
+    if (rc != WICK_OK) return rc;
+    if ((rc = upload_tables(t, stream)) != WICK_OK) return rc;
+    DeviceTables& d = t->dev;
+    const int n_sink = int(t->sink.size());
+    {   // sink terms as flat (row tuple ids, coefficient) arrays
+        std::lock_guard<std::mutex> lock(t->mu);
+        if (!d.block_blob) {
+            const size_t ns = size_t(n_sink);
+            std::vector<int32_t> ru(ns), rd(ns);
+            std::vector<double> c(2 * ns);
+            for (int i = 0; i < n_sink; ++i) { ru[size_t(i)] = t->sink[size_t(i)].qu; rd[size_t(i)] = t->sink[size_t(i)].qd; c[2 * size_t(i)] = t->sink[size_t(i)].c.real(); c[2 * size_t(i) + 1] = t->sink[size_t(i)].c.imag(); }
+            BlobBuilder bb;
+            const size_t o_c = bb.add(c.data(), c.size() * 8), o_u = bb.add(ru.data(), ru.size() * 4), o_d = bb.add(rd.data(), rd.size() * 4);
+            void* blob = nullptr;
+            WICK_CUDA(cudaMalloc(&blob, std::max<size_t>(bb.host.size(), 256)));
+            cudaError_t e = cudaMemcpyAsync(blob, bb.host.data(), bb.host.size(), cudaMemcpyHostToDevice, stream);
+            if (e == cudaSuccess) e = cudaStreamSynchronize(stream);
+            if (e != cudaSuccess) { cudaFree(blob); set_error(std::string("block table upload: ") + cudaGetErrorString(e)); return WICK_ERR_CUDA; }
+            d.block_blob = blob;
+            d.block_c = static_cast<unsigned char*>(blob) + o_c; d.block_ru = static_cast<unsigned char*>(blob) + o_u; d.block_rd = static_cast<unsigned char*>(blob) + o_d;
+        }
+    }
+    const int64_t V = int64_t(L) * L * L;
+    const int64_t nmu = int64_t(t->f[0].minor_row.size()), nmd = int64_t(t->f[1].minor_row.size());
+    const int n_cu = int(t->f[0].cols.size()), n_cd = int(t->f[1].cols.size());
+    const int64_t n_pairs = int64_t(n_cu) * n_cd;
+    const int64_t groups_t = (V + GROUP - 1) / GROUP;
+    const int S_b = int(std::min<int64_t>(groups_t * GROUP, std::max<int64_t>(GROUP, int64_t(TARGET_MINOR_BYTES / size_t((nmu + nmd) * 16)) / GROUP * GROUP)));
+    double2* MU = static_cast<double2*>(workspace_dev);
+    double2* MD = MU + nmu * S_b;
+    double2* part = MD + nmd * S_b;
+    const double2* U = static_cast<const double2*>(U_dev);
+    const double2* D = static_cast<const double2*>(D_dev);
+    const bool try_reg = !(flags & WICK_CONTRACT_NO_REG_MINORS);
+    for (int tt = 0; tt < T; ++tt) {
+        const int64_t t_end = int64_t(tt + 1) * V;                     // lanes beyond the timeslice are invalid
+        for (int64_t s0 = 0; s0 < V; s0 += S_b) {
+            const int64_t n_valid = std::min<int64_t>(S_b, V - s0);
+            const int n_groups = int((n_valid + GROUP - 1) / GROUP);
+            const int reg_bins = std::max(1, (148 + n_groups - 1) / n_groups) * (REG_THREADS / 32);
+            for (int f = 0; f < 2; ++f) {
+                RegTables rt;
+                rc = try_reg ? ensure_reg(t, f, reg_bins, stream, &rt) : 0;
+                if (rc < 0) return rc;
+                const double2* Pf = f == 0 ? U : D;
+                double2* Mf = f == 0 ? MU : MD;
+                const int pc = f == 0 ? PROF_MINORS_U : PROF_MINORS_D;
+                if (rc == 1) WICK_CUDA(launch_minors_reg(t->f[f].n, Pf, int64_t(tt) * V + s0, t_end, n_groups, S_b, rt, Mf, pc, stream));
+                else WICK_CUDA(launch_minors(t->f[f].n, Pf, int64_t(tt) * V + s0, t_end, n_groups, S_b, d.minor_desc[f], f == 0 ? nmu : nmd, true, Mf, pc, stream));
+            }
+            WICK_CUDA(launch_block_tensor(MU, MD, S_b, int(n_valid), n_cu, n_cd, static_cast<const int32_t*>(d.block_ru), static_cast<const int32_t*>(d.block_rd),
+                                          static_cast<const double2*>(d.block_c), n_sink, L, s0, momentum, part + (s0 / GROUP) * n_pairs, stream));
+        }
+        WICK_CUDA(launch_block_sum(part, int(groups_t), int(n_pairs), static_cast<double2*>(out_dev) + int64_t(tt) * n_pairs, stream));
+    }
+    return WICK_OK;
 }
 
 // Step a4 for one flavour of a handle, through exactly the kernels wick_contract launches for it (tests: every minor of

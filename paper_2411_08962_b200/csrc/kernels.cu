@@ -10,6 +10,7 @@
 //                            the active column and the multipliers (O(N^2) selects, not O(N^3)).
 //  a5  reduce_flat / reduce_outer : sigma(x,t) = sum_k w_k MU[uid_k] MD[did_k]  (Eq. A1-A5)
 //  a6  finalize_sigma, project    : fixed-order sum of the partials, momentum phases, fixed tree over sites
+#include <algorithm>
 #include <vector>
 
 #include "kernels.cuh"
@@ -1134,6 +1135,78 @@ cudaError_t launch_project(const double2* sigma, int L, int T, const MomentumLis
     return cudaGetLastError();
 }
 
+
+// ---------------------------------------------------------------------------------------------
+// Cluster sinks (block algorithm Eq. 6-8): block tensor of one cluster,
+//   part[g][cu][cd] = sum_{site in group g} e^{ip.x} sum_i c_i MU[ru_i, cu] MD[rd_i, cd]
+// lane = site, one (cu, cd) pair per warp iteration, fixed shuffle tree over the 32 sites; the groups of a timeslice are
+// summed in order by block_sum_kernel.  Flat over the sink terms: meant for small clusters (nucleons, deuteron).
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256)
+block_tensor_kernel(const c128* __restrict__ MU, const c128* __restrict__ MD, int S_b, int n_valid, int n_cu, int n_cd,
+                    const int32_t* __restrict__ sink_ru, const int32_t* __restrict__ sink_rd, const c128* __restrict__ sink_c, int n_sink,
+                    int L, int64_t site0, int3 mom, c128* __restrict__ part /* [group][n_cu * n_cd] of this batch */) {
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int g = blockIdx.x;
+    const int s = g * GROUP + lane;
+    const bool valid = s < n_valid;
+    const int sl = valid ? s : 0;
+    // e^{+2 pi i (n.x)/L}, (n.x) reduced mod L in integers
+    const int64_t site = site0 + sl;
+    const int x = int(site % L), y = int((site / L) % L), z = int(site / (int64_t(L) * L));
+    long long m = (long long)mom.x * x + (long long)mom.y * y + (long long)mom.z * z;
+    m %= L; if (m < 0) m += L;
+    double sn, cs;
+    sincospi(2.0 * double(m) / double(L), &sn, &cs);
+    const c128 ph = valid ? make_double2(cs, sn) : make_double2(0.0, 0.0);
+    const int n_pairs = n_cu * n_cd;
+    for (int p = blockIdx.y * 8 + warp; p < n_pairs; p += gridDim.y * 8) {
+        const int cu = p / n_cd, cd = p - cu * n_cd;
+        c128 acc = make_double2(0.0, 0.0);
+        for (int i = 0; i < n_sink; ++i) {
+            const c128 u = MU[(int64_t(__ldg(sink_ru + i)) * n_cu + cu) * S_b + sl];
+            const c128 d = MD[(int64_t(__ldg(sink_rd + i)) * n_cd + cd) * S_b + sl];
+            acc = cfma(cmul(__ldg(sink_c + i), u), d, acc);
+        }
+        acc = cmul(acc, ph);
+#pragma unroll
+        for (int off = 16; off > 0; off >>= 1) {
+            acc.x += __shfl_xor_sync(0xffffffffu, acc.x, off);
+            acc.y += __shfl_xor_sync(0xffffffffu, acc.y, off);
+        }
+        if (lane == 0) part[int64_t(g) * n_pairs + p] = acc;
+    }
+}
+
+__global__ void block_sum_kernel(const c128* __restrict__ part, int n_groups, int n_pairs, c128* __restrict__ out) {
+    const int p = blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= n_pairs) return;
+    c128 acc = make_double2(0.0, 0.0);
+    for (int g = 0; g < n_groups; ++g) acc = cadd(acc, part[int64_t(g) * n_pairs + p]);
+    out[p] = acc;
+}
+
+cudaError_t launch_block_tensor(const double2* MU, const double2* MD, int S_b, int n_valid, int n_cu, int n_cd,
+                                const int32_t* sink_ru, const int32_t* sink_rd, const double2* sink_c, int n_sink,
+                                int L, int64_t site0, const int mom[3], double2* part, cudaStream_t stream) {
+    const int n_groups = (n_valid + GROUP - 1) / GROUP;
+    if (n_groups == 0) return cudaSuccess;
+    const int n_pairs = n_cu * n_cd;
+    int chunks = std::max(1, std::min((n_pairs + 7) / 8, (148 * 8 + n_groups - 1) / n_groups));
+    dim3 grid(n_groups, chunks);
+    ProfScope prof(PROF_REDUCE, stream);
+    block_tensor_kernel<<<grid, 256, 0, stream>>>(MU, MD, S_b, n_valid, n_cu, n_cd, sink_ru, sink_rd, sink_c, n_sink, L, site0,
+                                                  make_int3(mom[0], mom[1], mom[2]), part);
+    ++g_launches;
+    return cudaGetLastError();
+}
+
+cudaError_t launch_block_sum(const double2* part, int n_groups, int n_pairs, double2* out, cudaStream_t stream) {
+    ProfScope prof(PROF_PROJECT, stream);
+    block_sum_kernel<<<(n_pairs + 127) / 128, 128, 0, stream>>>(part, n_groups, n_pairs, out);
+    ++g_launches;
+    return cudaGetLastError();
+}
 
 // ---------------------------------------------------------------------------------------------
 // Measurement helper: register-only DFMA stream (the FP64 roofline denominator)

@@ -108,6 +108,12 @@ cudaError_t launch_inverse12(const double2* P, int64_t st0, int64_t n_st_total, 
                              int prof_cls, cudaStream_t stream);
 cudaError_t launch_project(const double2* sigma, int L, int T, const MomentumList& mom, double2* C_out,
                            cudaStream_t stream);
+// cluster sinks: part[group][cu][cd] of one site batch of ONE timeslice (site0 = index of the batch's first site inside the
+// timeslice), then the ordered sum over the groups of the timeslice
+cudaError_t launch_block_tensor(const double2* MU, const double2* MD, int S_b, int n_valid, int n_cu, int n_cd,
+                                const int32_t* sink_ru, const int32_t* sink_rd, const double2* sink_c, int n_sink,
+                                int L, int64_t site0, const int mom[3], double2* part, cudaStream_t stream);
+cudaError_t launch_block_sum(const double2* part, int n_groups, int n_pairs, double2* out, cudaStream_t stream);
 cudaError_t configure_kernels();          // cudaFuncSetAttribute for the large-shared-memory kernels (once per device)
 
 int64_t launch_counter_get();

@@ -721,6 +721,109 @@ extern "C" int wick_build_terms_matrix(const wick_operator* const* ops, int n_op
     }
 }
 
+extern "C" int wick_operator_product(const wick_operator* a, const wick_operator* b, wick_operator** out) {
+    if (!a || !b || !out) { set_error("wick_operator_product: NULL argument"); return WICK_ERR_ARG; }
+    *out = nullptr;
+    if (a->n_u + b->n_u > 12 || a->n_d + b->n_d > 12) { set_error("wick_operator_product: more than 12 quarks of one flavour"); return WICK_ERR_ARG; }
+    try {
+        wick_operator* op = new wick_operator();
+        op->poly = poly_mul(a->poly, b->poly, 1.0);
+        operator_finish(op);
+        *out = op;
+        return WICK_OK;
+    } catch (const std::bad_alloc&) { set_error("wick_operator_product: out of host memory"); return WICK_ERR_NOMEM; }
+}
+
+// all n-subsets of {0..11} as masks, in lexicographic tuple order
+static std::vector<uint16_t> all_subsets(int n) {
+    std::vector<uint16_t> v;
+    for (unsigned m = 0; m < 4096; ++m) if (popc(m) == n) v.push_back(uint16_t(m));
+    std::sort(v.begin(), v.end(), tuple_less);
+    return v;
+}
+
+// Cluster sinks (block algorithm Eq. 6-8 :110-125): block handle of ONE cluster.  Rows = the cluster's own row
+// tuples, columns = EVERY n-subset of the 12 source indices, no source list: wick_block_tensor evaluates
+//   B[t][S_u][S_d] = sum_x e^{ip.x} sum_i c_i det U_x[a_u(i), S_u] det D_x[a_d(i), S_d].
+extern "C" int wick_build_block_terms(const wick_operator* cluster, wick_terms** out) {
+    if (!cluster || !out || cluster->poly.empty()) { set_error("wick_build_block_terms: NULL or empty operator"); return WICK_ERR_ARG; }
+    *out = nullptr;
+    try {
+        wick_terms* t = new wick_terms();
+        t->n_u = cluster->n_u; t->n_d = cluster->n_d;
+        t->f[0].n = t->n_u; t->f[1].n = t->n_d;
+        std::vector<uint16_t> us, ds;
+        for (const auto& kv : cluster->poly) { us.push_back(uint16_t(kv.first >> 16)); ds.push_back(uint16_t(kv.first & 0xffff)); }
+        t->f[0].rows = distinct_sorted(us); t->f[1].rows = distinct_sorted(ds);
+        t->f[0].cols = all_subsets(t->n_u); t->f[1].cols = all_subsets(t->n_d);
+        const auto iu = index_of(t->f[0].rows), id = index_of(t->f[1].rows);
+        for (const auto& kv : cluster->poly) {
+            FactorTerm ft;
+            ft.qu = iu.at(uint16_t(kv.first >> 16)); ft.qd = id.at(uint16_t(kv.first & 0xffff)); ft.c = kv.second;
+            t->sink.push_back(ft);
+        }
+        std::sort(t->sink.begin(), t->sink.end(), [](const FactorTerm& a, const FactorTerm& b) {
+            return a.qu != b.qu ? a.qu < b.qu : a.qd < b.qd; });
+        t->outer = true;                                       // grid tables; the source list stays empty
+        t->block_mode = true;
+        t->n_terms = 0;
+        grid_minors(t->f[0]);
+        grid_minors(t->f[1]);
+        *out = t;
+        return WICK_OK;
+    } catch (const std::bad_alloc&) { set_error("wick_build_block_terms: out of host memory"); return WICK_ERR_NOMEM; }
+}
+
+// rank of a 12-bit mask among the n-subsets in lexicographic tuple order
+static int subset_index(const std::unordered_map<uint16_t, int32_t>& idx, uint16_t mask) { return idx.at(mask); }
+
+// C[t] = sum_j conj(c_j) sum_{S_u in b_u(j), S_d in b_d(j)} sign B_A[t][S_u][S_d] B_B[t][b_u \ S_u][b_d \ S_d]
+// (generalised Laplace expansion of the two stacked determinants along the rows of cluster A; lattice independent).
+extern "C" int wick_combine_two_clusters(const wick_operator* a, const wick_operator* b, const wick_operator* source,
+                                         const double* BA_reim, const double* BB_reim, int T, double* C_reim) {
+    if (!a || !b || !source || !BA_reim || !BB_reim || !C_reim || T < 1) { set_error("wick_combine_two_clusters: bad argument"); return WICK_ERR_ARG; }
+    if (source->n_u != a->n_u + b->n_u || source->n_d != a->n_d + b->n_d) {
+        set_error("wick_combine_two_clusters: the source operator must have the quark content of A.B"); return WICK_ERR_ARG; }
+    try {
+        const std::vector<uint16_t> cua = all_subsets(a->n_u), cda = all_subsets(a->n_d), cub = all_subsets(b->n_u), cdb = all_subsets(b->n_d);
+        const auto iua = index_of(cua), ida = index_of(cda), iub = index_of(cub), idb = index_of(cdb);
+        const size_t na = cua.size() * cda.size(), nb = cub.size() * cdb.size();
+        // sign of taking the columns S (a subset of the ascending tuple b) for the first k = |S| rows: (-1)^(sum of positions of S + k(k-1)/2)
+        auto laplace_sign = [](uint16_t full, uint16_t sub) {
+            int pos = 0, sum = 0, k = 0;
+            for (int bit = 0; bit < 12; ++bit) if (full & (1u << bit)) { if (sub & (1u << bit)) { sum += pos; ++k; } ++pos; }
+            return ((sum + k * (k - 1) / 2) & 1) ? -1.0 : 1.0;
+        };
+        const double cluster_sign = ((a->n_d * b->n_u) & 1) ? -1.0 : 1.0;      // u_A d_A u_B d_B -> u_A u_B d_A d_B
+        for (int t = 0; t < T; ++t) {
+            const cplx* BA = reinterpret_cast<const cplx*>(BA_reim) + size_t(t) * na;
+            const cplx* BB = reinterpret_cast<const cplx*>(BB_reim) + size_t(t) * nb;
+            long double re = 0.0L, im = 0.0L;
+            for (const auto& kv : source->poly) {
+                const uint16_t bu = uint16_t(kv.first >> 16), bd = uint16_t(kv.first & 0xffff);
+                cplx acc(0.0, 0.0);
+                for (uint16_t su = bu;; su = uint16_t((su - 1) & bu)) {
+                    if (popc(su) == a->n_u) {
+                        const double sgu = laplace_sign(bu, su);
+                        for (uint16_t sd = bd;; sd = uint16_t((sd - 1) & bd)) {
+                            if (popc(sd) == a->n_d)
+                                acc += sgu * laplace_sign(bd, sd) *
+                                       BA[size_t(subset_index(iua, su)) * cda.size() + size_t(subset_index(ida, sd))] *
+                                       BB[size_t(subset_index(iub, uint16_t(bu & ~su))) * cdb.size() + size_t(subset_index(idb, uint16_t(bd & ~sd)))];
+                            if (sd == 0) break;
+                        }
+                    }
+                    if (su == 0) break;
+                }
+                const cplx v = cluster_sign * std::conj(kv.second) * acc;
+                re += v.real(); im += v.imag();
+            }
+            C_reim[2 * t] = double(re); C_reim[2 * t + 1] = double(im);
+        }
+        return WICK_OK;
+    } catch (const std::bad_alloc&) { set_error("wick_combine_two_clusters: out of host memory"); return WICK_ERR_NOMEM; }
+}
+
 extern "C" int wick_terms_get_info(const wick_terms* t, wick_terms_info* info) {
     if (!t || !info) { set_error("wick_terms_get_info: NULL argument"); return WICK_ERR_ARG; }
     info->n_u = t->n_u; info->n_d = t->n_d;

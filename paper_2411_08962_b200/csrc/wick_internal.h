@@ -72,6 +72,8 @@ struct DeviceTables {
     int reg_state[2] = {0, 0};                  // per flavour: 0 = not checked, 1 = register-resident minors kernel usable, -1 = not
     std::map<int, RegDev> reg[2];               // by number of warp bins per site group
     // flat list (uploaded only when the flat path runs)
+    void* block_blob = nullptr;                 // block handles: sink terms as flat arrays (contract.cu: wick_block_tensor)
+    const void *block_c = nullptr, *block_ru = nullptr, *block_rd = nullptr;
     void* jf_blob = nullptr;                    // fused Jacobi path: flat terms with complementary index sets (contract.cu)
     void* flat_blob = nullptr;
     const int32_t* t_uid = nullptr;
@@ -87,6 +89,7 @@ struct wick_terms {
     int n_u = 0, n_d = 0;
     wick::FlavourTables f[2];                   // 0 = u, 1 = d
     bool outer = false;
+    bool block_mode = false;                    // wick_build_block_terms: sink list only, columns = all subsets (wick_block_tensor)
     bool needs_u_equals_d = false;              // built with WICK_BUILD_ISOSPIN and changed by it: only valid for U == D
     std::vector<wick::FactorTerm> sink, source; // outer-product factor lists (source holds conj c_j)
     int64_t n_terms = 0, n_raw = 0, n_identity_merged = 0;

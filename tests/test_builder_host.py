@@ -357,3 +357,40 @@ def test_terms_matrix_shares_one_pair_of_minor_tables():
     ref, sabs = wo.site_value_outer(U, D, sink, src)
     got, _ = wo.site_terms_value(U, D, *m[0][1].term_tuples())
     assert abs(got - ref) <= 1e-12 * sabs
+
+
+# ---------------------------------------------------------------------------------------------
+# cluster sinks: host combination of block tensors (Eq. 6-8)
+# ---------------------------------------------------------------------------------------------
+
+def test_cluster_combination_on_one_site_equals_the_point_sink():
+    """With one lattice site the block tensors are plain sums over sink terms of products of minors (computed here with the
+    oracle's determinant), and the combination must return the point-sink value of the product operator."""
+    import itertools
+    rng = np.random.default_rng(52)
+    U, D = _rand(rng, 12, 12), _rand(rng, 12, 12)
+    a, b = wk.operator_from_nucleons([("p", 0)]), wk.operator_from_nucleons([("n", 1)])
+    ab = wk.operator_product(a, b)
+    assert _as_list(ab) == [(u, d, complex(c)) for u, d, c in wo.merged_terms([("p", 0), ("n", 1)])]
+
+    def block(op):
+        u, d, c = op.terms()
+        cu = np.array(list(itertools.combinations(range(12), op.n_u)), np.intp)
+        cd = np.array(list(itertools.combinations(range(12), op.n_d)), np.intp)
+        B = np.zeros((1, len(cu), len(cd)), complex)
+        for ui, di, ci in zip(u.astype(np.intp), d.astype(np.intp), c):
+            mu = wo.det_elim(U[ui[None, :, None], cu[:, None, :]])
+            md = wo.det_elim(D[di[None, :, None], cd[:, None, :]])
+            B[0] += ci * mu[:, None] * md[None, :]
+        return B
+    got = wk.combine_two_clusters(a, b, ab, block(a), block(b))
+    ref, sabs = wo.site_value_outer(U, D, wo.merged_terms([("p", 0), ("n", 1)]))
+    assert abs(got[0] - ref) <= 1e-12 * sabs
+    # a two-nucleon cluster next to a nucleon (3He as deuteron + proton): same identity
+    a2 = wk.operator_from_nucleons([("p", 0), ("n", 0)])
+    b2 = wk.operator_from_nucleons([("p", 1)])
+    got = wk.combine_two_clusters(a2, b2, wk.operator_product(a2, b2), block(a2), block(b2))
+    ref, sabs = wo.site_value_outer(U, D, wo.merged_terms([("p", 0), ("n", 0), ("p", 1)]))
+    assert abs(got[0] - ref) <= 1e-12 * sabs
+    with pytest.raises(wk.WickError, match="quark content"):
+        wk.combine_two_clusters(a, b, a, block(a), block(b))

@@ -458,3 +458,32 @@ def test_correlation_matrix_shares_the_determinants(cuda_device):
     other = wk.build_terms(CONFIGS["cfg0"].nucleus)
     with pytest.raises(wk.WickError, match="share"):
         wk.contract_many(Ud, Dd, [lists[0], other], mom, L, T)
+
+
+def test_two_cluster_sink_against_the_two_site_oracle(cuda_device):
+    """Cluster sink (plane-wave sink of Eq. 8 for single nucleons): proton at x, neutron at y, each projected to its
+    own momentum, against the oracle's explicit double sum over (x, y) with stacked determinants."""
+    L, T = 2, 2
+    U, D = make_propagators_numpy(8642, L, T)
+    Ud, Dd = _dev(U, cuda_device), _dev(D, cuda_device)
+    a, b = wk.operator_from_nucleons([("p", 0)]), wk.operator_from_nucleons([("n", 0)])
+    sa, sb, src = wo.merged_terms([("p", 0)]), wo.merged_terms([("n", 0)]), wo.merged_terms([("p", 0), ("n", 0)])
+    for mom_a, mom_b in (((0, 0, 0), (0, 0, 0)), ((1, 0, 0), (1, 1, 0))):
+        Cg = wk.two_cluster_correlator(Ud, Dd, a, b, mom_a, mom_b, L, T)
+        Cr, sabs = wo.two_cluster_correlator(U, D, sa, sb, src, mom_a, mom_b, L)
+        assert np.all(np.abs(Cg - Cr) <= REL_TOL * sabs), (np.abs(Cg - Cr) / sabs).max()
+    # the block tensor itself on a ragged lattice: one entry against the oracle's minors
+    L3 = 3
+    U3, D3 = make_propagators_numpy(8643, L3, 1)
+    B = wk.block_tensor(_dev(U3, cuda_device), _dev(D3, cuda_device), wk.build_block_terms(a), (0, 1, 2), L3, 1).cpu().numpy()
+    import itertools
+    cu = list(itertools.combinations(range(12), 2))
+    ph = wo.momentum_phases(L3, [(0, 1, 2)])[0]
+    for (iu, idd) in ((0, 0), (17, 5), (65, 11)):
+        ref, ref_abs = 0.0, 0.0
+        for x in range(L3 ** 3):
+            for (ua, da, ca) in sa:
+                v = ca * wo.det_elim(U3[0, x][np.ix_(ua, cu[iu])]) * D3[0, x][da[0], idd] * ph[x]
+                ref += v
+                ref_abs += abs(v)
+        assert abs(B[0, iu, idd] - ref) <= REL_TOL * ref_abs

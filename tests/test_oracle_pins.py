@@ -391,3 +391,38 @@ def test_deuteron_eq20_against_the_pairing_sum():
     part, _ = wo.site_value_outer(U, D, part_sink, sink)
     assert abs(vals - part) <= 1e-11 * sabs
     assert abs(full) > 0
+
+
+def test_two_cluster_value_reduces_to_the_point_sink_and_to_the_pairing_sum():
+    """Cluster sinks: with both clusters at the SAME site the two-cluster value is the point-sink value of the
+    product operator (a pinned function); with different sites it equals the explicit sum over all pairings (Eq. 11,
+    PAPER.md:159) in which every sink quark takes its propagator row from its own cluster's site."""
+    rng = np.random.default_rng(77)
+    Ux, Dx, Uy, Dy = (rng.standard_normal((12, 12)) + 1j * rng.standard_normal((12, 12)) for _ in range(4))
+    p, n = wo.merged_terms([("p", 0)]), wo.merged_terms([("n", 0)])
+    pn = wo.merged_terms([("p", 0), ("n", 0)])
+    same, sabs = wo.two_cluster_site_pair_value(Ux, Dx, Ux, Dx, p, n, pn)
+    ref, _ = wo.site_value_outer(Ux, Dx, pn)
+    assert abs(same - ref) <= 1e-12 * sabs
+    # different sites: RAW proton x RAW neutron at the sink, RAW product at the source, Leibniz sum with per-quark sites
+    raw_p, raw_n = wo.nucleon_raw_terms("p", 0), wo.nucleon_raw_terms("n", 0)
+    raw_src = wo.nucleus_raw_terms([("p", 0), ("n", 0)])
+    got, sabs = wo.two_cluster_site_pair_value(Ux, Dx, Uy, Dy, p, n, pn)
+    tot = 0.0
+    src = raw_src[::23]                                         # slices: the sum is linear in each of the three lists
+    raw_p, raw_n = raw_p[::2], raw_n[1::3]
+    for ca, qa in raw_p:
+        for cb, qb in raw_n:
+            sink_q = qa + qb
+            where = [0] * len(qa) + [1] * len(qb)
+            for cj, qj in src:
+                M = np.zeros((6, 6), complex)
+                for i, (fi, ci) in enumerate(sink_q):
+                    for j, (fj, cjx) in enumerate(qj):
+                        if fi == fj:
+                            P = ((Ux, Uy) if fi == "u" else (Dx, Dy))[where[i]]
+                            M[i, j] = P[ci, cjx]
+                tot += ca * cb * np.conj(cj) * wo.det_leibniz(M)
+    part, _ = wo.two_cluster_site_pair_value(Ux, Dx, Uy, Dy, wo.merged_from_raw(raw_p), wo.merged_from_raw(raw_n), wo.merged_from_raw(src))
+    assert abs(tot - part) <= 1e-11 * sabs
+    assert abs(got) > 0
