@@ -1069,23 +1069,35 @@ cudaError_t launch_reduce_outer(const double2* MU, const double2* MD, int n_grou
 // ---------------------------------------------------------------------------------------------
 // a6: sigma = fixed-order sum of the chunk partials; C(t,p) = sum_x e^{ip.x} sigma(x,t), fixed tree
 // ---------------------------------------------------------------------------------------------
-__global__ void finalize_sigma_kernel(const c128* __restrict__ partial, int n_chunks, int S_b, int64_t n_valid,
-                                      c128* __restrict__ sigma_batch, const c128* __restrict__ scale_a, const c128* __restrict__ scale_b) {
-    const int64_t s = int64_t(blockIdx.x) * blockDim.x + threadIdx.x;
-    if (s >= n_valid) return;
-    c128 acc = partial[s];
-    for (int c = 1; c < n_chunks; ++c) acc = cadd(acc, partial[int64_t(c) * S_b + s]);
-    if (scale_a) acc = cmul(acc, scale_a[s]);                   // Jacobi path: the common factor det U (det D) of every term of the site
-    if (scale_b) acc = cmul(acc, scale_b[s]);
-    sigma_batch[s] = acc;
+// 32 sites x 8 slices of the chunk range per CTA: thread (site, k) sums the chunks k, k + 8, ... in order, then the 8 partial
+// sums are added in order k = 0..7 (fixed shape: bit-reproducible)
+constexpr int FIN_SLICES = 8;
+
+__global__ void __launch_bounds__(32 * FIN_SLICES)
+finalize_sigma_kernel(const c128* __restrict__ partial, int n_chunks, int S_b, int64_t n_valid,
+                      c128* __restrict__ sigma_batch, const c128* __restrict__ scale_a, const c128* __restrict__ scale_b) {
+    __shared__ c128 sm[FIN_SLICES][32];
+    const int lane = threadIdx.x & 31, k = threadIdx.x >> 5;
+    const int64_t s = int64_t(blockIdx.x) * 32 + lane;
+    c128 acc = make_double2(0.0, 0.0);
+    if (s < n_valid)
+        for (int c = k; c < n_chunks; c += FIN_SLICES) acc = cadd(acc, partial[int64_t(c) * S_b + s]);
+    sm[k][lane] = acc;
+    __syncthreads();
+    if (k == 0 && s < n_valid) {
+#pragma unroll
+        for (int j = 1; j < FIN_SLICES; ++j) acc = cadd(acc, sm[j][lane]);
+        if (scale_a) acc = cmul(acc, scale_a[s]);               // Jacobi path: the common factor det U (det D) of every term of the site
+        if (scale_b) acc = cmul(acc, scale_b[s]);
+        sigma_batch[s] = acc;
+    }
 }
 
 cudaError_t launch_finalize_sigma(const double2* partial, int n_chunks, int S_b, int64_t n_valid,
                                   double2* sigma_batch, const double2* scale_a, const double2* scale_b, cudaStream_t stream) {
     if (n_valid <= 0) return cudaSuccess;
-    const int threads = 128;
     ProfScope prof(PROF_PROJECT, stream);
-    finalize_sigma_kernel<<<unsigned((n_valid + threads - 1) / threads), threads, 0, stream>>>(partial, n_chunks, S_b, n_valid, sigma_batch, scale_a, scale_b);
+    finalize_sigma_kernel<<<unsigned((n_valid + 31) / 32), 32 * FIN_SLICES, 0, stream>>>(partial, n_chunks, S_b, n_valid, sigma_batch, scale_a, scale_b);
     ++g_launches;
     return cudaGetLastError();
 }
