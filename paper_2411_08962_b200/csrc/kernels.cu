@@ -206,82 +206,99 @@ __device__ __forceinline__ double shfl16(double v, int src) { return __shfl_sync
 // column k (first wins); every lane then does  own[c] -= g * pivot_row[c]  with g = own[k] / piv (the pivot lane itself with
 // g = 1 - 1/piv, which scales it by 1/piv), and column k is replaced by the column of the inverse.  With p_k the pivot
 // lane of step k the lane p_i ends up holding (A^-1)[i][p_m] in register m.
-// Result of invert12 for one lane: row `my_step` of the inverse, entry m belongs to column p_m (4-bit fields of perm).
+// Result of invert12 for one lane and one matrix: row `my_step` of the inverse, entry m belongs to column p_m (4-bit fields of perm).
 struct InvRow { double re[12], im[12]; int my_step; unsigned long long perm; c128 det; bool singular; };
 
-// `bc`: 12 complex of shared memory per site, through which the pivot row of a step reaches the other lanes (one broadcast
-// LDS.128 per entry instead of four shuffles)
-__device__ __forceinline__ void invert12(const c128* __restrict__ P, int64_t st, bool row_ok, int sub, c128* bc, InvRow& R) {
-    double (&re)[12] = R.re;
-    double (&im)[12] = R.im;
+// NM matrices (the two flavours) are inverted TOGETHER: their pivot steps are independent instruction streams, which
+// doubles the work a thread has in flight between the dependent shuffle -> broadcast -> update stages of a step.
+// `bc`: NM x 12 complex of shared memory per site, through which the pivot rows of a step reach the other lanes (one
+// broadcast LDS.128 per entry instead of four shuffles).
+template <int NM>
+__device__ __forceinline__ void invert12(const c128* const (&P)[NM], int64_t st, bool row_ok, int sub, c128* bc, InvRow (&R)[NM]) {
 #pragma unroll
-    for (int c = 0; c < 12; ++c) {
-        c128 v = make_double2(0.0, 0.0);
-        if (row_ok) v = __ldg(P + st * 144 + sub * 12 + c);
-        re[c] = v.x; im[c] = v.y;
-    }
-    bool used = sub >= 12;                                                  // idle lanes never become pivots
-    int my_step = 0;                                                        // the step at which this lane was the pivot row
-    unsigned long long perm = 0;                                            // p_k, 4 bits each (the same on all lanes of a site)
-    c128 det = make_double2(1.0, 0.0);
-    bool singular = false;
-#pragma unroll
-    for (int k = 0; k < 12; ++k) {
-        // argmax of the pivot key over the 16 lanes of the site, smaller lane wins ties
-        int key = used ? -1 : pivot_key(re[k], im[k]);
-        int who = sub;
-#pragma unroll
-        for (int off = 8; off > 0; off >>= 1) {
-            const int k2 = __shfl_xor_sync(0xffffffffu, key, off, 16), w2 = __shfl_xor_sync(0xffffffffu, who, off, 16);
-            if (k2 > key || (k2 == key && w2 < who)) { key = k2; who = w2; }
-        }
-        const int p = who;
-        perm |= (unsigned long long)p << (4 * k);
-        const bool is_p = (sub == p);
-        if (is_p) { used = true; my_step = k; }
-        double pr[12], pi[12];
-        __syncwarp();                                                       // the previous step's reads of bc are done
-        if (is_p) {
-#pragma unroll
-            for (int c = 0; c < 12; ++c) bc[c] = make_double2(re[c], im[c]);
-        }
-        __syncwarp();
-#pragma unroll
-        for (int c = 0; c < 12; ++c) { const c128 v = bc[c]; pr[c] = v.x; pi[c] = v.y; }
-        const c128 piv = make_double2(pr[k], pi[k]);
-        singular = singular || (piv.x == 0.0 && piv.y == 0.0);
-        det = cmul(det, piv);
-        const c128 ip = crecip(piv);
-        // g = own[k] / piv for the other rows, 1 - 1/piv for the pivot row
-        c128 g = cmul(make_double2(re[k], im[k]), ip);
-        if (is_p) g = make_double2(1.0 - ip.x, -ip.y);
+    for (int q = 0; q < NM; ++q) {
 #pragma unroll
         for (int c = 0; c < 12; ++c) {
-            if (c == k) continue;
-            re[c] = fma(-g.x, pr[c], fma(g.y, pi[c], re[c]));
-            im[c] = fma(-g.x, pi[c], fma(-g.y, pr[c], im[c]));
+            c128 v = make_double2(0.0, 0.0);
+            if (row_ok) v = __ldg(P[q] + st * 144 + sub * 12 + c);
+            R[q].re[c] = v.x; R[q].im[c] = v.y;
         }
-        re[k] = is_p ? ip.x : -g.x;
-        im[k] = is_p ? ip.y : -g.y;
+        R[q].my_step = 0; R[q].perm = 0; R[q].det = make_double2(1.0, 0.0); R[q].singular = false;
     }
-    // sign of the permutation k -> p_k
-    int inv_count = 0;
+    bool used[NM];                                                          // idle lanes never become pivots
 #pragma unroll
-    for (int a = 0; a < 12; ++a)
+    for (int q = 0; q < NM; ++q) used[q] = sub >= 12;
 #pragma unroll
-        for (int b = a + 1; b < 12; ++b) inv_count += (int(perm >> (4 * a)) & 15) > (int(perm >> (4 * b)) & 15);
-    if (inv_count & 1) { det.x = -det.x; det.y = -det.y; }
-    if (singular) det = make_double2(0.0, 0.0);
-    R.my_step = my_step; R.perm = perm; R.det = det; R.singular = singular;
+    for (int k = 0; k < 12; ++k) {
+        int p[NM];
+        bool is_p[NM];
+#pragma unroll
+        for (int q = 0; q < NM; ++q) {
+            // argmax of the pivot key over the 16 lanes of the site, smaller lane wins ties
+            int key = used[q] ? -1 : pivot_key(R[q].re[k], R[q].im[k]);
+            int who = sub;
+#pragma unroll
+            for (int off = 8; off > 0; off >>= 1) {
+                const int k2 = __shfl_xor_sync(0xffffffffu, key, off, 16), w2 = __shfl_xor_sync(0xffffffffu, who, off, 16);
+                if (k2 > key || (k2 == key && w2 < who)) { key = k2; who = w2; }
+            }
+            p[q] = who;
+            R[q].perm |= (unsigned long long)who << (4 * k);
+            is_p[q] = (sub == who);
+            if (is_p[q]) { used[q] = true; R[q].my_step = k; }
+        }
+        __syncwarp();                                                       // the previous step's reads of bc are done
+#pragma unroll
+        for (int q = 0; q < NM; ++q)
+            if (is_p[q]) {
+#pragma unroll
+                for (int c = 0; c < 12; ++c) bc[q * 12 + c] = make_double2(R[q].re[c], R[q].im[c]);
+            }
+        __syncwarp();
+#pragma unroll
+        for (int q = 0; q < NM; ++q) {
+            double (&re)[12] = R[q].re;
+            double (&im)[12] = R[q].im;
+            double pr[12], pi[12];
+#pragma unroll
+            for (int c = 0; c < 12; ++c) { const c128 v = bc[q * 12 + c]; pr[c] = v.x; pi[c] = v.y; }
+            const c128 piv = make_double2(pr[k], pi[k]);
+            R[q].singular = R[q].singular || (piv.x == 0.0 && piv.y == 0.0);
+            R[q].det = cmul(R[q].det, piv);
+            const c128 ip = crecip(piv);
+            // g = own[k] / piv for the other rows, 1 - 1/piv for the pivot row (which scales it by 1/piv)
+            c128 g = cmul(make_double2(re[k], im[k]), ip);
+            if (is_p[q]) g = make_double2(1.0 - ip.x, -ip.y);
+#pragma unroll
+            for (int c = 0; c < 12; ++c) {
+                if (c == k) continue;
+                re[c] = fma(-g.x, pr[c], fma(g.y, pi[c], re[c]));
+                im[c] = fma(-g.x, pi[c], fma(-g.y, pr[c], im[c]));
+            }
+            re[k] = is_p[q] ? ip.x : -g.x;
+            im[k] = is_p[q] ? ip.y : -g.y;
+        }
+    }
+#pragma unroll
+    for (int q = 0; q < NM; ++q) {
+        // sign of the permutation k -> p_k
+        int inv_count = 0;
+#pragma unroll
+        for (int a = 0; a < 12; ++a)
+#pragma unroll
+            for (int b = a + 1; b < 12; ++b) inv_count += (int(R[q].perm >> (4 * a)) & 15) > (int(R[q].perm >> (4 * b)) & 15);
+        if (inv_count & 1) { R[q].det.x = -R[q].det.x; R[q].det.y = -R[q].det.y; }
+        if (R[q].singular) R[q].det = make_double2(0.0, 0.0);
+    }
 }
 
-// store the lane's row of the inverse into a [12][12] matrix (global or shared)
-__device__ __forceinline__ void store_inv_row(const InvRow& R, c128* dst_matrix) {
-    c128* dst = dst_matrix + R.my_step * 12;
+// store the lane's row of the inverse into a matrix whose element (r, c) sits at dst[(12 r + c) * stride]
+__device__ __forceinline__ void store_inv_row(const InvRow& R, c128* dst_matrix, int stride) {
+    c128* dst = dst_matrix + R.my_step * 12 * stride;
 #pragma unroll
     for (int m = 0; m < 12; ++m) {
         const int col = int(R.perm >> (4 * m)) & 15;
-        dst[col] = R.singular ? make_double2(0.0, 0.0) : make_double2(R.re[m], R.im[m]);
+        dst[col * stride] = R.singular ? make_double2(0.0, 0.0) : make_double2(R.re[m], R.im[m]);
     }
 }
 
@@ -293,10 +310,11 @@ inverse12_kernel(const c128* __restrict__ P, int64_t st0, int64_t n_st_total, in
     const bool live = site < n_batch && st < n_st_total;
     const bool row_ok = live && sub < 12;
     __shared__ __align__(16) c128 bcast[INV_THREADS / 16][12];
-    InvRow R;
-    invert12(P, st, row_ok, sub, bcast[threadIdx.x >> 4], R);
-    if (live && sub == 0) det_out[site] = R.det;
-    if (row_ok) store_inv_row(R, inv_out + site * 144);
+    InvRow R[1];
+    const c128* const Pq[1] = {P};
+    invert12<1>(Pq, st, row_ok, sub, bcast[threadIdx.x >> 4], R);
+    if (live && sub == 0) det_out[site] = R[0].det;
+    if (row_ok) store_inv_row(R[0], inv_out + site * 144, 1);
 }
 
 // Fused Jacobi path for lists whose BOTH flavours have 8 <= n <= 11 and whose term count is of the order of the number of
@@ -306,6 +324,8 @@ inverse12_kernel(const c128* __restrict__ P, int64_t st0, int64_t n_st_total, in
 // Nothing but the propagators is read from and sigma written to global memory: 4608 B per site-time.
 constexpr int JF_SITES = INV_THREADS / 16;
 
+// A: element (r, c) of the site's inverse at A[(12 r + c) * JF_SITES] (site-minor layout: the 8 sites of a quarter warp
+// read one 128-byte row, conflict free)
 template <int M>
 __device__ __forceinline__ c128 small_minor(const c128* A, uint32_t idx) {   // rows = nibbles 0..3, columns = nibbles 4..7 of idx
     if constexpr (M == 0) return make_double2(1.0, 0.0);
@@ -313,7 +333,7 @@ __device__ __forceinline__ c128 small_minor(const c128* A, uint32_t idx) {   // 
         int r[M], c[M];
 #pragma unroll
         for (int i = 0; i < M; ++i) { r[i] = int(idx >> (4 * i)) & 15; c[i] = int(idx >> (16 + 4 * i)) & 15; }
-        auto a = [&](int i, int j) { return A[r[i] * 12 + c[j]]; };
+        auto a = [&](int i, int j) { return A[(r[i] * 12 + c[j]) * JF_SITES]; };
         if constexpr (M == 1) return a(0, 0);
         else if constexpr (M == 2) return det2(a(0, 0), a(0, 1), a(1, 0), a(1, 1));
         else if constexpr (M == 3) {
@@ -333,43 +353,53 @@ __device__ __forceinline__ c128 small_minor(const c128* A, uint32_t idx) {   // 
 }
 
 template <int MU_, int MD_>
-__global__ void __launch_bounds__(INV_THREADS, 4)
+__global__ void __launch_bounds__(INV_THREADS, 3)
 jacobi_fused_kernel(const c128* __restrict__ U, const c128* __restrict__ D, bool same, int64_t st0, int64_t n_valid,
                     const JacobiTerm* __restrict__ terms, int n_terms, c128* __restrict__ sigma) {
-    __shared__ __align__(16) c128 inv_s[JF_SITES][2][144];
-    const int sub = threadIdx.x & 15, ls = threadIdx.x >> 4;
-    const int64_t site = int64_t(blockIdx.x) * JF_SITES + ls;
-    const bool live = site < n_valid;
-    const bool row_ok = live && sub < 12;
-    __shared__ __align__(16) c128 bcast[JF_SITES][12];
-    c128 dets;
-    {
-        InvRow R;
-        invert12(U, st0 + site, row_ok, sub, bcast[ls], R);
-        if (row_ok) store_inv_row(R, inv_s[ls][0]);
-        dets = R.det;
-        if (!same) {
-            invert12(D, st0 + site, row_ok, sub, bcast[ls], R);
-            if (row_ok) store_inv_row(R, inv_s[ls][1]);
-            dets = cmul(dets, R.det);
-        } else dets = cmul(dets, dets);
+    __shared__ __align__(16) c128 inv_s[2][144][JF_SITES];                  // [flavour][element][site]
+    __shared__ __align__(16) c128 bcast[JF_SITES][2 * 12];
+    __shared__ __align__(16) c128 psum[INV_THREADS / JF_SITES][JF_SITES];
+    __shared__ c128 dets_s[JF_SITES];
+    {   // phase 1: 16 lanes per site invert both propagators
+        const int sub = threadIdx.x & 15, ls = threadIdx.x >> 4;
+        const int64_t site = int64_t(blockIdx.x) * JF_SITES + ls;
+        const bool row_ok = site < n_valid && sub < 12;
+        c128 dets;
+        if (same) {
+            InvRow R[1];
+            const c128* const Pq[1] = {U};
+            invert12<1>(Pq, st0 + site, row_ok, sub, bcast[ls], R);
+            if (row_ok) store_inv_row(R[0], &inv_s[0][0][ls], JF_SITES);
+            dets = cmul(R[0].det, R[0].det);
+        } else {
+            InvRow R[2];
+            const c128* const Pq[2] = {U, D};
+            invert12<2>(Pq, st0 + site, row_ok, sub, bcast[ls], R);
+            if (row_ok) { store_inv_row(R[0], &inv_s[0][0][ls], JF_SITES); store_inv_row(R[1], &inv_s[1][0][ls], JF_SITES); }
+            dets = cmul(R[0].det, R[1].det);
+        }
+        if (sub == 0) dets_s[ls] = dets;
     }
-    __syncwarp();
-    const c128* Ui = inv_s[ls][0];
-    const c128* Di = same ? inv_s[ls][0] : inv_s[ls][1];
+    __syncthreads();
+    // phase 2: lane = (site, one of 16 term slots); a quarter warp = the 8 sites of one term
+    const int ls = threadIdx.x & (JF_SITES - 1), slot = threadIdx.x / JF_SITES;
+    const c128* Ui = &inv_s[0][0][ls];
+    const c128* Di = same ? Ui : &inv_s[1][0][ls];
     c128 acc = make_double2(0.0, 0.0);
-    for (int k = sub; k < n_terms; k += 16) {
+    for (int k = slot; k < n_terms; k += INV_THREADS / JF_SITES) {
         const uint4 h = __ldg(reinterpret_cast<const uint4*>(terms + k));
         const c128 w = __ldg(reinterpret_cast<const c128*>(terms + k) + 1);
         acc = cfma(cmul(w, small_minor<MU_>(Ui, h.x)), small_minor<MD_>(Di, h.y), acc);
     }
-    // fixed-shape tree over the 16 lanes of the site
+    psum[slot][ls] = acc;
+    __syncthreads();
+    if (threadIdx.x < JF_SITES) {                                           // fixed-order sum over the term slots
+        const int64_t site = int64_t(blockIdx.x) * JF_SITES + threadIdx.x;
+        c128 t = psum[0][threadIdx.x];
 #pragma unroll
-    for (int off = 8; off > 0; off >>= 1) {
-        acc.x += __shfl_xor_sync(0xffffffffu, acc.x, off, 16);
-        acc.y += __shfl_xor_sync(0xffffffffu, acc.y, off, 16);
+        for (int j = 1; j < INV_THREADS / JF_SITES; ++j) t = cadd(t, psum[j][threadIdx.x]);
+        if (site < n_valid) sigma[site] = cmul(t, dets_s[threadIdx.x]);
     }
-    if (live && sub == 0) sigma[site] = cmul(acc, dets);
 }
 
 template <int MU_>
