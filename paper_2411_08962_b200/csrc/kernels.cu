@@ -27,7 +27,13 @@ int64_t launch_counter_reset() { const int64_t v = g_launches; g_launches = 0; r
 struct ProfRec { cudaEvent_t a, b; int cls; };
 static thread_local bool g_prof_on = false;
 static thread_local std::vector<ProfRec> g_prof;
-void profile_enable(bool on) { g_prof_on = on; }
+void profile_enable(bool on) {
+    g_prof_on = on;
+    if (!on) {                                                   // records never read are dropped with their events
+        for (ProfRec& r : g_prof) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
+        g_prof.clear();
+    }
+}
 struct ProfScope {
     ProfRec r; cudaStream_t s; bool on;
     ProfScope(int cls, cudaStream_t stream) : s(stream), on(g_prof_on) {

@@ -1,16 +1,16 @@
-// a4 for "grid" minor tables (every row tuple x every column tuple, i.e. outer-product term lists), N = 5, 6:
-// register-resident instance kernel.
+// a4 for "grid" minor tables (every row tuple x every column tuple, i.e. outer-product term lists), N = 6: the instance kernel.
 //
-// A job = (row tuple, instance) where an instance is a set of K = N-4 leading columns shared by many column
-// tuples.  After the K pivot steps of the instance (left-looking LU with partial pivoting, lu_device.cuh) every
-// minor of the instance is  detp * det4(S[:, b_K], S[:, b_K+1], S[:, b_K+2], S[:, b_K+3])  with S the 4-row Schur
-// complement; its columns are needed for the NC <= 10 (11) "candidate" column indices that occur behind the
-// leading ones.  The thread computes all candidate Schur columns ONCE into registers (4 complex each) and then
-// walks the trie of 4-subsets of candidate POSITIONS with fully unrolled code, so every register index is
-// static: 2x2 minors of (i2, i3), signed 3x3 minors of (i2, i3, i4), Laplace sum with i5.  Which pairs, triples
-// and quadruples exist is a bit mask per instance (built on the host from the column tuples; warp uniform, so
-// every test is a uniform branch).  No per-thread shared-memory cache: shared memory holds the propagator tile
-// only, and levels 1-3 touch no memory but the result store.
+// A job = (row tuple, instance) where an instance is a set of K = N-4 leading columns shared by many column tuples.  After
+// the K pivot steps of the instance (left-looking LU with partial pivoting, lu_device.cuh) every minor of the instance is
+//   detp * det4(S[:, b_K], S[:, b_K+1], S[:, b_K+2], S[:, b_K+3])
+// with S the 4-row Schur complement; its columns are needed for the NC <= 10 "candidate" column indices that occur behind the
+// leading ones.  The thread computes all candidate Schur columns ONCE: into registers (4 complex each; the LAST level of the
+// trie is fully unrolled over the candidate positions, so its register indices are static and it touches no memory but the
+// result store) and into a per-thread shared-memory copy (positions 0 .. NC-2, for the pair and third levels, which fetch
+// their columns by dynamic index).  The trie of the instance's column tuples over candidate POSITIONS is a word program built
+// on the host (contract.cu: build_reg_host): it is the same for every row tuple, because an outer-product list pairs every
+// row tuple with the same column tuples.  Everything that steers a job is warp uniform (the warp index is taken through a
+// shuffle so that the compiler knows), so every test is a uniform branch.
 //
 // PAPER.md:203 ("analytic up to 4x4, LU above") and R.2 (:226, nothing is evaluated twice) one level below the
 // unique-minor table: every minor is still the pivoted LU of its own matrix, identical leading work is shared.
