@@ -36,6 +36,48 @@ def _worker(rank, world, port, T, n_mom, q):
         dist.destroy_process_group()
 
 
+def _sharded_worker(rank, world, port, T, n_mom, q):
+    """contract_sharded end to end with the device call replaced by a stand-in that returns, for the rank's local
+    timeslices, rows that encode WHICH global timeslice they belong to: checks the split, the order of the local rows and
+    the gather as bench.py --gpus N uses them (the real device call needs a GPU and is covered by the gpu tests)."""
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        from paper_2411_08962_b200 import binding, sharding
+        mine = timeslices_of_rank(T, rank, world)
+        full = _full(n_mom, T)
+        U_local = torch.tensor(mine, dtype=torch.float64).reshape(-1, 1, 1, 1)      # "propagators": the timeslice index itself
+
+        def fake_contract(U, D, terms, momenta, L, T_local, **kw):
+            assert T_local == U.shape[0] == len(mine) and kw == {"workspace": None}
+            ts = U.reshape(-1).to(torch.long)
+            return full[:, ts].contiguous()
+        binding.contract, saved = fake_contract, binding.contract
+        try:
+            got = sharding.contract_sharded(U_local, U_local, None, [(0, 0, 0)] * n_mom, 1, T, workspace=None)
+        finally:
+            binding.contract = saved
+        q.put((rank, bool(torch.equal(got, full))))
+    finally:
+        dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("world,T", [(2, 8), (3, 7), (2, 1)])
+def test_contract_sharded_plumbing_gloo(world, T):
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_sharded_worker, args=(r, world, port, T, 2, q)) for r in range(world)]
+    for p in procs:
+        p.start()
+    results = [q.get(timeout=120) for _ in range(world)]
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    assert sorted(results) == [(r, True) for r in range(world)]
+
+
 def test_timeslices_of_rank_partition():
     for T in (0, 1, 5, 8, 64):
         for world in (1, 2, 3, 8):
