@@ -233,8 +233,10 @@ int wick_contract_many(const void* U_dev, const void* D_dev, const wick_terms* c
 
 /* Same computation from HOST buffers (U_host, D_host, C_out_host, sigma_out_host: host memory,
  * pinned or pageable, same layouts).  Allocates device memory itself, streams the propagators
- * timeslice block by timeslice block (H2D overlapped with compute), copies C back
- * and synchronises before returning. */
+ * timeslice block by timeslice block (blocks of <= 256 MB per flavour; H2D of block b+1 on a second stream while block b
+ * computes), copies C back and synchronises before returning; on an error both streams are drained first.
+ * U_host == D_host is legal (one propagator, copied once, U_dev == D_dev on the device).  Test hook: the environment
+ * variable WICK_HOST_BLOCK_BYTES overrides the block size so that the multi-block path can be exercised on small lattices. */
 int wick_contract_host(const void* U_host, const void* D_host, const wick_terms* terms,
                        const int32_t* momenta, int n_mom, int L, int T,
                        void* C_out_host, void* sigma_out_host, unsigned flags);
