@@ -984,7 +984,7 @@ int contract_lists(const void* U_dev, const void* D_dev, const wick_terms* const
         const int64_t n_valid = std::min<int64_t>(S_b, p.n_st - st0);
         const int n_groups = int((n_valid + GROUP - 1) / GROUP);
         // grid tables of 6x6 minors: register-resident instance kernel, one wave of CTAs (8 warp bins each)
-        const int reg_bins = std::max(1, (148 + n_groups - 1) / n_groups) * (REG_THREADS / 32);
+        const int reg_bins = std::max(1, 148 / n_groups) * (REG_THREADS / 32);   // floor: the grid must not spill into a second wave
         for (int f = 0; f < (shared_minors ? 1 : 2); ++f) {
             const int n = f == 0 ? t->n_u : t->n_d;
             const double2* Pf = f == 0 ? U : D;
@@ -1126,7 +1126,7 @@ extern "C" int wick_block_tensor(const void* U_dev, const void* D_dev, const wic
         for (int64_t s0 = 0; s0 < V; s0 += S_b) {
             const int64_t n_valid = std::min<int64_t>(S_b, V - s0);
             const int n_groups = int((n_valid + GROUP - 1) / GROUP);
-            const int reg_bins = std::max(1, (148 + n_groups - 1) / n_groups) * (REG_THREADS / 32);
+            const int reg_bins = std::max(1, 148 / n_groups) * (REG_THREADS / 32);   // floor: the grid must not spill into a second wave
             for (int f = 0; f < 2; ++f) {
                 RegTables rt;
                 rc = try_reg ? ensure_reg(t, f, reg_bins, stream, &rt) : 0;
@@ -1158,7 +1158,7 @@ extern "C" int wick_terms_minor_table(const void* P_dev, int64_t n_sites, const 
     const FlavourTables& ft = t->f[flavour];
     const int n_groups = int((n_sites + GROUP - 1) / GROUP);
     const int S_b = n_groups * GROUP;
-    const int reg_bins = std::max(1, (148 + n_groups - 1) / n_groups) * (REG_THREADS / 32);
+    const int reg_bins = std::max(1, 148 / n_groups) * (REG_THREADS / 32);   // floor: the grid must not spill into a second wave
     RegTables rt;
     rc = (t->outer && !(flags & WICK_CONTRACT_NO_REG_MINORS)) ? ensure_reg(t, flavour, reg_bins, stream, &rt) : 0;
     if (rc < 0) return rc;
