@@ -394,3 +394,33 @@ def test_cluster_combination_on_one_site_equals_the_point_sink():
     assert abs(got[0] - ref) <= 1e-12 * sabs
     with pytest.raises(wk.WickError, match="quark content"):
         wk.combine_two_clusters(a, b, a, block(a), block(b))
+
+
+# ---------------------------------------------------------------------------------------------
+# measurement helpers of bench.py (host logic only)
+# ---------------------------------------------------------------------------------------------
+
+def test_bench_executed_flop_model_and_traffic_key(tmp_path, monkeypatch):
+    import json
+
+    import bench
+    t = wk.build_terms(NUCLEI["cfg3"])
+    ur, uc, dr, dc = t.tuples()
+    mu_row = t.minors()[0]
+    mid, pc, _ = t.minor_order(0)
+    f = bench.executed_flops_per_site(6, mu_row[mid], pc, uc)
+    # per row tuple: 12 instances (two pivot steps each) + 91 Schur columns + 96 pair nodes + 296 third nodes + 655 Laplace sums
+    per_row = 12 * (6 + 14 + 30 + (40 + 5 + 14 + 24 + 6)) + 91 * 72 + 96 * 108 + 296 * 88 + 655 * 30
+    assert f == per_row * 655 and 95 < f / 429025 < 100
+    assert f < 429025 * bench.flops_lu(6) / 6                   # far below one full LU per minor: never report that as a rate
+    # the committed ncu traffic only counts for the kernel sources it was measured on
+    monkeypatch.setattr(bench, "ROOT", str(tmp_path))
+    (tmp_path / "profiles").mkdir()
+    (tmp_path / "paper_2411_08962_b200" / "csrc").mkdir(parents=True)
+    (tmp_path / "paper_2411_08962_b200" / "csrc" / "k.cu").write_text("// kernel\n")
+    rec = {"kernel_source_hash": bench.kernel_source_hash(), "command": "ncu", "workloads": {"x": {"minors_dram_bytes_per_launch": 5}}}
+    (tmp_path / "profiles" / "r02_roofline_traffic.json.txt").write_text(json.dumps(rec))
+    assert bench.read_traffic("x")[0] == {"minors_dram_bytes_per_launch": 5}
+    (tmp_path / "paper_2411_08962_b200" / "csrc" / "k.cu").write_text("// kernel, edited\n")
+    got, why = bench.read_traffic("x")
+    assert got is None and "stale" in why
