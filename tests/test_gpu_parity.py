@@ -365,7 +365,20 @@ def test_isospin_lists_on_the_gpu(cfg, L, T, cuda_device):
     mom = [(0, 0, 0), (1, 0, 1)]
     U, Dother = make_propagators_numpy(c.seed, L, T)
     Ud = _dev(U, cuda_device)
-    Cr, sr, sabs = _oracle_lattice(cfg, U, U, mom, L)
+    if cfg == "cfg3":
+        # 18 s per site with two fresh determinants per term: that oracle on two sites, and on every site the oracle's method B
+        # (each distinct minor once, pinned to method A in tests/test_oracle_pins.py)
+        sink = wo.merged_terms(c.nucleus)
+        sr, sabs = np.zeros((T, L ** 3), complex), np.zeros((T, L ** 3))
+        for tt in range(T):
+            for x in range(L ** 3):
+                sr[tt, x], sabs[tt, x] = wo.site_value_method_b(U[tt, x], U[tt, x], sink)
+        for x in (0, L ** 3 - 1):
+            ref, ref_abs = _oracle_site(cfg, U[0, x], U[0, x])
+            assert abs(ref - sr[0, x]) <= 1e-13 * ref_abs
+        Cr = wo.reduce_sites(sr, mom, L)
+    else:
+        Cr, sr, sabs = _oracle_lattice(cfg, U, U, mom, L)
     handles = [wk.build_terms(c.nucleus, flags=wk.BUILD_ISOSPIN)]
     if cfg == "cfg1":
         handles.append(wk.build_terms(c.nucleus, flags=wk.BUILD_IDENTITY_TEST | wk.BUILD_ISOSPIN, seed=9))
