@@ -384,6 +384,8 @@ struct StagedHost {
     std::vector<int32_t> sink_ptr, sink_rdpos, src_ptr, src_cupos, ru_list, rd_list, cu_list, cd_list, bin_ptr;
     std::vector<double> sink_c, src_c;
     std::vector<StagedBatch> batches;
+    std::vector<int32_t> md_ids;                                  // per batch: id of MD[rd][cd], rd-major over its block
+    std::vector<double> b_dense;                                  // per piece: B[cu][cd], row stride = n_cd rounded up to 2 (real schedules)
 };
 
 // Host part of the staged schedule (no CUDA call): also what wick_terms_staged_schedule_check verifies.
@@ -502,7 +504,7 @@ StagedHost build_staged_host(const wick_terms* t, int n_bins, bool force_complex
                     ++kb;
                 }
                 Item it;
-                it.b = StagedBatch{ca, cb, cuA, cuB, rd_ptr[size_t(ka)], rd_ptr[size_t(kb)], ru_ptr[size_t(ka)], ru_ptr[size_t(kb)]};
+                it.b = StagedBatch{ca, cb, cuA, cuB, rd_ptr[size_t(ka)], rd_ptr[size_t(kb)], ru_ptr[size_t(ka)], ru_ptr[size_t(kb)], 0, 0, 0, 0};
                 const int rows = ru_ptr[size_t(kb)] - ru_ptr[size_t(ka)];
                 const int ent = sink_ptr[size_t(ru_ptr[size_t(kb)])] - sink_ptr[size_t(ru_ptr[size_t(ka)])];
                 it.cost = int64_t(n_rd) * n_cd + 16 + int64_t(rows) * ((cuB - cuA) + src_work + 4) + int64_t(ent) * n_cd;
@@ -528,6 +530,32 @@ StagedHost build_staged_host(const wick_terms* t, int n_bins, bool force_complex
     for (int b = 0; b < n_bins; ++b) {
         batches.insert(batches.end(), bins[size_t(b)].begin(), bins[size_t(b)].end());
         bin_ptr[size_t(b) + 1] = int32_t(batches.size());
+    }
+    // flattened prologue data: MD element ids per batch, dense B per piece (shared by the batches of the piece)
+    {
+        std::map<std::pair<int, int>, int32_t> piece_off;           // (cd_a, cu_a) identifies a piece
+        for (StagedBatch& b : batches) {
+            b.md_off = int32_t(h.md_ids.size());
+            for (int rdi = b.rd_a; rdi < b.rd_b; ++rdi)
+                for (int cdi = b.cd_a; cdi < b.cd_b; ++cdi)
+                    h.md_ids.push_back(rd_list[size_t(rdi)] * ncd + cd_list[size_t(cdi)]);
+            b.b_off = 0;
+            if (h.real) {
+                auto it = piece_off.find({b.cd_a, b.cu_a});
+                if (it == piece_off.end()) {
+                    const int n_cd = b.cd_b - b.cd_a, n_cu = b.cu_b - b.cu_a, ncdp = (n_cd + 1) & ~1;
+                    const int32_t off = int32_t(h.b_dense.size());
+                    h.b_dense.resize(h.b_dense.size() + size_t(n_cu) * size_t(ncdp), 0.0);
+                    for (int cdi = 0; cdi < n_cd; ++cdi)
+                        for (int j = src_ptr[size_t(b.cd_a + cdi)]; j < src_ptr[size_t(b.cd_a + cdi) + 1]; ++j)
+                            h.b_dense[size_t(off) + size_t(src_cupos[size_t(j)] - b.cu_a) * size_t(ncdp) + size_t(cdi)] += src_c[2 * size_t(j)];
+                    it = piece_off.emplace(std::make_pair(b.cd_a, b.cu_a), off).first;
+                }
+                b.b_off = it->second;
+            }
+        }
+        if (h.b_dense.empty()) h.b_dense.push_back(0.0);
+        if (h.md_ids.empty()) h.md_ids.push_back(0);
     }
     h.ok = true;
     h.sink_ptr = std::move(sink_ptr); h.sink_rdpos = std::move(sink_rdpos); h.src_ptr = std::move(src_ptr); h.src_cupos = std::move(src_cupos);
@@ -555,6 +583,7 @@ int ensure_staged(const wick_terms* t, int n_bins, bool force_complex, cudaStrea
         out->src_ptr = sd.src_ptr; out->src_cupos = sd.src_cupos; out->src_c = reinterpret_cast<const double2*>(sd.src_c);
         out->ru_list = sd.ru_list; out->rd_list = sd.rd_list; out->cu_list = sd.cu_list; out->cd_list = sd.cd_list;
         out->bin_ptr = sd.bin_ptr; out->batches = static_cast<const StagedBatch*>(sd.batches);
+        out->md_ids = sd.md_ids; out->b_dense = sd.b_dense;
     };
     const int key = 2 * n_bins + (force_complex ? 1 : 0);          // schedules differ: the real-coefficient kernel stages larger MD blocks
     auto hit = d.staged.find(key);
@@ -574,6 +603,7 @@ int ensure_staged(const wick_terms* t, int n_bins, bool force_complex, cudaStrea
     const size_t o_ru = bb.add(ru_list.data(), ru_list.size() * 4), o_rd = bb.add(rd_list.data(), rd_list.size() * 4);
     const size_t o_cu = bb.add(cu_list.data(), cu_list.size() * 4), o_cd = bb.add(cd_list.data(), cd_list.size() * 4);
     const size_t o_bp = bb.add(bin_ptr.data(), bin_ptr.size() * 4), o_ba = bb.add(batches.data(), batches.size() * sizeof(StagedBatch));
+    const size_t o_mi = bb.add(h.md_ids.data(), h.md_ids.size() * 4), o_bd = bb.add(h.b_dense.data(), h.b_dense.size() * 8);
     void* blob = nullptr;
     WICK_CUDA(cudaMalloc(&blob, std::max<size_t>(bb.host.size(), 256)));
     cudaError_t e = cudaMemcpyAsync(blob, bb.host.data(), bb.host.size(), cudaMemcpyHostToDevice, stream);
@@ -588,6 +618,7 @@ int ensure_staged(const wick_terms* t, int n_bins, bool force_complex, cudaStrea
     sd.ru_list = reinterpret_cast<const int32_t*>(b + o_ru); sd.rd_list = reinterpret_cast<const int32_t*>(b + o_rd);
     sd.cu_list = reinterpret_cast<const int32_t*>(b + o_cu); sd.cd_list = reinterpret_cast<const int32_t*>(b + o_cd);
     sd.bin_ptr = reinterpret_cast<const int32_t*>(b + o_bp); sd.batches = b + o_ba;
+    sd.md_ids = reinterpret_cast<const int32_t*>(b + o_mi); sd.b_dense = reinterpret_cast<const double*>(b + o_bd);
     d.staged[key] = sd;
     fill(sd);
     return 1;

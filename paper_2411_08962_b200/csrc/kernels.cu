@@ -992,13 +992,14 @@ reduce_staged_kernel(const c128* __restrict__ MU, const c128* __restrict__ MD, i
     for (int b = b0; b < b1; ++b) {
         const int4 v0 = __ldg(reinterpret_cast<const int4*>(st.batches + b));
         const int4 v1 = __ldg(reinterpret_cast<const int4*>(st.batches + b) + 1);
+        const int4 v2 = __ldg(reinterpret_cast<const int4*>(st.batches + b) + 2);
         const int cd_a = v0.x, n_cd = v0.y - v0.x, cu_a = v0.z, n_cu = v0.w - v0.z;
         const int rd_a = v1.x, n_rd = v1.y - v1.x, ru_a = v1.z, n_rows = v1.w - v1.z;
         __syncthreads();                                                 // every warp is done with the previous batch
-        for (int e = warp; e < n_rd * n_cd; e += STG_W) {
-            const int rdi = e / n_cd, cdi = e - rdi * n_cd;
-            const int id = __ldg(st.rd_list + rd_a + rdi) * st.n_cols_d + __ldg(st.cd_list + cd_a + cdi);
-            cp_async16(MDs + e * GROUP + lane, MDg + int64_t(id) * S_b);
+        {   // MD block: the element ids were laid out on the host (no division, no dependent look-up per element)
+            const int32_t* ids = st.md_ids + v2.x;
+            for (int e = warp; e < n_rd * n_cd; e += STG_W)
+                cp_async16(MDs + e * GROUP + lane, MDg + int64_t(__ldg(ids + e)) * S_b);
         }
         // coefficient lists of the batch -> shared memory, offsets already in elements of the staged buffers
         const int sp0 = __ldg(st.sink_ptr + ru_a), sp1 = __ldg(st.sink_ptr + ru_a + n_rows);
@@ -1015,14 +1016,8 @@ reduce_staged_kernel(const c128* __restrict__ MU, const c128* __restrict__ MD, i
         if constexpr (REAL) {
             // dense B[cu][cd] of the piece (row stride = n_cd rounded up to 2 doubles; zeros where there is no source term)
             const int ncdp = (n_cd + 1) & ~1;
-            for (int e = threadIdx.x; e < n_cu * ncdp; e += STG_THREADS) {
-                const int cul = e / ncdp, cdi = e - cul * ncdp;
-                double v = 0.0;
-                if (cdi < n_cd)
-                    for (int j = __ldg(st.src_ptr + cd_a + cdi); j < __ldg(st.src_ptr + cd_a + cdi + 1); ++j)
-                        if (__ldg(st.src_cupos + j) - cu_a == cul) v += __ldg(st.src_c + j).x;
-                Bd[e] = v;
-            }
+            const double* bsrc = st.b_dense + v2.y;                      // built once per piece on the host
+            for (int e = threadIdx.x; e < n_cu * ncdp; e += STG_THREADS) Bd[e] = __ldg(bsrc + e);
             if (threadIdx.x < n_cu) cuoff[threadIdx.x] = __ldg(st.cu_list + cu_a + threadIdx.x) * S_b;
         } else {
             const int q0 = __ldg(st.src_ptr + cd_a), q1 = __ldg(st.src_ptr + cd_a + n_cd);

@@ -83,7 +83,11 @@ constexpr int STG_SINK_CAP = 512;         // sink entries of a batch's u-row tup
 constexpr int STG_SRC_CAP = 256;          // source entries of a batch piece's d columns
 constexpr int STG_ROWS_CAP = STG_MD_CAP_REAL;  // u-row tuples of a batch
 constexpr int stg_md_cap(bool real) { return real ? STG_MD_CAP_REAL : STG_MD_CAP; }
-struct StagedBatch { int32_t cd_a, cd_b, cu_a, cu_b, rd_a, rd_b, ru_a, ru_b; };
+// md_off: the batch's MD element ids ((rd, cd) pairs of its block, rd-major) in StagedTables::md_ids; b_off: the dense real
+// B[cu][cd] of its piece in StagedTables::b_dense (real-coefficient schedules).  Both are laid out on the host so that the
+// per-batch prologue of the kernel has no dependent look-ups.
+struct StagedBatch { int32_t cd_a, cd_b, cu_a, cu_b, rd_a, rd_b, ru_a, ru_b, md_off, b_off, pad0, pad1; };
+static_assert(sizeof(StagedBatch) == 48, "StagedBatch is read with three 16-byte loads");
 struct StagedTables {
     int n_cols_u, n_cols_d, n_bins;
     bool real_coeffs;                                              // all c_i, cbar_j real: 16-byte {coefficient, offset} entries, 2 DFMA per term
@@ -91,6 +95,7 @@ struct StagedTables {
     const int32_t *src_ptr, *src_cupos; const double2* src_c;      // CSR over POSITION in cd_list: (position of cu in cu_list, conj c_j)
     const int32_t *ru_list, *rd_list, *cu_list, *cd_list;
     const int32_t* bin_ptr; const StagedBatch* batches;            // per CTA bin: its batches, fixed order
+    const int32_t* md_ids; const double* b_dense;                  // per batch / per piece, see StagedBatch
 };
 cudaError_t launch_reduce_staged(const double2* MU, const double2* MD, int n_groups, int S_b, const StagedTables& st,
                                  double2* partial, int* n_chunks_out, cudaStream_t stream);

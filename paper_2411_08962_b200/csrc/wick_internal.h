@@ -35,6 +35,8 @@ struct StagedDev {
     const int32_t *ru_list = nullptr, *rd_list = nullptr, *cu_list = nullptr, *cd_list = nullptr;
     const int32_t* bin_ptr = nullptr;
     const void* batches = nullptr;
+    const int32_t* md_ids = nullptr;            // MD element ids of every batch
+    const double* b_dense = nullptr;            // dense B[cu][cd] of every piece (real-coefficient schedules)
 };
 
 // Job schedule of the register-resident minors kernel for one flavour and bin count (contract.cu: ensure_reg)
