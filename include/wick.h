@@ -249,6 +249,22 @@ int wick_contract_host(const void* U_host, const void* D_host, const wick_terms*
 int wick_minor_dets(const void* P_dev, int64_t n_sites, int n, const uint8_t* rows, const uint8_t* cols,
                     int64_t n_minors, void* out_dev, void* cuda_stream);
 
+/* wick_minor_dets for callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses
+ * that forbid it): same arguments, same kernels, same result, but NOTHING is allocated.  The scratch wick_minor_dets
+ * allocates per call (device copy of the minor descriptors; for n_sites not a multiple of 32 the padded staging buffer of
+ * the results) lives in one static device array of WICK_STATIC_SCRATCH_BYTES that every GPU which loads the library
+ * holds until exit.  Limits: n_minors <= WICK_STATIC_MAX_MINORS per call; if n_sites is not a multiple of 32,
+ * n_minors x 32 sites x 16 B must fit the array behind the descriptors (always true within the minor limit).  Beyond
+ * them the call returns WICK_ERR_UNSUPPORTED with a message; it never falls back to allocating.  All calls on a device
+ * share the array, which keeps the last call's contents (nothing in it needs to start at zero: each call rewrites the
+ * part it reads), so calls that overlap on the GPU (different streams or host threads) race: serialise them.
+ * Synchronises the stream before returning, like wick_minor_dets.  wick_static_scratch_bytes() returns the array size. */
+#define WICK_STATIC_SCRATCH_BYTES (16u << 20)
+#define WICK_STATIC_MAX_MINORS    4096
+int wick_minor_dets_static(const void* P_dev, int64_t n_sites, int n, const uint8_t* rows, const uint8_t* cols,
+                           int64_t n_minors, void* out_dev, void* cuda_stream);
+size_t wick_static_scratch_bytes(void);
+
 /* Step a4 for one flavour (0 = u, 1 = d) of a handle's unique-minor table, through exactly the kernels wick_contract
  * launches for it (the register-resident / cached kernels for the library's own tables; `flags` as for wick_contract).
  * P_dev: device complex128 [n_sites][12][12]; out_dev: device complex128 [n_minors][S] with S = n_sites rounded up to a

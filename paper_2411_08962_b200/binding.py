@@ -29,7 +29,7 @@ EXPORTED_SYMBOLS = (
     "wick_terms_export_minors", "wick_terms_export_terms", "wick_terms_export_factors",
     "wick_terms_staged_schedule_check", "wick_terms_export_minor_order", "wick_terms_free",
     "wick_contract_min_workspace_bytes", "wick_contract_workspace_bytes", "wick_contract",
-    "wick_contract_host", "wick_release_cached_buffers", "wick_minor_dets", "wick_terms_minor_table", "wick_launch_count", "wick_launch_count_reset",
+    "wick_contract_host", "wick_release_cached_buffers", "wick_minor_dets", "wick_minor_dets_static", "wick_static_scratch_bytes", "wick_terms_minor_table", "wick_launch_count", "wick_launch_count_reset",
     "wick_operator_from_nucleons", "wick_operator_from_raw", "wick_operator_paper", "wick_operator_info", "wick_operator_export",
     "wick_operator_free", "wick_operator_product", "wick_build_block_terms", "wick_block_tensor", "wick_block_tensor_workspace_bytes",
     "wick_combine_two_clusters", "wick_build_terms_matrix", "wick_contract_many", "wick_contract_many_workspace_bytes",
@@ -92,6 +92,9 @@ def load_library():
     lib.wick_contract.argtypes = [vp, vp, vp, vp, i32, i32, i32, vp, vp, vp, sz, u32, vp]
     lib.wick_contract_host.argtypes = [vp, vp, vp, vp, i32, i32, i32, vp, vp, u32]
     lib.wick_minor_dets.argtypes = [vp, i64, i32, vp, vp, i64, vp, vp]
+    lib.wick_minor_dets_static.argtypes = [vp, i64, i32, vp, vp, i64, vp, vp]
+    lib.wick_static_scratch_bytes.argtypes = []
+    lib.wick_static_scratch_bytes.restype = sz
     lib.wick_terms_minor_table.argtypes = [vp, i64, vp, i32, u32, vp, vp]
     lib.wick_operator_from_nucleons.argtypes = [C.POINTER(_Nucleon), i32, C.POINTER(vp)]
     lib.wick_operator_from_raw.argtypes = [i32, i64, vp, vp, vp, C.POINTER(vp)]
@@ -464,6 +467,28 @@ def minor_dets(P, rows, cols, stream=None):
                                  _stream_ptr(stream))
     _check(rc, "wick_minor_dets")
     return out
+
+
+def minor_dets_static(P, rows, cols, out, stream=None):
+    """wick_minor_dets_static: step a4 with no allocation inside the library (scratch in a static device array).  The caller
+    passes the output too: out CUDA complex128 [n_minors][n_sites]."""
+    lib = load_library()
+    _check_dev(P, "P")
+    rows = np.ascontiguousarray(rows, dtype=np.uint8)
+    cols = np.ascontiguousarray(cols, dtype=np.uint8)
+    n_minors, n = rows.shape
+    n_sites = P.shape[0]
+    _check_dev(out, "out", (n_minors, n_sites))
+    import torch
+    with torch.cuda.device(P.device):
+        rc = lib.wick_minor_dets_static(P.data_ptr(), n_sites, n, _np_ptr(rows), _np_ptr(cols), n_minors, out.data_ptr(),
+                                        _stream_ptr(stream))
+    _check(rc, "wick_minor_dets_static")
+    return out
+
+
+def static_scratch_bytes() -> int:
+    return int(load_library().wick_static_scratch_bytes())
 
 
 def minor_table(P, terms: Terms, flavour: int, flags: int = 0, stream=None):

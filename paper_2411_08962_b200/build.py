@@ -12,7 +12,7 @@ import sys
 PKG_DIR = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(PKG_DIR, "csrc")
 LIB_PATH = os.path.join(PKG_DIR, "libwick_b200.so")
-SOURCES = ["term_builder.cpp", "kernels.cu", "minors_reg.cu", "contract.cu"]
+SOURCES = ["term_builder.cpp", "kernels.cu", "minors_reg.cu", "contract.cu", "no_alloc.cu"]
 HEADERS = ["kernels.cuh", "lu_device.cuh", "wick_internal.h", os.path.join("..", "..", "include", "wick.h")]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-std=c++17", "-O3", "-lineinfo",
