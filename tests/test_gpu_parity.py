@@ -500,3 +500,26 @@ def test_two_cluster_sink_against_the_two_site_oracle(cuda_device):
                 ref += v
                 ref_abs += abs(v)
         assert abs(B[0, iu, idd] - ref) <= REL_TOL * ref_abs
+
+
+def test_two_cluster_sink_with_a_two_nucleon_cluster(cuda_device):
+    """Cluster sink with a multi-nucleon cluster: 3He as (a slice of) the p n cluster at x and a proton at y.
+    Block tensors of 3x3 / 2x1 minors over all 220 x 220 / 66 x 12 column subsets, Laplace combination on the host, against the
+    oracle's double sum over (x, y) with stacked 5x5 and 4x4 determinants."""
+    L, T = 2, 1
+    U, D = make_propagators_numpy(8644, L, T)
+    Ud, Dd = _dev(U, cuda_device), _dev(D, cuda_device)
+    sa = wo.merged_terms([("p", 0), ("n", 0)])[::12]             # 20 of the 231 sink terms: the oracle stays below a minute
+    sb = wo.merged_terms([("p", 1)])
+    raw = lambda lst: [(c, tuple(("u", x) for x in u) + tuple(("d", x) for x in d)) for (u, d, c) in lst]
+    src = wo.merged_from_raw([(c1 * c2, q1 + q2) for (c1, q1) in raw(sa) for (c2, q2) in raw(sb)])   # the product A.B, oracle side
+    fl = np.array([[0] * 3 + [1] * 3 for _ in sa], np.uint8)
+    chi = np.array([list(u) + list(d) for (u, d, _) in sa], np.uint8)
+    a = wk.operator_from_raw(fl, chi, np.array([c for (_, _, c) in sa], complex))
+    b = wk.operator_from_nucleons([("p", 1)])
+    ab = wk.operator_product(a, b)
+    assert ab.n_terms == len(src) and (ab.n_u, ab.n_d) == (5, 4)
+    for mom_a, mom_b in (((1, 0, 1), (0, 1, 0)),):
+        Cg = wk.two_cluster_correlator(Ud, Dd, a, b, mom_a, mom_b, L, T, source=ab)
+        Cr, sabs = wo.two_cluster_correlator(U, D, sa, sb, src, mom_a, mom_b, L)
+        assert np.all(np.abs(Cg - Cr) <= REL_TOL * sabs), (np.abs(Cg - Cr) / sabs).max()
