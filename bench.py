@@ -370,6 +370,45 @@ def rooflines(wk, cfg, terms, info, prof, ms_step, Tb, fp64_probe, hbm_gbs, d_ru
                             "algorithmic_bytes_per_timeslice": 4608.0 * cfg.volume}
 
 
+def bench_gevp(wk, torch, dev, Tb, steps, warmup):
+    """Correlation matrix (GEVP, Sec. V) of two deuteron interpolators -- the p n product operator of cfg1 and
+    the paper's Eq. (20) -- on the cfg1 lattice: wick_contract_many (every determinant once for the four entries) against four
+    separate wick_contract calls on the same four term lists."""
+    from wick_inputs import make_propagators_torch
+    cfg = CONFIGS["cfg1"]
+    ops = [wk.operator_from_nucleons(cfg.nucleus), wk.operator_paper(wk.OP_DEUTERON_EQ20)]
+    m = wk.build_terms_matrix(ops)
+    lists = [m[k][kp] for k in range(2) for kp in range(2)]
+    U, D = make_propagators_torch(cfg.seed, cfg.L, cfg.T, dev, t0=0, nt=Tb)
+
+    def many():
+        return wk.contract_many(U, D, lists, cfg.momenta, cfg.L, Tb)
+
+    def separate():
+        return [wk.contract(U, D, t, cfg.momenta, cfg.L, Tb) for t in lists]
+
+    out = {}
+    for name, fn in (("contract_many", many), ("four_contract_calls", separate)):
+        for _ in range(max(warmup, 3)):
+            fn()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(steps):
+            fn()
+        e1.record()
+        torch.cuda.synchronize()
+        out[name] = e0.elapsed_time(e1) / steps
+    Cm, Cs = many(), separate()
+    same = all(bool(torch.allclose(Cm[e], Cs[e], rtol=1e-12, atol=0.0)) for e in range(4))
+    i = lists[0].info
+    return {"workload": "cfg1 lattice, 2 x 2 correlation matrix of {p0 n0 product, Eq. (20)}", "operators_terms": [o.n_terms for o in ops],
+            "unique_minors_per_site": int(i.n_minors_u + i.n_minors_d), "terms_per_entry": [int(t.info.n_terms) for t in lists],
+            "timeslices_per_step": Tb, "steps": steps, "ms_per_step": out["contract_many"], "value": Tb / (out["contract_many"] * 1e-3),
+            "unit": "correlation-matrix timeslices/s", "ms_per_step_four_separate_calls": out["four_contract_calls"],
+            "speedup_from_sharing_the_minors": out["four_contract_calls"] / out["contract_many"], "entries_agree_with_separate_calls": same}
+
+
 def bench_workload(wk, torch, cfg, key, Tb, steps, warmup, dev, fp64_probe, hbm_gbs, isospin=False, sampler=None, flags=0):
     """One workload on this rank's GPU, device-resident inputs: timeslices/s, rooflines, launches.  Single-GPU path.
     isospin: one propagator for both flavours and the swap-symmetrised factorised list (WICK_BUILD_ISOSPIN)."""
@@ -608,6 +647,9 @@ def main():
                                        fp64_probe, hbm_gbs, isospin=True)
             rec["speedup_over_two_flavour_run"] = rec["value"] / value
             workloads[cfg.name + "+isospin"] = rec
+            torch.cuda.empty_cache()
+        if args.side_workloads:
+            workloads["gevp_2x2_deuteron"] = bench_gevp(wk, torch, dev, args.timeslices_per_step, min(args.side_steps, 50), args.warmup)
             torch.cuda.empty_cache()
 
     cpu_baseline = None
