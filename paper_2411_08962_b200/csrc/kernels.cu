@@ -209,18 +209,34 @@ __device__ __forceinline__ double shfl16(double v, int src) { return __shfl_sync
 
 // 16 lanes per site (12 used): lane = row of the propagator, its 12 entries in registers.  Gauss-Jordan in place without
 // moving rows: step k picks, among the lanes that have not been a pivot row yet, the one with the largest |re| + |im| in
-// column k (first wins); every lane then does  own[c] -= g * pivot_row[c]  with g = own[k] / piv (the pivot lane itself with
+// column k (compared to 2^-16, first wins); every lane then does  own[c] -= g * pivot_row[c]  with g = own[k] / piv (the pivot lane itself with
 // g = 1 - 1/piv, which scales it by 1/piv), and column k is replaced by the column of the inverse.  With p_k the pivot
 // lane of step k the lane p_i ends up holding (A^-1)[i][p_m] in register m.
 // Result of invert12 for one lane and one matrix: row `my_step` of the inverse, entry m belongs to column p_m (4-bit fields of perm).
 struct InvRow { double re[12], im[12]; int my_step; unsigned long long perm; c128 det; bool singular; };
 
-// NM matrices (the two flavours) are inverted TOGETHER: their pivot steps are independent instruction streams, which
-// doubles the work a thread has in flight between the dependent shuffle -> broadcast -> update stages of a step.
-// `bc`: NM x 12 complex of shared memory per site, through which the pivot rows of a step reach the other lanes (one
-// broadcast LDS.128 per entry instead of four shuffles).
+// NM matrices can be inverted TOGETHER (independent instruction streams in one thread); the fused kernel inverts the two
+// flavours one after the other instead, which halves the registers and lets 16 warps per SM hide the latencies.
+// The pivot row of a step and the reciprocal of its pivot reach the other lanes of the site by shuffles (52 per step; the
+// round-2 profile showed the LSU data pipe as the limiter, 82 % busy, and a single-lane STS.128 costs it the same four
+// cycles as a full-warp one, so the earlier shared-memory broadcast, 13 stores + 13 loads, was no cheaper).
+// The steps are software-pipelined ("look-ahead"): step k updates column k+1 FIRST, then starts the pivot search of step
+// k+1 (one packed {key, lane} word per lane, four max-shuffles) and the reciprocal of every lane's own candidate, and only
+// then updates the other ten columns, so the search, the MUFU and the Newton steps run under the 40 DFMAs of the update
+// instead of in front of them.  The packed word keeps the pivot key to 2^-16 (the low four bits hold the lane, smaller
+// lane wins ties).
+
+__device__ __forceinline__ unsigned packed_pivot_key(bool used, double re, double im, int sub) {
+    return used ? 0u : ((((unsigned(pivot_key(re, im)) >> 4) + 1u) << 4) | unsigned(15 - sub));
+}
+__device__ __forceinline__ int pivot_lane16(unsigned pk) {
+#pragma unroll
+    for (int off = 8; off > 0; off >>= 1) pk = max(pk, __shfl_xor_sync(0xffffffffu, pk, off, 16));
+    return 15 - int(pk & 15u);
+}
+
 template <int NM>
-__device__ __forceinline__ void invert12(const c128* const (&P)[NM], int64_t st, bool row_ok, int sub, c128* bc, InvRow (&R)[NM]) {
+__device__ __forceinline__ void invert12(const c128* const (&P)[NM], int64_t st, bool row_ok, int sub, InvRow (&R)[NM]) {
 #pragma unroll
     for (int q = 0; q < NM; ++q) {
 #pragma unroll
@@ -232,55 +248,49 @@ __device__ __forceinline__ void invert12(const c128* const (&P)[NM], int64_t st,
         R[q].my_step = 0; R[q].perm = 0; R[q].det = make_double2(1.0, 0.0); R[q].singular = false;
     }
     bool used[NM];                                                          // idle lanes never become pivots
+    int who[NM];                                                            // pivot lane of the coming step
+    c128 my_ip[NM];                                                         // reciprocal of this lane's candidate
 #pragma unroll
-    for (int q = 0; q < NM; ++q) used[q] = sub >= 12;
+    for (int q = 0; q < NM; ++q) {
+        used[q] = sub >= 12;
+        who[q] = pivot_lane16(packed_pivot_key(used[q], R[q].re[0], R[q].im[0], sub));
+        my_ip[q] = crecip(make_double2(R[q].re[0], R[q].im[0]));
+    }
 #pragma unroll
     for (int k = 0; k < 12; ++k) {
-        int p[NM];
         bool is_p[NM];
 #pragma unroll
         for (int q = 0; q < NM; ++q) {
-            // argmax of the pivot key over the 16 lanes of the site, smaller lane wins ties
-            int key = used[q] ? -1 : pivot_key(R[q].re[k], R[q].im[k]);
-            int who = sub;
-#pragma unroll
-            for (int off = 8; off > 0; off >>= 1) {
-                const int k2 = __shfl_xor_sync(0xffffffffu, key, off, 16), w2 = __shfl_xor_sync(0xffffffffu, who, off, 16);
-                if (k2 > key || (k2 == key && w2 < who)) { key = k2; who = w2; }
-            }
-            p[q] = who;
-            R[q].perm |= (unsigned long long)who << (4 * k);
-            is_p[q] = (sub == who);
+            is_p[q] = (sub == who[q]);
+            R[q].perm |= (unsigned long long)who[q] << (4 * k);
             if (is_p[q]) { used[q] = true; R[q].my_step = k; }
         }
-        __syncwarp();                                                       // the previous step's reads of bc are done
-#pragma unroll
-        for (int q = 0; q < NM; ++q)
-            if (is_p[q]) {
-#pragma unroll
-                for (int c = 0; c < 12; ++c) bc[q * 12 + c] = make_double2(R[q].re[c], R[q].im[c]);
-            }
-        __syncwarp();
 #pragma unroll
         for (int q = 0; q < NM; ++q) {
             double (&re)[12] = R[q].re;
             double (&im)[12] = R[q].im;
             double pr[12], pi[12];
 #pragma unroll
-            for (int c = 0; c < 12; ++c) { const c128 v = bc[q * 12 + c]; pr[c] = v.x; pi[c] = v.y; }
+            for (int c = 0; c < 12; ++c) { pr[c] = shfl16(re[c], who[q]); pi[c] = shfl16(im[c], who[q]); }
+            const c128 ip = make_double2(shfl16(my_ip[q].x, who[q]), shfl16(my_ip[q].y, who[q]));
             const c128 piv = make_double2(pr[k], pi[k]);
             R[q].singular = R[q].singular || (piv.x == 0.0 && piv.y == 0.0);
             R[q].det = cmul(R[q].det, piv);
-            const c128 ip = crecip(piv);
             // g = own[k] / piv for the other rows, 1 - 1/piv for the pivot row (which scales it by 1/piv)
             c128 g = cmul(make_double2(re[k], im[k]), ip);
             if (is_p[q]) g = make_double2(1.0 - ip.x, -ip.y);
-#pragma unroll
-            for (int c = 0; c < 12; ++c) {
-                if (c == k) continue;
+            auto update = [&](int c) {
                 re[c] = fma(-g.x, pr[c], fma(g.y, pi[c], re[c]));
                 im[c] = fma(-g.x, pi[c], fma(-g.y, pr[c], im[c]));
+            };
+            if (k < 11) {                                                   // look-ahead: everything step k+1 waits for
+                update(k + 1);
+                who[q] = pivot_lane16(packed_pivot_key(used[q], re[k + 1], im[k + 1], sub));
+                my_ip[q] = crecip(make_double2(re[k + 1], im[k + 1]));
             }
+#pragma unroll
+            for (int c = 0; c < 12; ++c)
+                if (c != k && c != k + 1) update(c);
             re[k] = is_p[q] ? ip.x : -g.x;
             im[k] = is_p[q] ? ip.y : -g.y;
         }
@@ -315,10 +325,9 @@ inverse12_kernel(const c128* __restrict__ P, int64_t st0, int64_t n_st_total, in
     const int64_t st = st0 + site;
     const bool live = site < n_batch && st < n_st_total;
     const bool row_ok = live && sub < 12;
-    __shared__ __align__(16) c128 bcast[INV_THREADS / 16][12];
     InvRow R[1];
     const c128* const Pq[1] = {P};
-    invert12<1>(Pq, st, row_ok, sub, bcast[threadIdx.x >> 4], R);
+    invert12<1>(Pq, st, row_ok, sub, R);
     if (live && sub == 0) det_out[site] = R[0].det;
     if (row_ok) store_inv_row(R[0], inv_out + site * 144, 1);
 }
@@ -330,16 +339,28 @@ inverse12_kernel(const c128* __restrict__ P, int64_t st0, int64_t n_st_total, in
 // Nothing but the propagators is read from and sigma written to global memory: 4608 B per site-time.
 constexpr int JF_SITES = INV_THREADS / 16;
 
-// A: element (r, c) of the site's inverse at A[(12 r + c) * JF_SITES] (site-minor layout: the 8 sites of a quarter warp
-// read one 128-byte row, conflict free)
+// A: element (r, c) of site ls of the CTA at A[jf_elem(r, c, ls)]: site-minor layout (the 8 sites of a quarter warp read
+// one 128-byte row, conflict free) with the site position rotated by the row, so that the 12 lanes of a site, which
+// store 12 different rows of one column at a time, spread over the banks as well (2-way instead of 12-way conflicts).
+__device__ __forceinline__ int jf_elem(int r, int c, int ls) { return (r * 12 + c) * JF_SITES + ((ls + r) & (JF_SITES - 1)); }
+
+// the lane's row of the inverse into that layout
+__device__ __forceinline__ void store_inv_row_shared(const InvRow& R, c128* A, int ls) {
+#pragma unroll
+    for (int m = 0; m < 12; ++m) {
+        const int col = int(R.perm >> (4 * m)) & 15;
+        A[jf_elem(R.my_step, col, ls)] = R.singular ? make_double2(0.0, 0.0) : make_double2(R.re[m], R.im[m]);
+    }
+}
+
 template <int M>
-__device__ __forceinline__ c128 small_minor(const c128* A, uint32_t idx) {   // rows = nibbles 0..3, columns = nibbles 4..7 of idx
+__device__ __forceinline__ c128 small_minor(const c128* A, int ls, uint32_t idx) {   // rows = nibbles 0..3, columns = nibbles 4..7 of idx
     if constexpr (M == 0) return make_double2(1.0, 0.0);
     else {
         int r[M], c[M];
 #pragma unroll
         for (int i = 0; i < M; ++i) { r[i] = int(idx >> (4 * i)) & 15; c[i] = int(idx >> (16 + 4 * i)) & 15; }
-        auto a = [&](int i, int j) { return A[(r[i] * 12 + c[j]) * JF_SITES]; };
+        auto a = [&](int i, int j) { return A[jf_elem(r[i], c[j], ls)]; };
         if constexpr (M == 1) return a(0, 0);
         else if constexpr (M == 2) return det2(a(0, 0), a(0, 1), a(1, 0), a(1, 1));
         else if constexpr (M == 3) {
@@ -359,11 +380,10 @@ __device__ __forceinline__ c128 small_minor(const c128* A, uint32_t idx) {   // 
 }
 
 template <int MU_, int MD_>
-__global__ void __launch_bounds__(INV_THREADS, 3)
+__global__ void __launch_bounds__(INV_THREADS, 4)
 jacobi_fused_kernel(const c128* __restrict__ U, const c128* __restrict__ D, bool same, int64_t st0, int64_t n_valid,
                     const JacobiTerm* __restrict__ terms, int n_terms, c128* __restrict__ sigma) {
     __shared__ __align__(16) c128 inv_s[2][144][JF_SITES];                  // [flavour][element][site]
-    __shared__ __align__(16) c128 bcast[JF_SITES][2 * 12];
     __shared__ __align__(16) c128 psum[INV_THREADS / JF_SITES][JF_SITES];
     __shared__ c128 dets_s[JF_SITES];
     {   // phase 1: 16 lanes per site invert both propagators
@@ -374,28 +394,39 @@ jacobi_fused_kernel(const c128* __restrict__ U, const c128* __restrict__ D, bool
         if (same) {
             InvRow R[1];
             const c128* const Pq[1] = {U};
-            invert12<1>(Pq, st0 + site, row_ok, sub, bcast[ls], R);
-            if (row_ok) store_inv_row(R[0], &inv_s[0][0][ls], JF_SITES);
+            invert12<1>(Pq, st0 + site, row_ok, sub, R);
+            if (row_ok) store_inv_row_shared(R[0], &inv_s[0][0][0], ls);
             dets = cmul(R[0].det, R[0].det);
         } else {
-            InvRow R[2];
-            const c128* const Pq[2] = {U, D};
-            invert12<2>(Pq, st0 + site, row_ok, sub, bcast[ls], R);
-            if (row_ok) { store_inv_row(R[0], &inv_s[0][0][ls], JF_SITES); store_inv_row(R[1], &inv_s[1][0][ls], JF_SITES); }
-            dets = cmul(R[0].det, R[1].det);
+            c128 du;
+            {
+                InvRow R[1];
+                const c128* const Pq[1] = {U};
+                invert12<1>(Pq, st0 + site, row_ok, sub, R);
+                if (row_ok) store_inv_row_shared(R[0], &inv_s[0][0][0], ls);
+                du = R[0].det;
+            }
+            {
+                InvRow R[1];
+                const c128* const Pq[1] = {D};
+                invert12<1>(Pq, st0 + site, row_ok, sub, R);
+                if (row_ok) store_inv_row_shared(R[0], &inv_s[1][0][0], ls);
+                dets = cmul(du, R[0].det);
+            }
         }
         if (sub == 0) dets_s[ls] = dets;
     }
     __syncthreads();
     // phase 2: lane = (site, one of 16 term slots); a quarter warp = the 8 sites of one term
     const int ls = threadIdx.x & (JF_SITES - 1), slot = threadIdx.x / JF_SITES;
-    const c128* Ui = &inv_s[0][0][ls];
-    const c128* Di = same ? Ui : &inv_s[1][0][ls];
+    const c128* Ui = &inv_s[0][0][0];
+    const c128* Di = same ? Ui : &inv_s[1][0][0];
     c128 acc = make_double2(0.0, 0.0);
+#pragma unroll 4
     for (int k = slot; k < n_terms; k += INV_THREADS / JF_SITES) {
         const uint4 h = __ldg(reinterpret_cast<const uint4*>(terms + k));
         const c128 w = __ldg(reinterpret_cast<const c128*>(terms + k) + 1);
-        acc = cfma(cmul(w, small_minor<MU_>(Ui, h.x)), small_minor<MD_>(Di, h.y), acc);
+        acc = cfma(cmul(w, small_minor<MU_>(Ui, ls, h.x)), small_minor<MD_>(Di, ls, h.y), acc);
     }
     psum[slot][ls] = acc;
     __syncthreads();
