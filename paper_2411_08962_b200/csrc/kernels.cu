@@ -333,24 +333,138 @@ inverse12_kernel(const c128* __restrict__ P, int64_t st0, int64_t n_st_total, in
 }
 
 // Fused Jacobi path for lists whose BOTH flavours have 8 <= n <= 11 and whose term count is of the order of the number of
-// unique minors (Li-7-sized lists): per site both propagators are inverted (16 lanes per site, registers), the inverses
-// go to shared memory, and the 16 lanes share the flat term list:
+// unique minors (Li-7-sized lists): per site both propagators are inverted in registers, the inverses go to shared
+// memory, and the threads of the CTA share the flat term list:
 //   sigma = det U det D sum_k w'_k det (U^-1)[J_u^c, I_u^c] det (D^-1)[J_d^c, I_d^c],   w'_k = w_k (-1)^(sum of the index sets)
 // Nothing but the propagators is read from and sigma written to global memory: 4608 B per site-time.
-constexpr int JF_SITES = INV_THREADS / 16;
+//
+// Inversion: FOUR lanes per matrix, three rows each (all 32 lanes busy; with one row per lane 12 of 16 are).  The profile of
+// the row-per-lane version showed the LSU data pipe as the limiter (82 % busy): every lane needs the whole pivot row every
+// step, 52 shuffles per step whatever the number of lanes a matrix is spread over, so three rows per lane cut that
+// traffic per matrix four times (8 matrices per warp instead of 2).  Same Gauss-Jordan without row moves, same look-ahead
+// as invert12: step k updates column k+1 first, every lane picks its best unused row of that column (its candidate),
+// starts the pivot search of step k+1 over the four lanes (two max-shuffles on a packed {key, row} word) and the reciprocal
+// of its candidate, then updates the other columns; the next step's shuffles read every lane's candidate row through
+// two selp.f64 per value.
+constexpr int JF_THREADS = 128;
+constexpr int JF_SITES = 16;                                                // 32 lane groups: 16 sites x 2 flavours
+
+struct InvRows3 { double re[3][12], im[3][12]; int my_step[3]; unsigned long long perm; c128 det; bool singular; };
+
+__device__ __forceinline__ double shfl4(double v, int src) { return __shfl_sync(0xffffffffu, v, src, 4); }
+// x_loc by two selp.f64 (the plain ternaries compile to a divergent three-way branch full of register moves)
+__device__ __forceinline__ double sel3(int loc, double x0, double x1, double x2) {
+    double r;
+    asm("{\n\t.reg .pred p0, p1;\n\tsetp.eq.s32 p0, %4, 0;\n\tsetp.eq.s32 p1, %4, 1;\n\tselp.f64 %0, %2, %3, p1;\n\tselp.f64 %0, %1, %0, p0;\n\t}"
+        : "=&d"(r) : "d"(x0), "d"(x1), "d"(x2), "r"(loc));
+    return r;
+}
+
+// this lane's best unused row of column k: packed {key to 2^-16, 15 - global row} (0 if all three are used), its position
+__device__ __forceinline__ unsigned local_candidate(const InvRows3& R, const bool (&used)[3], int k, int l, int& loc) {
+    unsigned best = 0u;
+    loc = 0;
+#pragma unroll
+    for (int j = 0; j < 3; ++j) {
+        const unsigned pk = used[j] ? 0u : ((((unsigned(pivot_key(R.re[j][k], R.im[j][k])) >> 4) + 1u) << 4) | unsigned(15 - (3 * l + j)));
+        if (pk > best) { best = pk; loc = j; }
+    }
+    return best;
+}
+
+__device__ __forceinline__ void invert12_rows3(const c128* __restrict__ P, bool ok, int l, InvRows3& R) {
+#pragma unroll
+    for (int j = 0; j < 3; ++j) {
+#pragma unroll
+        for (int c = 0; c < 12; ++c) {
+            c128 v = make_double2(0.0, 0.0);
+            if (ok) v = __ldg(P + (3 * l + j) * 12 + c);
+            R.re[j][c] = v.x; R.im[j][c] = v.y;
+        }
+        R.my_step[j] = 0;
+    }
+    R.perm = 0; R.det = make_double2(1.0, 0.0); R.singular = false;
+    bool used[3] = {false, false, false};
+    c128 my_ip;
+    unsigned pk;
+    int loc;                                                                // this lane's candidate row (the pivot row if the lane wins)
+    pk = local_candidate(R, used, 0, l, loc);
+    my_ip = crecip(make_double2(sel3(loc, R.re[0][0], R.re[1][0], R.re[2][0]), sel3(loc, R.im[0][0], R.im[1][0], R.im[2][0])));
+    pk = max(pk, __shfl_xor_sync(0xffffffffu, pk, 1, 4));
+    pk = max(pk, __shfl_xor_sync(0xffffffffu, pk, 2, 4));
+#pragma unroll
+    for (int k = 0; k < 12; ++k) {
+        const int p = 15 - int(pk & 15u);                                  // pivot row (global index), its lane
+        const int owner = (p * 11) >> 5;                                    // p / 3 for p < 16
+        double pr[12], pi[12];
+#pragma unroll
+        for (int c = 0; c < 12; ++c) {
+            pr[c] = shfl4(sel3(loc, R.re[0][c], R.re[1][c], R.re[2][c]), owner);
+            pi[c] = shfl4(sel3(loc, R.im[0][c], R.im[1][c], R.im[2][c]), owner);
+        }
+        const c128 ip = make_double2(shfl4(my_ip.x, owner), shfl4(my_ip.y, owner));
+        const c128 piv = make_double2(pr[k], pi[k]);
+        R.singular = R.singular || (piv.x == 0.0 && piv.y == 0.0);
+        R.det = cmul(R.det, piv);
+        R.perm |= (unsigned long long)p << (4 * k);
+        bool is_p[3];
+        c128 g[3];
+#pragma unroll
+        for (int j = 0; j < 3; ++j) {
+            is_p[j] = (p == 3 * l + j);
+            if (is_p[j]) { used[j] = true; R.my_step[j] = k; }
+            // g = own[k] / piv for the other rows, 1 - 1/piv for the pivot row (which scales it by 1/piv)
+            g[j] = cmul(make_double2(R.re[j][k], R.im[j][k]), ip);
+            if (is_p[j]) g[j] = make_double2(1.0 - ip.x, -ip.y);
+        }
+        auto update = [&](int c) {
+#pragma unroll
+            for (int j = 0; j < 3; ++j) {
+                R.re[j][c] = fma(-g[j].x, pr[c], fma(g[j].y, pi[c], R.re[j][c]));
+                R.im[j][c] = fma(-g[j].x, pi[c], fma(-g[j].y, pr[c], R.im[j][c]));
+            }
+        };
+        if (k < 11) {                                                       // look-ahead: everything step k+1 waits for
+            update(k + 1);
+            pk = local_candidate(R, used, k + 1, l, loc);
+            my_ip = crecip(make_double2(sel3(loc, R.re[0][k + 1], R.re[1][k + 1], R.re[2][k + 1]),
+                                        sel3(loc, R.im[0][k + 1], R.im[1][k + 1], R.im[2][k + 1])));
+            pk = max(pk, __shfl_xor_sync(0xffffffffu, pk, 1, 4));
+            pk = max(pk, __shfl_xor_sync(0xffffffffu, pk, 2, 4));
+        }
+#pragma unroll
+        for (int c = 0; c < 12; ++c)
+            if (c != k && c != k + 1) update(c);
+#pragma unroll
+        for (int j = 0; j < 3; ++j) {
+            R.re[j][k] = is_p[j] ? ip.x : -g[j].x;
+            R.im[j][k] = is_p[j] ? ip.y : -g[j].y;
+        }
+    }
+    // sign of the permutation k -> p_k
+    int inv_count = 0;
+#pragma unroll
+    for (int a = 0; a < 12; ++a)
+#pragma unroll
+        for (int b = a + 1; b < 12; ++b) inv_count += (int(R.perm >> (4 * a)) & 15) > (int(R.perm >> (4 * b)) & 15);
+    if (inv_count & 1) { R.det.x = -R.det.x; R.det.y = -R.det.y; }
+    if (R.singular) R.det = make_double2(0.0, 0.0);
+}
 
 // A: element (r, c) of site ls of the CTA at A[jf_elem(r, c, ls)]: site-minor layout (the 8 sites of a quarter warp read
-// one 128-byte row, conflict free) with the site position rotated by the row, so that the 12 lanes of a site, which
-// store 12 different rows of one column at a time, spread over the banks as well (2-way instead of 12-way conflicts).
+// one 128-byte half of a 256-byte row, conflict free) with the site position rotated by the row, so that the lanes of a
+// matrix, which store different rows of one column at a time, spread over the banks as well.
 __device__ __forceinline__ int jf_elem(int r, int c, int ls) { return (r * 12 + c) * JF_SITES + ((ls + r) & (JF_SITES - 1)); }
 
-// the lane's row of the inverse into that layout
-__device__ __forceinline__ void store_inv_row_shared(const InvRow& R, c128* A, int ls) {
+// the lane's three rows of the inverse into that layout
+__device__ __forceinline__ void store_inv_rows3_shared(const InvRows3& R, c128* A, int ls) {
 #pragma unroll
-    for (int m = 0; m < 12; ++m) {
-        const int col = int(R.perm >> (4 * m)) & 15;
-        A[jf_elem(R.my_step, col, ls)] = R.singular ? make_double2(0.0, 0.0) : make_double2(R.re[m], R.im[m]);
-    }
+    for (int j = 0; j < 3; ++j)
+#pragma unroll
+        for (int m = 0; m < 12; ++m) {
+            const int col = int(R.perm >> (4 * m)) & 15;
+            A[jf_elem(R.my_step[j], col, ls)] = R.singular ? make_double2(0.0, 0.0) : make_double2(R.re[j][m], R.im[j][m]);
+        }
 }
 
 template <int M>
@@ -380,78 +494,66 @@ __device__ __forceinline__ c128 small_minor(const c128* A, int ls, uint32_t idx)
 }
 
 template <int MU_, int MD_>
-__global__ void __launch_bounds__(INV_THREADS, 4)
-jacobi_fused_kernel(const c128* __restrict__ U, const c128* __restrict__ D, bool same, int64_t st0, int64_t n_valid,
+__global__ void __launch_bounds__(JF_THREADS, 2)
+jacobi_fused_kernel(const c128* __restrict__ U, const c128* __restrict__ D, int64_t st0, int64_t n_valid,
                     const JacobiTerm* __restrict__ terms, int n_terms, c128* __restrict__ sigma) {
-    __shared__ __align__(16) c128 inv_s[2][144][JF_SITES];                  // [flavour][element][site]
-    __shared__ __align__(16) c128 psum[INV_THREADS / JF_SITES][JF_SITES];
-    __shared__ c128 dets_s[JF_SITES];
-    {   // phase 1: 16 lanes per site invert both propagators
-        const int sub = threadIdx.x & 15, ls = threadIdx.x >> 4;
+    extern __shared__ __align__(16) unsigned char jf_smem[];
+    c128* inv_s = reinterpret_cast<c128*>(jf_smem);                        // [flavour][element][site] (jf_elem)
+    c128* psum = inv_s + 2 * 144 * JF_SITES;                                // [term slot][site]
+    c128* dets_s = psum + (JF_THREADS / JF_SITES) * JF_SITES;               // [flavour][site]
+    {   // phase 1: lane group = (flavour, site), 4 lanes x 3 rows; U == D simply inverts the same matrix twice
+        const int l = threadIdx.x & 3, grp = threadIdx.x >> 2;
+        const int f = grp / JF_SITES, ls = grp % JF_SITES;
         const int64_t site = int64_t(blockIdx.x) * JF_SITES + ls;
-        const bool row_ok = site < n_valid && sub < 12;
-        c128 dets;
-        if (same) {
-            InvRow R[1];
-            const c128* const Pq[1] = {U};
-            invert12<1>(Pq, st0 + site, row_ok, sub, R);
-            if (row_ok) store_inv_row_shared(R[0], &inv_s[0][0][0], ls);
-            dets = cmul(R[0].det, R[0].det);
-        } else {
-            c128 du;
-            {
-                InvRow R[1];
-                const c128* const Pq[1] = {U};
-                invert12<1>(Pq, st0 + site, row_ok, sub, R);
-                if (row_ok) store_inv_row_shared(R[0], &inv_s[0][0][0], ls);
-                du = R[0].det;
-            }
-            {
-                InvRow R[1];
-                const c128* const Pq[1] = {D};
-                invert12<1>(Pq, st0 + site, row_ok, sub, R);
-                if (row_ok) store_inv_row_shared(R[0], &inv_s[1][0][0], ls);
-                dets = cmul(du, R[0].det);
-            }
-        }
-        if (sub == 0) dets_s[ls] = dets;
+        const bool ok = site < n_valid;
+        InvRows3 R;
+        invert12_rows3((f ? D : U) + (st0 + site) * 144, ok, l, R);
+        store_inv_rows3_shared(R, inv_s + f * 144 * JF_SITES, ls);
+        if (l == 0) dets_s[f * JF_SITES + ls] = R.det;
     }
     __syncthreads();
-    // phase 2: lane = (site, one of 16 term slots); a quarter warp = the 8 sites of one term
+    // phase 2: lane = (site, one of 8 term slots); a half warp = the 16 sites of one term
     const int ls = threadIdx.x & (JF_SITES - 1), slot = threadIdx.x / JF_SITES;
-    const c128* Ui = &inv_s[0][0][0];
-    const c128* Di = same ? Ui : &inv_s[1][0][0];
+    const c128* Ui = inv_s;
+    const c128* Di = inv_s + 144 * JF_SITES;
     c128 acc = make_double2(0.0, 0.0);
 #pragma unroll 4
-    for (int k = slot; k < n_terms; k += INV_THREADS / JF_SITES) {
-        const uint4 h = __ldg(reinterpret_cast<const uint4*>(terms + k));
+    for (int k = slot; k < n_terms; k += JF_THREADS / JF_SITES) {
+        const uint2 h = __ldg(reinterpret_cast<const uint2*>(terms + k));
         const c128 w = __ldg(reinterpret_cast<const c128*>(terms + k) + 1);
         acc = cfma(cmul(w, small_minor<MU_>(Ui, ls, h.x)), small_minor<MD_>(Di, ls, h.y), acc);
     }
-    psum[slot][ls] = acc;
+    psum[slot * JF_SITES + ls] = acc;
     __syncthreads();
     if (threadIdx.x < JF_SITES) {                                           // fixed-order sum over the term slots
         const int64_t site = int64_t(blockIdx.x) * JF_SITES + threadIdx.x;
-        c128 t = psum[0][threadIdx.x];
+        c128 t = psum[threadIdx.x];
 #pragma unroll
-        for (int j = 1; j < INV_THREADS / JF_SITES; ++j) t = cadd(t, psum[j][threadIdx.x]);
-        if (site < n_valid) sigma[site] = cmul(t, dets_s[threadIdx.x]);
+        for (int j = 1; j < JF_THREADS / JF_SITES; ++j) t = cadd(t, psum[j * JF_SITES + threadIdx.x]);
+        if (site < n_valid) sigma[site] = cmul(t, cmul(dets_s[threadIdx.x], dets_s[JF_SITES + threadIdx.x]));
     }
+}
+
+constexpr size_t JF_SMEM = size_t(2 * 144 * JF_SITES + (JF_THREADS / JF_SITES) * JF_SITES + 2 * JF_SITES) * 16;
+
+template <int MU_, int MD_>
+static cudaError_t launch_jf(const c128* U, const c128* D, int64_t st0, int64_t n_valid, const JacobiTerm* terms, int n_terms,
+                             c128* sigma, cudaStream_t stream) {
+    const unsigned grid = unsigned((n_valid + JF_SITES - 1) / JF_SITES);
+    jacobi_fused_kernel<MU_, MD_><<<grid, JF_THREADS, JF_SMEM, stream>>>(U, D, st0, n_valid, terms, n_terms, sigma);
+    return cudaGetLastError();
 }
 
 template <int MU_>
 static cudaError_t launch_jf_d(int md, const c128* U, const c128* D, int64_t st0, int64_t n_valid, const JacobiTerm* terms, int n_terms,
                                c128* sigma, cudaStream_t stream) {
-    const unsigned grid = unsigned((n_valid + JF_SITES - 1) / JF_SITES);
-    const bool same = (U == D);
     switch (md) {
-        case 1: jacobi_fused_kernel<MU_, 1><<<grid, INV_THREADS, 0, stream>>>(U, D, same, st0, n_valid, terms, n_terms, sigma); break;
-        case 2: jacobi_fused_kernel<MU_, 2><<<grid, INV_THREADS, 0, stream>>>(U, D, same, st0, n_valid, terms, n_terms, sigma); break;
-        case 3: jacobi_fused_kernel<MU_, 3><<<grid, INV_THREADS, 0, stream>>>(U, D, same, st0, n_valid, terms, n_terms, sigma); break;
-        case 4: jacobi_fused_kernel<MU_, 4><<<grid, INV_THREADS, 0, stream>>>(U, D, same, st0, n_valid, terms, n_terms, sigma); break;
+        case 1: return launch_jf<MU_, 1>(U, D, st0, n_valid, terms, n_terms, sigma, stream);
+        case 2: return launch_jf<MU_, 2>(U, D, st0, n_valid, terms, n_terms, sigma, stream);
+        case 3: return launch_jf<MU_, 3>(U, D, st0, n_valid, terms, n_terms, sigma, stream);
+        case 4: return launch_jf<MU_, 4>(U, D, st0, n_valid, terms, n_terms, sigma, stream);
         default: return cudaErrorInvalidValue;
     }
-    return cudaGetLastError();
 }
 
 cudaError_t launch_jacobi_fused(int n_u, int n_d, const double2* U, const double2* D, int64_t st0, int64_t n_valid,
@@ -1328,8 +1430,18 @@ template <int N> static cudaError_t set_smem_attr() {
     return cudaFuncSetAttribute(minors_kernel<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(MinorCfg<N>::kSmem));
 }
 
+template <int MU_> static cudaError_t set_jf_attr() {
+    cudaError_t e;
+    if ((e = cudaFuncSetAttribute(jacobi_fused_kernel<MU_, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(JF_SMEM))) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(jacobi_fused_kernel<MU_, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(JF_SMEM))) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(jacobi_fused_kernel<MU_, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(JF_SMEM))) != cudaSuccess) return e;
+    return cudaFuncSetAttribute(jacobi_fused_kernel<MU_, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(JF_SMEM));
+}
+
 cudaError_t configure_kernels() {
     cudaError_t e;
+    if ((e = set_jf_attr<1>()) != cudaSuccess || (e = set_jf_attr<2>()) != cudaSuccess || (e = set_jf_attr<3>()) != cudaSuccess ||
+        (e = set_jf_attr<4>()) != cudaSuccess) return e;
     if ((e = configure_reg_kernels()) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(minors_large_cached_kernel<10, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(mlc_smem<10, 0>()))) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(minors_large_cached_kernel<11, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(mlc_smem<11, 1>()))) != cudaSuccess) return e;
