@@ -205,6 +205,12 @@ minors_kernel(const c128* __restrict__ P, int64_t st0, int64_t n_st_total, int S
 // ---------------------------------------------------------------------------------------------
 constexpr int INV_THREADS = 128;
 
+__device__ __forceinline__ void cp_async16(void* smem_dst, const void* gmem_src) {
+    const uint32_t d = static_cast<uint32_t>(__cvta_generic_to_shared(smem_dst));
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d), "l"(gmem_src) : "memory");
+}
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.commit_group;\n\tcp.async.wait_group 0;" ::: "memory"); }
+
 __device__ __forceinline__ double shfl16(double v, int src) { return __shfl_sync(0xffffffffu, v, src, 16); }
 
 // 16 lanes per site (12 used): lane = row of the propagator, its 12 entries in registers.  Gauss-Jordan in place without
@@ -493,7 +499,9 @@ __device__ __forceinline__ c128 small_minor(const c128* A, int ls, uint32_t idx)
     }
 }
 
-template <int MU_, int MD_>
+// STAGE_TERMS: the term records (32 B each) fit the CTA's shared memory beside the inverses (JF_TERMS_CAP) and are copied
+// there once per CTA instead of being read through L1 / L2 in the term loop
+template <int MU_, int MD_, bool STAGE_TERMS>
 __global__ void __launch_bounds__(JF_THREADS, 2)
 jacobi_fused_kernel(const c128* __restrict__ U, const c128* __restrict__ D, int64_t st0, int64_t n_valid,
                     const JacobiTerm* __restrict__ terms, int n_terms, c128* __restrict__ sigma) {
@@ -501,6 +509,11 @@ jacobi_fused_kernel(const c128* __restrict__ U, const c128* __restrict__ D, int6
     c128* inv_s = reinterpret_cast<c128*>(jf_smem);                        // [flavour][element][site] (jf_elem)
     c128* psum = inv_s + 2 * 144 * JF_SITES;                                // [term slot][site]
     c128* dets_s = psum + (JF_THREADS / JF_SITES) * JF_SITES;               // [flavour][site]
+    const JacobiTerm* terms_s = reinterpret_cast<const JacobiTerm*>(dets_s + 2 * JF_SITES);
+    if (STAGE_TERMS) {                                                      // term records: in flight during the inversions
+        for (int i = threadIdx.x; i < 2 * n_terms; i += JF_THREADS)
+            cp_async16(reinterpret_cast<uint4*>(dets_s + 2 * JF_SITES) + i, reinterpret_cast<const uint4*>(terms) + i);
+    }
     {   // phase 1: lane group = (flavour, site), 4 lanes x 3 rows; U == D simply inverts the same matrix twice
         const int l = threadIdx.x & 3, grp = threadIdx.x >> 2;
         const int f = grp / JF_SITES, ls = grp % JF_SITES;
@@ -511,6 +524,7 @@ jacobi_fused_kernel(const c128* __restrict__ U, const c128* __restrict__ D, int6
         store_inv_rows3_shared(R, inv_s + f * 144 * JF_SITES, ls);
         if (l == 0) dets_s[f * JF_SITES + ls] = R.det;
     }
+    if (STAGE_TERMS) cp_async_wait_all();
     __syncthreads();
     // phase 2: lane = (site, one of 8 term slots); a half warp = the 16 sites of one term
     const int ls = threadIdx.x & (JF_SITES - 1), slot = threadIdx.x / JF_SITES;
@@ -519,8 +533,10 @@ jacobi_fused_kernel(const c128* __restrict__ U, const c128* __restrict__ D, int6
     c128 acc = make_double2(0.0, 0.0);
 #pragma unroll 4
     for (int k = slot; k < n_terms; k += JF_THREADS / JF_SITES) {
-        const uint2 h = __ldg(reinterpret_cast<const uint2*>(terms + k));
-        const c128 w = __ldg(reinterpret_cast<const c128*>(terms + k) + 1);
+        uint2 h;
+        c128 w;
+        if (STAGE_TERMS) { h = *reinterpret_cast<const uint2*>(terms_s + k); w = *(reinterpret_cast<const c128*>(terms_s + k) + 1); }
+        else { h = __ldg(reinterpret_cast<const uint2*>(terms + k)); w = __ldg(reinterpret_cast<const c128*>(terms + k) + 1); }
         acc = cfma(cmul(w, small_minor<MU_>(Ui, ls, h.x)), small_minor<MD_>(Di, ls, h.y), acc);
     }
     psum[slot * JF_SITES + ls] = acc;
@@ -535,12 +551,17 @@ jacobi_fused_kernel(const c128* __restrict__ U, const c128* __restrict__ D, int6
 }
 
 constexpr size_t JF_SMEM = size_t(2 * 144 * JF_SITES + (JF_THREADS / JF_SITES) * JF_SITES + 2 * JF_SITES) * 16;
+constexpr int JF_TERMS_CAP = 1024;                                          // 32 KB of records; two CTAs per SM still fit
+constexpr size_t JF_SMEM_STAGED = JF_SMEM + size_t(JF_TERMS_CAP) * sizeof(JacobiTerm);
 
 template <int MU_, int MD_>
 static cudaError_t launch_jf(const c128* U, const c128* D, int64_t st0, int64_t n_valid, const JacobiTerm* terms, int n_terms,
                              c128* sigma, cudaStream_t stream) {
     const unsigned grid = unsigned((n_valid + JF_SITES - 1) / JF_SITES);
-    jacobi_fused_kernel<MU_, MD_><<<grid, JF_THREADS, JF_SMEM, stream>>>(U, D, st0, n_valid, terms, n_terms, sigma);
+    if (n_terms <= JF_TERMS_CAP)
+        jacobi_fused_kernel<MU_, MD_, true><<<grid, JF_THREADS, JF_SMEM + size_t(n_terms) * sizeof(JacobiTerm), stream>>>(U, D, st0, n_valid, terms, n_terms, sigma);
+    else
+        jacobi_fused_kernel<MU_, MD_, false><<<grid, JF_THREADS, JF_SMEM, stream>>>(U, D, st0, n_valid, terms, n_terms, sigma);
     return cudaGetLastError();
 }
 
@@ -906,11 +927,6 @@ reduce_outer_kernel(const c128* __restrict__ MU, const c128* __restrict__ MD, in
 // Every minor is read from DRAM once per batch that needs it.  Work order is fixed by the host
 // schedule: bit-reproducible.
 // ---------------------------------------------------------------------------------------------
-__device__ __forceinline__ void cp_async16(void* smem_dst, const void* gmem_src) {
-    const uint32_t d = static_cast<uint32_t>(__cvta_generic_to_shared(smem_dst));
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d), "l"(gmem_src) : "memory");
-}
-__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.commit_group;\n\tcp.async.wait_group 0;" ::: "memory"); }
 
 constexpr int STG_W = STG_THREADS / 32;
 // shared memory map (bytes)
@@ -1430,12 +1446,15 @@ template <int N> static cudaError_t set_smem_attr() {
     return cudaFuncSetAttribute(minors_kernel<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(MinorCfg<N>::kSmem));
 }
 
+template <int MU_, int MD_> static cudaError_t set_jf_attr2() {
+    const cudaError_t e = cudaFuncSetAttribute(jacobi_fused_kernel<MU_, MD_, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(JF_SMEM_STAGED));
+    if (e != cudaSuccess) return e;
+    return cudaFuncSetAttribute(jacobi_fused_kernel<MU_, MD_, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(JF_SMEM));
+}
 template <int MU_> static cudaError_t set_jf_attr() {
     cudaError_t e;
-    if ((e = cudaFuncSetAttribute(jacobi_fused_kernel<MU_, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(JF_SMEM))) != cudaSuccess) return e;
-    if ((e = cudaFuncSetAttribute(jacobi_fused_kernel<MU_, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(JF_SMEM))) != cudaSuccess) return e;
-    if ((e = cudaFuncSetAttribute(jacobi_fused_kernel<MU_, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(JF_SMEM))) != cudaSuccess) return e;
-    return cudaFuncSetAttribute(jacobi_fused_kernel<MU_, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(JF_SMEM));
+    if ((e = set_jf_attr2<MU_, 1>()) != cudaSuccess || (e = set_jf_attr2<MU_, 2>()) != cudaSuccess || (e = set_jf_attr2<MU_, 3>()) != cudaSuccess) return e;
+    return set_jf_attr2<MU_, 4>();
 }
 
 cudaError_t configure_kernels() {
