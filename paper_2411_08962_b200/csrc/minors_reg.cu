@@ -6,7 +6,8 @@
 // with S the 4-row Schur complement; its columns are needed for the NC <= 10 "candidate" column indices that occur behind the
 // leading ones.  The thread computes all candidate Schur columns ONCE: into registers (4 complex each; the LAST level of the
 // trie is fully unrolled over the candidate positions, so its register indices are static and it touches no memory but the
-// result store) and into a per-thread shared-memory copy (positions 0 .. NC-2, for the pair and third levels, which fetch
+// result store; every lane stores, the output rows are S_b >= 32 * gridDim.x wide, so lanes beyond the end of the lattice,
+// whose tiles are zero, write zeros into the padding) and into a per-thread shared-memory copy (positions 0 .. NC-2, for the pair and third levels, which fetch
 // their columns by dynamic index).  The trie of the instance's column tuples over candidate POSITIONS is a word program built
 // on the host (contract.cu: build_reg_host): it is the same for every row tuple, because an outer-product list pairs every
 // row tuple with the same column tuples.  Everything that steers a job is warp uniform (the warp index is taken through a
@@ -28,7 +29,6 @@ struct Trie {
     c128 c3[4];                       // 3x3 minors of (.., T[i4]) over the row triples that leave out row r
     c128* o;                          // where the next minor goes (this lane)
     size_t step;                      // S_b
-    bool valid;
 };
 
 // 3x3 minors of (.., t): c3[r] = det(rows != r), expanded along the last column in the 2x2 minors s
@@ -47,7 +47,7 @@ __device__ __forceinline__ void finish_all(Trie<NC>& c, uint32_t mask5) {
         if ((mask5 >> I5) & 1u) {
             const c128 e0 = cfnma(c.T[I5][0], c.c3[0], cmul(c.T[I5][1], c.c3[1]));   // -t0 m0 + t1 m1
             const c128 e1 = cfnma(c.T[I5][2], c.c3[2], cmul(c.T[I5][3], c.c3[3]));   // -t2 m2 + t3 m3
-            if (c.valid) *c.o = cadd(e0, e1);
+            *c.o = cadd(e0, e1);                                  // lanes beyond the lattice hold zero tiles and store 0 into the padding of the row
             c.o += c.step;
         }
         finish_all<NC, I5 + 1>(c, mask5);
@@ -96,7 +96,6 @@ minors_reg_kernel(const c128* __restrict__ P, int64_t st0, int64_t n_st_total, i
     const int bin = blockIdx.y * (REG_THREADS / 32) + warp;
     const int j0 = __ldg(rt.bin_ptr + bin), j1 = __ldg(rt.bin_ptr + bin + 1);
     Trie<NC> c;
-    c.valid = st_first + lane < n_st_total;
     c.step = size_t(S_b);
     c128* outp = out + int64_t(g) * GROUP + lane;
     for (int j = j0; j < j1; ++j) {
