@@ -27,8 +27,9 @@ struct Trie {
     c128 T[NC][4];                    // Schur columns of the candidate positions (registers: the static last level)
     c128 s[6];                        // 2x2 minors of (detp * T[i2], T[i3]) over the row pairs 01 02 03 12 13 23
     c128 c3[4];                       // 3x3 minors of (.., T[i4]) over the row triples that leave out row r
-    c128* o;                          // where the next minor goes (this lane)
-    size_t step;                      // S_b
+    c128* o;                          // where the job's first minor goes (this lane)
+    uint32_t k;                       // element offset of the job's next minor (minors stored so far x S_b; a job has <= 165 minors)
+    uint32_t step;                    // S_b
 };
 
 // 3x3 minors of (.., t): c3[r] = det(rows != r), expanded along the last column in the 2x2 minors s
@@ -47,8 +48,11 @@ __device__ __forceinline__ void finish_all(Trie<NC>& c, uint32_t mask5) {
         if ((mask5 >> I5) & 1u) {
             const c128 e0 = cfnma(c.T[I5][0], c.c3[0], cmul(c.T[I5][1], c.c3[1]));   // -t0 m0 + t1 m1
             const c128 e1 = cfnma(c.T[I5][2], c.c3[2], cmul(c.T[I5][3], c.c3[3]));   // -t2 m2 + t3 m3
-            *c.o = cadd(e0, e1);                                  // lanes beyond the lattice hold zero tiles and store 0 into the padding of the row
-            c.o += c.step;
+            // the address is formed from a 32-bit element offset right before the store: a store holds its source registers
+            // until the LSU has read them (~30 cycles here), and a pointer that is incremented after every store waits for that
+            c128* const here = c.o + c.k;
+            c.k += c.step;
+            *here = cadd(e0, e1);                                 // lanes beyond the lattice hold zero tiles and store 0 into the padding of the row
         }
         finish_all<NC, I5 + 1>(c, mask5);
     }
@@ -96,7 +100,7 @@ minors_reg_kernel(const c128* __restrict__ P, int64_t st0, int64_t n_st_total, i
     const int bin = blockIdx.y * (REG_THREADS / 32) + warp;
     const int j0 = __ldg(rt.bin_ptr + bin), j1 = __ldg(rt.bin_ptr + bin + 1);
     Trie<NC> c;
-    c.step = size_t(S_b);
+    c.step = uint32_t(S_b);
     c128* outp = out + int64_t(g) * GROUP + lane;
     for (int j = j0; j < j1; ++j) {
         const uint32_t jr = __ldg(rt.bin_jobs + j);
@@ -116,6 +120,7 @@ minors_reg_kernel(const c128* __restrict__ P, int64_t st0, int64_t n_st_total, i
             detp = lu.detp;
         }
         c.o = outp + (size_t(r) * size_t(rt.n_cols) + size_t(h1.w)) * size_t(S_b);
+        c.k = 0;
         // the instance's trie: pair words {i2, i3, number of third words}, each followed by its third words {i4, mask of i5}
         const uint32_t* pw = rt.prog + h1.y;
         const uint32_t* const pend = rt.prog + h1.z;
