@@ -73,9 +73,15 @@ __device__ __forceinline__ void schur_columns(const LuState<N, 0, REG_THREADS>& 
     }
 }
 
-__device__ __forceinline__ void cached_column(const c128* Sc, uint32_t pos, c128 (&t)[4]) {
-#pragma unroll
-    for (int r = 0; r < 4; ++r) t[r] = Sc[(pos * 4 + r) * REG_THREADS];
+// `sc` = shared-window address of this thread's Sc[0], held in a register (given the chance the compiler rebuilds it from
+// S2R for every fetch)
+__device__ __forceinline__ void cached_column(uint32_t sc, uint32_t pos, c128 (&t)[4]) {
+    const uint32_t a = sc + pos * uint32_t(4 * REG_THREADS * 16);
+    constexpr int kStep = REG_THREADS * 16;
+    asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(t[0].x), "=d"(t[0].y) : "r"(a) : "memory");
+    asm volatile("ld.shared.v2.f64 {%0, %1}, [%2+%3];" : "=d"(t[1].x), "=d"(t[1].y) : "r"(a), "n"(kStep) : "memory");
+    asm volatile("ld.shared.v2.f64 {%0, %1}, [%2+%3];" : "=d"(t[2].x), "=d"(t[2].y) : "r"(a), "n"(2 * kStep) : "memory");
+    asm volatile("ld.shared.v2.f64 {%0, %1}, [%2+%3];" : "=d"(t[3].x), "=d"(t[3].y) : "r"(a), "n"(3 * kStep) : "memory");
 }
 
 }  // namespace
@@ -89,6 +95,8 @@ minors_reg_kernel(const c128* __restrict__ P, int64_t st0, int64_t n_st_total, i
     extern __shared__ __align__(16) unsigned char smem_raw[];
     c128* tile = reinterpret_cast<c128*>(smem_raw);
     c128* Sc = tile + TILE_ELEMS + threadIdx.x;                       // this thread's copy of the Schur columns: entry e at Sc[e * NT]
+    uint32_t sc = uint32_t(__cvta_generic_to_shared(Sc));
+    asm volatile("mov.b32 %0, %0;" : "+r"(sc));                       // opaque: stays in its register
     const int g = blockIdx.x;
     const int64_t st_first = st0 + int64_t(g) * GROUP;
     const int lane = threadIdx.x & 31;
@@ -124,13 +132,15 @@ minors_reg_kernel(const c128* __restrict__ P, int64_t st0, int64_t n_st_total, i
         // the instance's trie: pair words {i2, i3, number of third words}, each followed by its third words {i4, mask of i5}
         const uint32_t* pw = rt.prog + h1.y;
         const uint32_t* const pend = rt.prog + h1.z;
-        while (pw < pend) {
-            const uint32_t w = __ldg(pw++);
+        if (pw >= pend) continue;
+        uint32_t w = __ldg(pw), w3 = __ldg(pw + 1);                   // every pair word is followed by >= 1 third word
+        while (true) {
             const uint32_t n3 = w >> 8;
+            const uint32_t* const pn = pw + 1 + n3;                   // the next pair word
             {
                 c128 a[4], b[4];
-                cached_column(Sc, w & 15u, a);
-                cached_column(Sc, (w >> 4) & 15u, b);
+                cached_column(sc, w & 15u, a);
+                cached_column(sc, (w >> 4) & 15u, b);
 #pragma unroll
                 for (int q = 0; q < 4; ++q) a[q] = cmul(detp, a[q]);
                 int k = 0;
@@ -139,19 +149,22 @@ minors_reg_kernel(const c128* __restrict__ P, int64_t st0, int64_t n_st_total, i
 #pragma unroll
                     for (int y = x + 1; y < 4; ++y) c.s[k++] = det2(a[x], b[x], a[y], b[y]);
             }
-            uint32_t w3 = __ldg(pw);
             c128 t[4];
-            cached_column(Sc, w3 & 15u, t);
+            cached_column(sc, w3 & 15u, t);
             for (uint32_t q = 0; q < n3; ++q) {
                 third_from(c.s, t, c.c3);
                 const uint32_t mask5 = w3 >> 4;
-                ++pw;
                 if (q + 1 < n3) {                                     // next third column: in flight during this node's last level
-                    w3 = __ldg(pw);
-                    cached_column(Sc, w3 & 15u, t);
+                    w3 = __ldg(pw + 2 + q);
+                    cached_column(sc, w3 & 15u, t);
+                } else if (pn < pend) {                               // ... or the words of the next pair
+                    w = __ldg(pn);
+                    w3 = __ldg(pn + 1);
                 }
                 finish_all<NC, 3>(c, mask5);
             }
+            if (pn >= pend) break;
+            pw = pn;
         }
     }
 }
