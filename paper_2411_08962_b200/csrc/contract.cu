@@ -666,22 +666,18 @@ RegHost build_reg_host(const FlavourTables& ft, bool grid) {
         j.prog_begin = uint32_t(h.prog.size());
         int pos_of[12];
         { int k = 0; for (int b = 0; b < 12; ++b) pos_of[b] = (cand_mask & (1u << b)) ? k++ : -1; }
-        // the tuples are sorted, so consecutive tuples with equal (i2, i3) form a pair node and with equal (i2, i3, i4) a third node
+        // the tuples are sorted, so consecutive tuples with equal (i2, i3) form a pair node and with equal (i2, i3, i4) a third node;
+        // one word per THIRD node: i4 | mask(i5) << 4 | i2 << 14 | i3 << 18 | (first third node of its pair) << 22
         int n_pairs = 0, n_thirds = 0;
-        size_t pair_word = 0;
         int p2 = -1, p3 = -1, p4 = -1;
         for (size_t c = c0; c < c1; ++c) {
             const uint64_t w = nibbles_of_mask(ft.cols[c]) >> (4 * K);
             int x[4];
             for (int i = 0; i < 4; ++i) x[i] = pos_of[(w >> (4 * i)) & 15u];
-            if (x[0] != p2 || x[1] != p3) {
-                pair_word = h.prog.size();
-                h.prog.push_back(uint32_t(x[0]) | (uint32_t(x[1]) << 4));
-                p2 = x[0]; p3 = x[1]; p4 = -1; ++n_pairs;
-            }
+            const bool new_pair = (x[0] != p2 || x[1] != p3);
+            if (new_pair) { p2 = x[0]; p3 = x[1]; p4 = -1; ++n_pairs; }
             if (x[2] != p4) {
-                h.prog.push_back(uint32_t(x[2]));
-                h.prog[pair_word] += 1u << 8;
+                h.prog.push_back(uint32_t(x[2]) | (uint32_t(x[0]) << 14) | (uint32_t(x[1]) << 18) | (new_pair ? 1u << 22 : 0u));
                 p4 = x[2]; ++n_thirds;
             }
             h.prog.back() |= 1u << (4 + x[3]);
@@ -693,7 +689,7 @@ RegHost build_reg_host(const FlavourTables& ft, bool grid) {
         c0 = c1;
     }
     if (h.jobs.size() > 256 || !minors_reg_supported(n, max_cand)) { h.jobs.clear(); return h; }
-    h.prog.push_back(0);                                            // the kernel reads one word ahead
+    h.prog.push_back(0); h.prog.push_back(0);                       // the kernel reads two words ahead
     h.rows.resize(ft.rows.size());
     for (size_t r = 0; r < ft.rows.size(); ++r) h.rows[r] = uint32_t(nibbles_of_mask(ft.rows[r]));
     h.ok = true;

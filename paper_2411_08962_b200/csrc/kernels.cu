@@ -128,7 +128,7 @@ minors_kernel(const c128* __restrict__ P, int64_t st0, int64_t n_st_total, int S
     stage_tile(tile, P, st_first, n_st_total, NT);
     __syncthreads();
     const c128* tl = tile + lane;
-    const bool valid = st_first + lane < n_st_total;
+    // every lane stores: the rows of `out` are S_b >= 32 * gridDim.x wide, lanes beyond the end of the lattice hold zero tiles
     c128* outp = out + int64_t(g) * GROUP + lane;
     if constexpr (N == 3) {
         // 3x3: the cofactors of the last column depend on (row tuple, first two columns) only and are kept
@@ -153,7 +153,7 @@ minors_kernel(const c128* __restrict__ P, int64_t st0, int64_t n_st_total, int S
             const int c2 = int(dc.col(2));
             const c128 det = cfma(ld(tl, re[2], c2), cof[2], cfma(ld(tl, re[1], c2), cof[1], cmul(ld(tl, re[0], c2), cof[0])));
             prow = rws; pcol = cls;
-            if (valid) outp[int64_t(m) * S_b] = dc.signed_result(det);
+            outp[int64_t(m) * S_b] = dc.signed_result(det);
         }
     } else if constexpr (N <= 2) {
         for (; m < m_stop; m += kStride) {
@@ -163,7 +163,7 @@ minors_kernel(const c128* __restrict__ P, int64_t st0, int64_t n_st_total, int S
 #pragma unroll
             for (int i = 0; i < N; ++i) { ix.re[i] = int(dc.row(i)) * 12; ix.ce[i] = int(dc.col(i)); }
             const c128 det = det_small<N>(tl, ix);
-            if (valid) outp[int64_t(m) * S_b] = dc.signed_result(det);
+            outp[int64_t(m) * S_b] = dc.signed_result(det);
         }
     } else {
         constexpr int K = N - 4;
@@ -190,7 +190,7 @@ minors_kernel(const c128* __restrict__ P, int64_t st0, int64_t n_st_total, int S
             if (new_pair || (diff & kLead3) != 0) lu.third_column(tb, Ls, dc.col(K + 2) * kColStep);
             const c128 det = lu.finish(tb, Ls, dc.col(K + 3) * kColStep);
             prow = rws; pcol = dc.cols_bits();
-            if (valid) outp[int64_t(dc.out_index(m)) * S_b] = dc.signed_result(det);
+            outp[int64_t(dc.out_index(m)) * S_b] = dc.signed_result(det);
         }
     }
 }
@@ -632,7 +632,7 @@ minors6_cached_kernel(const c128* __restrict__ P, int64_t st0, int64_t n_st_tota
     stage_tile(tile, P, st_first, n_st_total, NT);
     __syncthreads();
     const unsigned char* tb = reinterpret_cast<const unsigned char*>(tile + lane);
-    const bool valid = st_first + lane < n_st_total;
+    // every lane stores: the rows of `out` are S_b >= 32 * gridDim.x wide, lanes beyond the end of the lattice hold zero tiles
     c128* outp = out + int64_t(g) * GROUP + lane;
     constexpr uint32_t kRowStep = 12 * GROUP * 16, kColStep = GROUP * 16;
     LuState<N, 0, NT> lu;
@@ -684,7 +684,7 @@ minors6_cached_kernel(const c128* __restrict__ P, int64_t st0, int64_t n_st_tota
         cached(dc.col(5), t);
         const c128 det = lu.finish_from(t);
         prow = rws; pcol = dc.cols_bits();
-        if (valid) outp[int64_t(m) * S_b] = det;
+        outp[int64_t(m) * S_b] = det;
     }
 }
 
@@ -720,7 +720,7 @@ minors_large_cached_kernel(const c128* __restrict__ P, int64_t st0, int64_t n_st
     stage_tile(tile, P, st_first, n_st_total, NT);
     __syncthreads();
     const unsigned char* tb = reinterpret_cast<const unsigned char*>(tile + lane);
-    const bool valid = st_first + lane < n_st_total;
+    // every lane stores: the rows of `out` are S_b >= 32 * gridDim.x wide, lanes beyond the end of the lattice hold zero tiles
     c128* outp = out + int64_t(g) * GROUP + lane;
     constexpr uint32_t kRowStep = 12 * GROUP * 16, kColStep = GROUP * 16;
     constexpr unsigned long long kLead = (1ull << (4 * K)) - 1, kLeadPair = (1ull << (4 * (K + 2))) - 1,
@@ -773,7 +773,7 @@ minors_large_cached_kernel(const c128* __restrict__ P, int64_t st0, int64_t n_st
         cached(dc.col(K + 3), t);
         const c128 det = lu.finish_from(t);
         prow = rws; pcol = dc.cols_bits();
-        if (valid) outp[int64_t(dc.out_index(m)) * S_b] = dc.negate() ? make_double2(-det.x, -det.y) : det;
+        outp[int64_t(dc.out_index(m)) * S_b] = dc.negate() ? make_double2(-det.x, -det.y) : det;
     }
 }
 

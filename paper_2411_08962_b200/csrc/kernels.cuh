@@ -45,7 +45,7 @@ static_assert(sizeof(RegJob) == 32, "RegJob is read with 16-byte loads");
 struct RegTables {
     int n_cols, n_bins;                   // column tuples per row tuple; warps of work per site group (multiple of 8)
     const RegJob* jobs;                   // [n_jobs <= 256]
-    const uint32_t* prog;                 // pair words i2 | i3 << 4 | n_third << 8, each followed by its third words i4 | mask(i5) << 4
+    const uint32_t* prog;                 // one word per third node: i4 | mask(i5) << 4 | i2 << 14 | i3 << 18 | first-of-its-pair << 22
     const uint32_t* row_nibbles;          // [n_rows] row indices as 4-bit fields
     const uint32_t* bin_ptr;              // [n_bins + 1]
     const uint32_t* bin_jobs;             // (row tuple << 8) | job, grouped by bin

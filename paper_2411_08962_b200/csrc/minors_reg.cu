@@ -9,7 +9,7 @@
 // result store; every lane stores, the output rows are S_b >= 32 * gridDim.x wide, so lanes beyond the end of the lattice,
 // whose tiles are zero, write zeros into the padding) and into a per-thread shared-memory copy (positions 0 .. NC-2, for the pair and third levels, which fetch
 // their columns by dynamic index).  The trie of the instance's column tuples over candidate POSITIONS is a word program built
-// on the host (contract.cu: build_reg_host): it is the same for every row tuple, because an outer-product list pairs every
+// on the host (contract.cu: build_reg_host; one word per third node): it is the same for every row tuple, because an outer-product list pairs every
 // row tuple with the same column tuples.  Everything that steers a job is warp uniform (the warp index is taken through a
 // shuffle so that the compiler knows), so every test is a uniform branch.
 //
@@ -129,18 +129,19 @@ minors_reg_kernel(const c128* __restrict__ P, int64_t st0, int64_t n_st_total, i
         }
         c.o = outp + (size_t(r) * size_t(rt.n_cols) + size_t(h1.w)) * size_t(S_b);
         c.k = 0;
-        // the instance's trie: pair words {i2, i3, number of third words}, each followed by its third words {i4, mask of i5}
+        // the instance's trie as a flat stream of third-node words {i4, mask of i5, i2, i3, first-of-its-pair flag}
+        // (contract.cu: build_reg_host); the column of the next node and the word after it are in flight during a node's last level
         const uint32_t* pw = rt.prog + h1.y;
         const uint32_t* const pend = rt.prog + h1.z;
         if (pw >= pend) continue;
-        uint32_t w = __ldg(pw), w3 = __ldg(pw + 1);                   // every pair word is followed by >= 1 third word
+        uint32_t w = __ldg(pw), wn = __ldg(pw + 1);
+        c128 t[4];
+        cached_column(sc, w & 15u, t);
         while (true) {
-            const uint32_t n3 = w >> 8;
-            const uint32_t* const pn = pw + 1 + n3;                   // the next pair word
-            {
+            if (w & (1u << 22)) {                                     // new pair node: 2x2 minors of (detp * T[i2], T[i3])
                 c128 a[4], b[4];
-                cached_column(sc, w & 15u, a);
-                cached_column(sc, (w >> 4) & 15u, b);
+                cached_column(sc, (w >> 14) & 15u, a);
+                cached_column(sc, (w >> 18) & 15u, b);
 #pragma unroll
                 for (int q = 0; q < 4; ++q) a[q] = cmul(detp, a[q]);
                 int k = 0;
@@ -149,22 +150,18 @@ minors_reg_kernel(const c128* __restrict__ P, int64_t st0, int64_t n_st_total, i
 #pragma unroll
                     for (int y = x + 1; y < 4; ++y) c.s[k++] = det2(a[x], b[x], a[y], b[y]);
             }
-            c128 t[4];
-            cached_column(sc, w3 & 15u, t);
-            for (uint32_t q = 0; q < n3; ++q) {
-                third_from(c.s, t, c.c3);
-                const uint32_t mask5 = w3 >> 4;
-                if (q + 1 < n3) {                                     // next third column: in flight during this node's last level
-                    w3 = __ldg(pw + 2 + q);
-                    cached_column(sc, w3 & 15u, t);
-                } else if (pn < pend) {                               // ... or the words of the next pair
-                    w = __ldg(pn);
-                    w3 = __ldg(pn + 1);
-                }
-                finish_all<NC, 3>(c, mask5);
+            third_from(c.s, t, c.c3);
+            const uint32_t mask5 = (w >> 4) & 0x3ffu;
+            ++pw;
+            const bool more = pw < pend;
+            uint32_t w2 = 0;
+            if (more) {
+                cached_column(sc, wn & 15u, t);
+                w2 = __ldg(pw + 1);                                   // two padding words follow the last job's program
             }
-            if (pn >= pend) break;
-            pw = pn;
+            finish_all<NC, 3>(c, mask5);
+            if (!more) break;
+            w = wn; wn = w2;
         }
     }
 }
