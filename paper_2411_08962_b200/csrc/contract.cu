@@ -555,7 +555,7 @@ StagedHost build_staged_host(const wick_terms* t, int n_bins, bool force_complex
             }
         }
         if (h.b_dense.empty()) h.b_dense.push_back(0.0);
-        if (h.md_ids.empty()) h.md_ids.push_back(0);
+        h.md_ids.resize(h.md_ids.size() + 32 * STG_THREADS / 32, 0);  // the kernel requests the next batch's ids one batch ahead, unguarded
     }
     h.ok = true;
     h.sink_ptr = std::move(sink_ptr); h.sink_rdpos = std::move(sink_rdpos); h.src_ptr = std::move(src_ptr); h.src_cupos = std::move(src_cupos);

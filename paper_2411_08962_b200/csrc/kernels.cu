@@ -1138,6 +1138,7 @@ reduce_staged_kernel(const c128* __restrict__ MU, const c128* __restrict__ MD, i
     const c128* MDg = MD + s;
     c128 acc = make_double2(0.0, 0.0);
     const int b0 = __ldg(st.bin_ptr + blockIdx.y), b1 = __ldg(st.bin_ptr + blockIdx.y + 1);
+    int my_id = 0;                                                       // MD element id this lane holds for its warp (see below)
     for (int b = b0; b < b1; ++b) {
         const int4 v0 = __ldg(reinterpret_cast<const int4*>(st.batches + b));
         const int4 v1 = __ldg(reinterpret_cast<const int4*>(st.batches + b) + 1);
@@ -1145,10 +1146,23 @@ reduce_staged_kernel(const c128* __restrict__ MU, const c128* __restrict__ MD, i
         const int cd_a = v0.x, n_cd = v0.y - v0.x, cu_a = v0.z, n_cu = v0.w - v0.z;
         const int rd_a = v1.x, n_rd = v1.y - v1.x, ru_a = v1.z, n_rows = v1.w - v1.z;
         __syncthreads();                                                 // every warp is done with the previous batch
-        {   // MD block: the element ids were laid out on the host (no division, no dependent look-up per element)
+        {   // MD block: the element ids were laid out on the host (no division, no dependent look-up per element).  Warp w copies
+            // the elements w, w + STG_W, ...: lane l fetches the id of the l-th of them (ONE load latency per batch; a load per
+            // element in front of its copy cost the prologue eight dependent L2 round trips) and the ids go round by shuffle
+            static_assert(STG_MD_CAP_REAL <= 32 * STG_W && STG_MD_CAP <= 32 * STG_W, "one id per lane");
+            // The id lists of a bin's batches follow one another in md_ids (padded by 32 * STG_W entries), so the ids of the NEXT
+            // batch are requested here as well and arrive during this batch's arithmetic.
             const int32_t* ids = st.md_ids + v2.x;
-            for (int e = warp; e < n_rd * n_cd; e += STG_W)
-                cp_async16(MDs + e * GROUP + lane, MDg + int64_t(__ldg(ids + e)) * S_b);
+            const int n_el = n_rd * n_cd;
+            const int my_e = warp + STG_W * lane;
+            if (b == b0) my_id = __ldg(ids + my_e);
+            for (int j = 0, e = warp; e < n_el; ++j, e += STG_W)
+                cp_async16(MDs + e * GROUP + lane, MDg + int64_t(__shfl_sync(0xffffffffu, my_id, j)) * S_b);
+            my_id = __ldg(ids + n_el + my_e);
+            if (b + 1 < b1) {                                            // next batch descriptor -> L1
+                asm volatile("prefetch.global.L1 [%0];" ::"l"(st.batches + b + 1));
+                asm volatile("prefetch.global.L1 [%0];" ::"l"(reinterpret_cast<const char*>(st.batches + b + 1) + 32));
+            }
         }
         // coefficient lists of the batch -> shared memory, offsets already in elements of the staged buffers
         const int sp0 = __ldg(st.sink_ptr + ru_a), sp1 = __ldg(st.sink_ptr + ru_a + n_rows);
