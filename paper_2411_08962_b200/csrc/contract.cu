@@ -535,6 +535,8 @@ StagedHost build_staged_host(const wick_terms* t, int n_bins, bool force_complex
     {
         std::map<std::pair<int, int>, int32_t> piece_off;           // (cd_a, cu_a) identifies a piece
         for (StagedBatch& b : batches) {
+            b.sink_a = sink_ptr[size_t(b.ru_a)];                     // the batch's sink entries: no look-up of the range in the kernel
+            b.sink_n = sink_ptr[size_t(b.ru_b)] - b.sink_a;
             b.md_off = int32_t(h.md_ids.size());
             for (int rdi = b.rd_a; rdi < b.rd_b; ++rdi)
                 for (int cdi = b.cd_a; cdi < b.cd_b; ++cdi)

@@ -1165,7 +1165,7 @@ reduce_staged_kernel(const c128* __restrict__ MU, const c128* __restrict__ MD, i
             }
         }
         // coefficient lists of the batch -> shared memory, offsets already in elements of the staged buffers
-        const int sp0 = __ldg(st.sink_ptr + ru_a), sp1 = __ldg(st.sink_ptr + ru_a + n_rows);
+        const int sp0 = v2.z, sp1 = v2.z + v2.w;
         for (int e = threadIdx.x; e < sp1 - sp0; e += STG_THREADS) {
             const c128 cf = __ldg(st.sink_c + sp0 + e);
             const int off = (__ldg(st.sink_rdpos + sp0 + e) - rd_a) * n_cd * GROUP;

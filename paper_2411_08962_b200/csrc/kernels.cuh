@@ -86,7 +86,7 @@ constexpr int stg_md_cap(bool real) { return real ? STG_MD_CAP_REAL : STG_MD_CAP
 // md_off: the batch's MD element ids ((rd, cd) pairs of its block, rd-major) in StagedTables::md_ids; b_off: the dense real
 // B[cu][cd] of its piece in StagedTables::b_dense (real-coefficient schedules).  Both are laid out on the host so that the
 // per-batch prologue of the kernel has no dependent look-ups.
-struct StagedBatch { int32_t cd_a, cd_b, cu_a, cu_b, rd_a, rd_b, ru_a, ru_b, md_off, b_off, pad0, pad1; };
+struct StagedBatch { int32_t cd_a, cd_b, cu_a, cu_b, rd_a, rd_b, ru_a, ru_b, md_off, b_off, sink_a, sink_n; };   // sink_a, sink_n: first sink entry of the batch's rows, their number
 static_assert(sizeof(StagedBatch) == 48, "StagedBatch is read with three 16-byte loads");
 struct StagedTables {
     int n_cols_u, n_cols_d, n_bins;
