@@ -268,7 +268,7 @@ size_t wick_static_scratch_bytes(void);
 /* Step a4 for one flavour (0 = u, 1 = d) of a handle's unique-minor table, through exactly the kernels wick_contract
  * launches for it (the register-resident / cached kernels for the library's own tables; `flags` as for wick_contract).
  * P_dev: device complex128 [n_sites][12][12]; out_dev: device complex128 [n_minors][S] with S = n_sites rounded up to a
- * multiple of 32 (columns >= n_sites are not written).  Enqueues on cuda_stream, does not synchronise. */
+ * multiple of 32 (columns >= n_sites hold the minors of a zero propagator: 0 for n >= 1).  Enqueues on cuda_stream, does not synchronise. */
 int wick_terms_minor_table(const void* P_dev, int64_t n_sites, const wick_terms* terms, int flavour, unsigned flags,
                            void* out_dev, void* cuda_stream);
 
