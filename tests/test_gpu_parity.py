@@ -438,6 +438,31 @@ def test_jacobi_path_on_generic_lists(n_u, n_d, cuda_device):
     _check_C(Cg.cpu().numpy(), wo.reduce_sites(sr, mom, L), sabs.sum(axis=1))
 
 
+def test_jacobi_fused_kernel_long_list_ragged_sites_and_one_propagator(cuda_device):
+    """The fused Jacobi kernel beyond the cases above: a list longer than the 1024 term records it stages in shared memory
+    (the records are then read from global memory), a site count (27) that is no multiple of its 16-site CTAs, and U == D
+    (both lane groups of a site invert the same matrix).  Same launch count as a short list: the fused path was taken."""
+    n_u, n_d, L, T, mom = 9, 10, 3, 1, [(0, 0, 0), (1, 2, 0)]
+    U, D = make_propagators_numpy(977, L, T)
+    Ud, Dd = _dev(U, cuda_device), _dev(D, cuda_device)
+    counts = []
+    for n_terms, same in ((300, False), (1500, False), (1500, True)):
+        lst = make_random_term_list(81, n_u, n_d, n_terms)
+        t = wk.build_terms_from_list(*lst)
+        assert (t.info.n_terms > 1024) == (n_terms > 1024)
+        wk.launch_count(reset=True)
+        Cg, sg = wk.contract(Ud, Ud if same else Dd, t, mom, L, T, want_sigma=True, flags=wk.CONTRACT_JACOBI)
+        sg = sg.cpu().numpy()
+        counts.append(wk.launch_count())
+        Dh = U if same else D
+        sr, sabs = np.zeros((T, L ** 3), complex), np.zeros((T, L ** 3))
+        for x in range(L ** 3):
+            sr[0, x], sabs[0, x] = wo.site_terms_value(U[0, x], Dh[0, x], *lst)
+        assert np.all(np.abs(sg - sr) <= REL_TOL * sabs), (np.abs(sg - sr) / sabs).max()
+        _check_C(Cg.cpu().numpy(), wo.reduce_sites(sr, mom, L), sabs.sum(axis=1))
+    assert counts[0] == counts[1] == counts[2] and counts[0] <= 3, counts
+
+
 def test_correlation_matrix_shares_the_determinants(cuda_device):
     """wick_contract_many (GEVP, Sec. V PAPER.md:394-420): the 2x2 correlation matrix of {p n product operator, Eq. (20)}
     against the oracle's sink x conj(source) expansion for every entry, with the minors launched once for all four."""
