@@ -221,8 +221,8 @@ __device__ __forceinline__ double shfl16(double v, int src) { return __shfl_sync
 // Result of invert12 for one lane and one matrix: row `my_step` of the inverse, entry m belongs to column p_m (4-bit fields of perm).
 struct InvRow { double re[12], im[12]; int my_step; unsigned long long perm; c128 det; bool singular; };
 
-// NM matrices can be inverted TOGETHER (independent instruction streams in one thread); the fused kernel inverts the two
-// flavours one after the other instead, which halves the registers and lets 16 warps per SM hide the latencies.
+// NM matrices can be inverted TOGETHER (independent instruction streams in one thread; inverse12_kernel, the only user
+// left, takes one: the fused kernel has its own four-lanes-per-matrix routine, invert12_rows3 below).
 // The pivot row of a step and the reciprocal of its pivot reach the other lanes of the site by shuffles (52 per step; the
 // round-2 profile showed the LSU data pipe as the limiter, 82 % busy, and a single-lane STS.128 costs it the same four
 // cycles as a full-warp one, so the earlier shared-memory broadcast, 13 stores + 13 loads, was no cheaper).
